@@ -1,0 +1,122 @@
+/* oracle/opmc.h — C interface of the fp64 CPU ORACLE.
+ *
+ * TEST INFRASTRUCTURE ONLY.  Nothing in the product path (paper_1409_8336_b200/,
+ * include/, csrc/) includes, links or calls this.  Only tests/, __graft_entry__.smoke()
+ * and bench.py's cpu_baseline / --impl reference legs may use it.
+ *
+ * The oracle follows arxiv 1409.8336 step by step in fp64, one history at a
+ * time; every place where the paper is silent is resolved by the reading listed in
+ * DESIGN.md ("Readings").  It shares no code with the CUDA path: this header is NOT
+ * include/pmc.h, although the five calls mirror it (host pointers everywhere).
+ *
+ * Parity pins (tests/test_oracle_*.py): Philox known answers; CSDA range vs direct
+ * integration; Eq.1/Eq.2 identity; Highland 1.07*theta0; Fermi-Eyges hinge moments;
+ * straggling cumulants; per-history energy ledger; exact Z/A conservation; Ranft
+ * t-distribution; INC collision-probability closed form; evaporation spectra.
+ * Parity UNPINNED (comparison material missing from the container): agreement with
+ * Chibani's Vavilov sampler (ref [18]), with the INC of ref [13], with Furihata's GEM
+ * (ref [21]) and with any Geant4-derived table.
+ */
+#ifndef OPMC_H
+#define OPMC_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define OPMC_MAX_ELEM 8
+
+typedef struct {                 /* all input data */
+  int32_t n_e; double e_min, e_max;            /* log-uniform kinetic-energy grid, MeV */
+  int32_t n_sr;                                 /* stopping/range tables: 0 water, 1 air, 2 Ti */
+  const double *stop_mass;                      /* [n_sr][n_e] MeV cm2/g */
+  const double *ln_range, *ln_range_d2;         /* [n_sr][n_e] ln R(g/cm2) vs ln E knots + spline y'' */
+  int32_t n_r;
+  const double *ln_r_lo, *ln_r_hi;              /* [n_sr] inverse-table abscissa range (ln g/cm2) */
+  const double *ln_energy, *ln_energy_d2;       /* [n_sr][n_r] ln E vs uniform ln R + spline y'' */
+  int32_t n_elem; const int32_t *elem_z, *elem_a;
+  const double *sigma_ne_mb, *sigma_el_mb;      /* [n_elem][n_e] */
+  int32_t mass_zdim, mass_adim;
+  const double *nuclear_mass;                   /* [zdim][adim] MeV, 0 = not a nuclide */
+  const double *evap_k, *evap_c;                /* [6][zdim] Dostrovsky k_j, c_j vs daughter Z */
+  double e_cut, highland_factor, kappa_gauss, s_max_wet_cm;
+  int32_t n_batches;
+} opmc_tables;
+
+typedef struct {                 /* PAPER.md:L49, Eq.1, Eq.2 */
+  int32_t hu_lo, hu_hi;          /* HU in [hu_lo, hu_hi) */
+  double rho_lo, rho_hi;         /* g/cm3 at hu_lo / hu_hi, linear in between */
+  double w[OPMC_MAX_ELEM];       /* mass fractions over the tables' element list */
+  double f_m;                    /* Eq.1/Eq.2 scaling factor (table_id 0 only) */
+  double x0_gcm2;                /* radiation length */
+  int32_t table_id;              /* 0: water table scaled by Eq.1/2; k>0: own table k, unscaled */
+} opmc_hu_bin;
+
+typedef struct {                 /* PAPER.md:L102-106 restated as a Gaussian spot */
+  double pos_cm[3], dir[3];
+  double e_mev, sigma_e_mev, sigma_x_cm, sigma_y_cm, div_x_rad, div_y_rad, weight;
+} opmc_spot;
+
+typedef struct {
+  int16_t Z, A;                  /* n=(0,1) p=(1,1) d t 3He alpha, residual=(Zr,Ar) */
+  uint8_t origin;                /* 0 INC, 1 evaporation, 2 final residual */
+  uint8_t pad[3];
+  float ke_mev; float dir[3];
+} opmc_secondary;
+
+typedef struct {
+  uint64_t n_steps, n_draws, n_elastic, n_nonelastic, n_secondary_protons, n_missed, n_inc_tries;
+  double e_source, e_deposit, e_escape, e_neutron, e_gamma, e_q, e_air;
+  double max_ledger_residual;    /* max over histories of |E0 - sum of all sinks| (MeV) */
+  double max_event_residual;     /* max |4-momentum imbalance| over INC/evaporation/elastic events */
+  uint64_t n_zab_violations;     /* events where charge or baryon number failed to balance (must be 0) */
+} opmc_counters;
+
+typedef struct opmc_ctx opmc_ctx;
+
+int  opmc_create(opmc_ctx **out);
+void opmc_destroy(opmc_ctx *);
+int  opmc_load_physics_tables(opmc_ctx *, const opmc_tables *);
+int  opmc_set_hu_materials(opmc_ctx *, const opmc_hu_bin *bins, int nbins);
+int  opmc_load_ct(opmc_ctx *, const int16_t *hu, int nx, int ny, int nz,
+                  double dx, double dy, double dz, const double origin[3]);
+/* keys: "straggling" "mcs" "elastic" "nonelastic" (0/1), "s_max_wet_cm", "n_batches", "threads" */
+int  opmc_set_option(opmc_ctx *, const char *key, double value);
+int  opmc_simulate(opmc_ctx *, const opmc_spot *spots, int nspots, uint64_t n_histories, uint64_t seed,
+                   double *dose, double *sigma);
+int  opmc_nonelastic(opmc_ctx *, int Z, int A, double e_mev, uint64_t n, uint64_t seed,
+                     opmc_secondary *out, uint64_t capacity, uint32_t *event_offsets, uint64_t *n_out);
+int  opmc_get_counters(opmc_ctx *, opmc_counters *);
+const char *opmc_last_error(opmc_ctx *);
+
+/* ---- hooks used only by the pin tests ---- */
+void   opmc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
+double opmc_test_range_gcm2(opmc_ctx *, int table, double e_mev);
+double opmc_test_energy_of_range(opmc_ctx *, int table, double r_gcm2);
+/* n straggled losses for a step of wet-path rho*L (g/cm2) in a medium of given <Z/A> */
+int    opmc_test_straggle(opmc_ctx *, double e_mev, double mean_loss, double rhoL_gcm2, double z_over_a,
+                          uint64_t n, uint64_t seed, double *out);
+/* follow n primaries of spot[0] for at most max_steps condensed steps; out[n][8]=x,y,z,u,v,w,E,pathlen */
+int    opmc_test_first_steps(opmc_ctx *, const opmc_spot *spot, uint64_t n, uint64_t seed, int max_steps,
+                             double *out);
+/* n p-A (or p-p when A==1) elastic events at kinetic energy t: out[n][4] = |t| (GeV/c)^2, T_out, T_recoil,
+   opening angle between the two outgoing lab directions (rad) */
+int    opmc_test_elastic(opmc_ctx *, int Z, int A, double t_mev, uint64_t n, uint64_t seed, double *out);
+/* single uniform shell of radius R (fm), nucleon density rho (fm^-3, all neutrons), constant sigma (mb),
+   potentials zero, Pauli off: returns fraction of entries with >= 1 collision */
+double opmc_test_inc_uniform_sphere(double radius_fm, double rho_fm3, double sigma_mb, double t_mev,
+                                    uint64_t n, uint64_t seed);
+/* shells of nucleus (Z,A): out[15][6] = r_out, rho_p, rho_n, pF_p, EF_p, V_p ; returns r_max */
+double opmc_test_nucleus(opmc_ctx *, int Z, int A, double *out);
+/* mean of p^2 over n sampled Fermi partners in the central shell divided by pF^2 (-> 3/5) */
+double opmc_test_fermi_p2(opmc_ctx *, int Z, int A, uint64_t n, uint64_t seed);
+/* evaporation of (Z,A,E*) at rest: widths[6] by quadrature; first emission of n samples restricted to
+   channel_mask (bit j): out_channel[n], out_eps[n]; spectrum[6*64] = the discretised P_j(eps) bins */
+int    opmc_test_evap_first(opmc_ctx *, int Z, int A, double estar, uint32_t channel_mask, uint64_t n,
+                            uint64_t seed, double *widths, int32_t *out_channel, double *out_eps,
+                            double *out_cos);
+double opmc_test_cugnon(int which /*0 sigma_pp,1 sigma_np,2 B_pp,3 B_np,4 a_np*/, double p_gev);
+#ifdef __cplusplus
+}
+#endif
+#endif
