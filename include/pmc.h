@@ -1,0 +1,178 @@
+/* include/pmc.h — C-ABI boundary of libpmc: B200-native condensed-history proton Monte Carlo.
+ *
+ * Hot path of arxiv 1409.8336 (Wan Chan Tseung, Ma, Beltran): proton transport through a CT voxel grid
+ * with continuous energy loss + straggling, multiple Coulomb scattering, nuclear elastic scattering and
+ * non-elastic collisions (intranuclear cascade + evaporation), dose tallied with batch statistical errors.
+ * Citations are "PAPER.md:Lnn (§section)"; "Reading Rk" refers to DESIGN.md.
+ *
+ * Conventions
+ *   - plain C types only; every pointer argument says whether it is HOST or DEVICE memory;
+ *   - all calls return 0 (PMC_OK) or a negative pmc_status; the message is available from pmc_last_error();
+ *   - the context owns its internal device scratch (particle queues, batch tallies, tables);
+ *   - caller-owned device arrays (HU grid, dose, sigma, secondaries) are never freed by the library;
+ *   - every call is synchronous on return (the context's stream is synchronised), so CUDA errors and queue
+ *     overflows surface as the return code; nothing is ever silently dropped;
+ *   - there is NO CPU fallback: without a CUDA device pmc_create() fails with PMC_E_CUDA.
+ *   - call order: pmc_create -> pmc_load_physics_tables -> pmc_set_hu_materials -> pmc_load_ct -> pmc_simulate;
+ *     pmc_nonelastic needs only the physics tables.
+ */
+#ifndef PMC_H
+#define PMC_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define PMC_MAX_ELEM 8
+
+typedef enum {
+  PMC_OK = 0,
+  PMC_E_INVALID_ARG = -1,
+  PMC_E_STATE = -2,        /* call order violated */
+  PMC_E_CAPACITY = -3,     /* an output or internal queue is too small; nothing was truncated silently */
+  PMC_E_CUDA = -4,
+  PMC_E_UNSUPPORTED = -5
+} pmc_status;
+
+/* Physics input tables (HOST pointers, copied at call time).  The paper reads these from Geant4.9.6p2:
+ * dE/dx and CSDA range tables for water, air and titanium with pre-computed cubic-spline second derivatives
+ * (§II.A.2), non-elastic (L75 §II.A.4) and elastic (L83 §II.A.5) cross-section tables, and the
+ * evaporation model's parameters (L79 ref [21]).  Layout: all 2-D arrays are row-major [row][column].
+ * The kinetic-energy grid is log-uniform: E_i = e_min * (e_max/e_min)^(i/(n_e-1)). */
+typedef struct pmc_tables {
+  int32_t n_e; double e_min, e_max;            /* MeV */
+  int32_t n_sr;                                 /* stopping/range media: 0 water, 1 air, 2 titanium */
+  const double *stop_mass;                      /* [n_sr][n_e] MeV cm2/g (informational; the path uses ranges) */
+  const double *ln_range, *ln_range_d2;         /* [n_sr][n_e] ln R(g/cm2) at the knots ln E_i, and spline y'' */
+  int32_t n_r;
+  const double *ln_r_lo, *ln_r_hi;              /* [n_sr] abscissa range of the inverse table, ln(g/cm2) */
+  const double *ln_energy, *ln_energy_d2;       /* [n_sr][n_r] ln E on a uniform ln R grid, and spline y'' */
+  int32_t n_elem; const int32_t *elem_z, *elem_a;   /* one isotope per element (Reading R5) */
+  const double *sigma_ne_mb, *sigma_el_mb;      /* [n_elem][n_e] millibarn, linear in ln E between knots */
+  int32_t mass_zdim, mass_adim;
+  const double *nuclear_mass;                   /* [zdim][adim] ground-state nuclear masses, MeV; 0 = no such nuclide */
+  const double *evap_k, *evap_c;                /* [6][zdim] Dostrovsky k_j, c_j vs daughter Z; j = n,p,d,t,3He,alpha */
+  double e_cut;                                 /* 0.1 MeV */
+  double highland_factor;                       /* 1.07 */
+  double kappa_gauss;                           /* Reading R4: Vavilov kappa above which straggling is Gaussian */
+  double s_max_wet_cm;                          /* Reading R3.2: step cap in g/cm2 of the table medium; <=0: none */
+  int32_t n_batches;                            /* 10 */
+} pmc_tables;
+
+/* One HU bin of the HU -> material conversion (§II.A.1; Eq.1/Eq.2; L59). */
+typedef struct pmc_hu_bin {
+  int32_t hu_lo, hu_hi;          /* HU in [hu_lo, hu_hi); bins sorted and contiguous; HU outside is clamped */
+  double rho_lo, rho_hi;         /* g/cm3 at hu_lo / hu_hi, linear in between */
+  double w[PMC_MAX_ELEM];        /* mass fractions over the element list of pmc_tables (sum 1 within 1e-6) */
+  double f_m;                    /* Eq.1/Eq.2 water-scaling factor (used when table_id == 0) */
+  double x0_gcm2;                /* radiation length */
+  int32_t table_id;              /* 0: water table scaled by Eq.1/Eq.2; k>0: own stopping/range table k, unscaled */
+} pmc_hu_bin;
+
+/* One scanned-beam spot (§II.A.6 restated as a parametric Gaussian spot, Reading R2).
+ * 13 doubles.  The transverse axes are e_x = unit(a x dir), e_y = dir x e_x with a = (0,1,0) if |dir_z| >= 0.9
+ * else (0,0,1). */
+typedef struct pmc_spot {
+  double pos_cm[3];              /* spot centre on the source plane, same frame as the CT origin */
+  double dir[3];                 /* central axis (normalised by the library) */
+  double e_mev, sigma_e_mev;
+  double sigma_x_cm, sigma_y_cm;
+  double div_x_rad, div_y_rad;
+  double weight;                 /* relative number of histories */
+} pmc_spot;
+
+/* One product of a non-elastic collision, 24 bytes. */
+typedef struct pmc_secondary {
+  int16_t Z, A;                  /* n=(0,1) p=(1,1) d=(1,2) t=(1,3) 3He=(2,3) alpha=(2,4); residual=(Z_r,A_r) */
+  uint8_t origin;                /* 0 intranuclear cascade, 1 evaporation, 2 final residual nucleus */
+  uint8_t pad[3];
+  float ke_mev;
+  float dir[3];                  /* unit vector; the incident proton travels along +z */
+} pmc_secondary;
+
+typedef struct pmc_counters {    /* totals of the last pmc_simulate / pmc_nonelastic call */
+  uint64_t n_steps, n_elastic, n_nonelastic, n_secondary_protons, n_missed, n_inc_tries, n_generations;
+  /* energy ledger, MeV: e_source = all the sinks below, up to fp32 rounding */
+  double e_source, e_deposit, e_escape, e_neutron, e_gamma, e_q, e_air;
+  uint64_t n_zab_violations;     /* events whose charge or baryon number failed to balance (must be 0) */
+} pmc_counters;
+
+typedef struct pmc_timing {      /* CUDA-event time (ms) per kernel class over the last pmc_simulate call */
+  float total_ms, sampler_ms, transport_ms, elastic_ms, inc_ms, evaporation_ms, statistics_ms;
+  uint32_t launches_total, launches_transport;
+} pmc_timing;
+
+typedef struct pmc_ctx pmc_ctx;
+
+/* Create a context on CUDA device `device`.  `cuda_stream` is a cudaStream_t owned by the caller (NULL = the
+ * legacy default stream); all kernels of this context are launched on it. */
+int  pmc_create(pmc_ctx **out, int device, void *cuda_stream);
+void pmc_destroy(pmc_ctx *ctx);
+
+/* load the physics tables (HOST, copied).  Builds the device tables and the
+ * 15-shell nucleus models (L77) for every element with A > 1.
+ * Errors: null pointers, sizes out of range, non-monotone range table, element missing from the mass table. */
+int  pmc_load_physics_tables(pmc_ctx *ctx, const pmc_tables *tables_host);
+
+/* HU -> density + composition (HOST array, copied).  Needs the physics tables. */
+int  pmc_set_hu_materials(pmc_ctx *ctx, const pmc_hu_bin *bins_host, int nbins);
+
+/* PAPER.md:L144 "CT geometry in global memory".  hu_dev: DEVICE pointer to nx*ny*nz int16 HU values, x fastest,
+ * then y, then z; BORROWED until the next pmc_load_ct / pmc_load_ct_host / pmc_destroy.  Voxel sizes in cm; origin_cm (HOST, 3 doubles,
+ * may be NULL = 0) is the position of the grid's lower corner in the frame of pmc_spot.pos_cm.
+ * Errors: null pointer, non-positive sizes, nx*ny*nz >= 2^31. */
+int  pmc_load_ct(pmc_ctx *ctx, const int16_t *hu_dev, int nx, int ny, int nz,
+                 double dx_cm, double dy_cm, double dz_cm, const double *origin_cm);
+/* Same with a HOST HU array: copied to a device buffer owned by the context (end-to-end path). */
+int  pmc_load_ct_host(pmc_ctx *ctx, const int16_t *hu_host, int nx, int ny, int nz,
+                      double dx_cm, double dy_cm, double dz_cm, const double *origin_cm);
+
+/* Options: "straggling" "mcs" "elastic" "nonelastic" (0/1), "s_max_wet_cm", "n_batches",
+ * "chunk_histories" (histories per sub-group), "history_offset" (first history id, for sharding
+ * a run over several GPUs), "dose_aggregate" (0/1 warp-aggregated dose atomics). */
+int  pmc_set_option(pmc_ctx *ctx, const char *key, double value);
+
+/* PAPER.md:L134-138 (Fig 2): simulate n_histories primaries drawn from the spot list (HOST, nspots entries),
+ * in n_batches groups; history h uses the Philox4x32-10 stream keyed (seed, h).  dose_dev / sigma_dev: DEVICE
+ * arrays of nx*ny*nz float, overwritten: mean dose in Gy per primary history and its standard error from the
+ * batch-to-batch scatter (Reading R8).  n_histories must be < 2^32 per call.
+ * Errors: PMC_E_STATE (tables/materials/CT missing), PMC_E_CAPACITY (particle queue overflow), PMC_E_CUDA. */
+int  pmc_simulate(pmc_ctx *ctx, const pmc_spot *spots_host, int nspots, uint64_t n_histories, uint64_t seed,
+                  float *dose_dev, float *sigma_dev);
+/* Same with HOST output arrays (device -> host copies included; end-to-end path). */
+int  pmc_simulate_host(pmc_ctx *ctx, const pmc_spot *spots_host, int nspots, uint64_t n_histories, uint64_t seed,
+                       float *dose_host, float *sigma_host);
+
+/* PAPER.md:L75-79, Table I: n standalone non-elastic collisions of a proton of kinetic energy e_mev (along +z)
+ * with nucleus (Z,A): intranuclear cascade then evaporation.  out_dev: DEVICE array of `capacity` records,
+ * grouped by event; event_offsets_dev: DEVICE array of n+1 uint32 (CSR); *n_out_host (HOST) = records needed.
+ * The last record of each event is the final residual nucleus (origin 2).  Event i uses the Philox stream
+ * (seed, i).  Errors: PMC_E_CAPACITY if capacity < *n_out_host (nothing valid is written beyond capacity),
+ * PMC_E_UNSUPPORTED if (Z,A) or its neighbours are not in the mass table. */
+int  pmc_nonelastic(pmc_ctx *ctx, int Z, int A, double e_mev, uint64_t n, uint64_t seed,
+                    pmc_secondary *out_dev, uint64_t capacity, uint32_t *event_offsets_dev, uint64_t *n_out_host);
+
+int  pmc_get_counters(pmc_ctx *ctx, pmc_counters *out_host);
+int  pmc_get_timing(pmc_ctx *ctx, pmc_timing *out_host);
+const char *pmc_last_error(pmc_ctx *ctx);     /* owned by ctx, valid until the next call on ctx */
+
+/* ---- sub-step entry points (device implementations of single steps of the path, used by the parity tests) ---- */
+/* Philox4x32-10 (north_star): in_dev [n][6] = ctr0..3,key0,key1 ; out_dev [n][4]. */
+int  pmc_philox4x32_10(pmc_ctx *ctx, const uint32_t *in_dev, uint64_t n, uint32_t *out_dev);
+/* CSDA range R(E) (g/cm2) of table `table` and its inverse; e_dev/r_dev DEVICE float[n]. */
+int  pmc_range_of_energy(pmc_ctx *ctx, int table, const float *e_dev, uint64_t n, float *r_dev);
+int  pmc_energy_of_range(pmc_ctx *ctx, int table, const float *r_dev, uint64_t n, float *e_dev);
+/* n straggled losses for a step with mean loss mean_loss, mass thickness rhoL (g/cm2), <Z/A>. */
+int  pmc_straggle(pmc_ctx *ctx, double e_mev, double mean_loss, double rhoL_gcm2, double z_over_a,
+                  uint64_t n, uint64_t seed, float *out_dev);
+/* n p-A (p-p if A==1) elastic events: out_dev [n][4] = |t| (GeV/c)^2, T_out, T_recoil,
+ * opening angle (rad). */
+int  pmc_elastic(pmc_ctx *ctx, int Z, int A, double t_mev, uint64_t n, uint64_t seed, float *out_dev);
+/* follow n primaries of spot[0] for at most max_steps condensed steps (no secondaries);
+ * out_dev [n][8] = x,y,z (cm, grid frame), u,v,w, E, path length. */
+int  pmc_first_steps(pmc_ctx *ctx, const pmc_spot *spot_host, uint64_t n, uint64_t seed, int max_steps,
+                     float *out_dev);
+#ifdef __cplusplus
+}
+#endif
+#endif

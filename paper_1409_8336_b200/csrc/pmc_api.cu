@@ -1,0 +1,622 @@
+// pmc_api.cu — libpmc: context, host-side table preparation, the event-based transport scheduler and the C-ABI
+// of include/pmc.h.  No torch types, no CPU fallback: every step of the path runs in the kernels of
+// pmc_transport.cuh / pmc_nuclear.cuh.
+#include "../../include/pmc.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "pmc_device.cuh"
+#include "pmc_transport.cuh"
+#include "pmc_nuclear.cuh"
+
+using namespace pmc;
+
+namespace {
+
+constexpr double NAVO = 6.02214076e23;
+constexpr double PI_D = 3.14159265358979323846;
+
+struct HostMat { pmc_hu_bin b; double zoa; };
+
+template <typename T>
+struct DevBuf {
+  T *p = nullptr; size_t n = 0;
+  cudaError_t alloc(size_t count) {
+    if (count <= n && p) return cudaSuccess;
+    release();
+    cudaError_t e = cudaMalloc(&p, count * sizeof(T));
+    if (e == cudaSuccess) n = count; else p = nullptr;
+    return e;
+  }
+  cudaError_t upload(const std::vector<T> &h, cudaStream_t s) {
+    cudaError_t e = alloc(h.size() ? h.size() : 1);
+    if (e != cudaSuccess) return e;
+    if (h.empty()) return cudaSuccess;
+    return cudaMemcpyAsync(p, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice, s);
+  }
+  void release() { if (p) cudaFree(p); p = nullptr; n = 0; }
+};
+
+struct QueueMem {
+  DevBuf<float> f; DevBuf<int> vox; DevBuf<uint32_t> u; DevBuf<uint32_t> count;
+  Queue q{};
+  cudaError_t alloc(uint32_t cap) {
+    cudaError_t e;
+    if ((e = f.alloc((size_t)cap * 7)) != cudaSuccess) return e;
+    if ((e = vox.alloc(cap)) != cudaSuccess) return e;
+    if ((e = u.alloc((size_t)cap * 4)) != cudaSuccess) return e;
+    if ((e = count.alloc(1)) != cudaSuccess) return e;
+    q.x = f.p; q.y = f.p + cap; q.z = f.p + 2ull * cap; q.u = f.p + 3ull * cap; q.v = f.p + 4ull * cap; q.w = f.p + 5ull * cap;
+    q.e = f.p + 6ull * cap; q.vox = vox.p; q.hist = u.p; q.pid = u.p + cap; q.blk = u.p + 2ull * cap; q.aux = u.p + 3ull * cap;
+    q.count = count.p; q.cap = cap;
+    return cudaSuccess;
+  }
+  void release() { f.release(); vox.release(); u.release(); count.release(); q = Queue{}; }
+};
+
+}  // namespace
+
+struct pmc_ctx {
+  int device = 0; cudaStream_t stream = nullptr;
+  std::string err;
+  // host copies
+  bool have_tables = false, have_mats = false, have_ct = false, tables_dirty = true;
+  int n_e = 0, n_r = 0, n_sr = 0, n_elem = 0, zdim = 0, adim = 0;
+  double e_min = 0, e_max = 0;
+  std::vector<double> h_lnR, h_lnR2, h_lnrlo, h_lnrhi, h_lnE, h_lnE2, h_sne, h_sel, h_mass, h_ek, h_ec;
+  std::vector<int> ez, ea;
+  double e_cut = 0.1, highland = 1.07, kappa_g = 10, s_max = 0.2; int n_batches = 10;
+  bool opt_strag = true, opt_mcs = true, opt_el = true, opt_ne = true; int aggregate = 1;
+  uint64_t chunk = 1u << 21, history_offset = 0;
+  std::vector<HostMat> mats;
+  // device tables
+  DevBuf<float> d_lnR, d_lnR2, d_lnE, d_lnE2, d_sel, d_sne, d_sigbin, d_ek, d_ec;
+  DevBuf<double> d_mass; DevBuf<MatBin> d_bins; DevBuf<uint8_t> d_lut; DevBuf<Nucleus> d_nuc, d_nuc1;
+  std::vector<Nucleus> h_nuc;
+  Tables T{}; Grid G{}; double origin[3] = {0, 0, 0};
+  DevBuf<int16_t> d_hu_own;
+  // scratch
+  QueueMem qa, qb, qel, qne, qres; DevBuf<uint32_t> d_resza; DevBuf<float> d_resp;
+  DevBuf<uint32_t> d_head; DevBuf<Counters> d_cnt; DevBuf<float> d_tally, d_mean, d_m2, d_out;
+  DevBuf<SpotDev> d_spots; DevBuf<double> d_cdf;
+  DevBuf<SecRec> d_slots; DevBuf<uint32_t> d_counts; DevBuf<unsigned long long> d_base;
+  uint32_t *h_pinned = nullptr;     // pinned readback word(s)
+  uint32_t qcap = 0;
+  int n_sm = 148; size_t smem_transport = 0;
+  pmc_counters counters{}; pmc_timing timing{};
+  cudaEvent_t ev[2] = {nullptr, nullptr};
+};
+
+namespace {
+
+int fail(pmc_ctx *c, int code, const std::string &msg) { if (c) c->err = msg; return code; }
+int cuda_fail(pmc_ctx *c, cudaError_t e, const char *where) {
+  return fail(c, PMC_E_CUDA, std::string(where) + ": " + cudaGetErrorString(e));
+}
+#define CK(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) return cuda_fail(c, e__, #call); } while (0)
+
+double h_nmass(const pmc_ctx *c, int z, int a) {
+  return (z < 0 || a < 1 || z >= c->zdim || a >= c->adim || z > a) ? 0.0 : c->h_mass[(size_t)z * c->adim + a];
+}
+
+// Woods-Saxon density approximated by 15 constant-density shells of a two-component Fermi gas.
+// Reading R6.1: c = 1.07 A^(1/3) fm, a = 0.545 fm, r_max at 1 % of the central density, equal radial widths,
+// shell density = volume average (Simpson), normalised to A; V = E_F + separation energy; B_C = 1.44 (Z-1)/r_max.
+Nucleus build_nucleus(const pmc_ctx *c, int Z, int A) {
+  Nucleus n{}; n.Z = Z; n.A = A; n.nshell = NSHELL; n.pauli = 1; n.const_sigma_mb = -1.f;
+  const double c0 = 1.07 * std::cbrt((double)A), a = 0.545, rmax = c0 + a * std::log(99.0), dr = rmax / NSHELL;
+  double avg[NSHELL], tot = 0;
+  auto ws = [&](double r) { return r * r / (1.0 + std::exp((r - c0) / a)); };
+  for (int k = 0; k < NSHELL; ++k) {
+    const double r0 = k * dr, r1 = (k + 1) * dr; const int M = 256; const double h = (r1 - r0) / M;
+    double s = ws(r0) + ws(r1);
+    for (int i = 1; i < M; ++i) s += ws(r0 + i * h) * ((i & 1) ? 4.0 : 2.0);
+    const double integral = s * h / 3.0, vol = 4 * PI_D / 3 * (r1 * r1 * r1 - r0 * r0 * r0);
+    avg[k] = 4 * PI_D * integral / vol; tot += avg[k] * vol; n.rout[k] = (float)r1;
+  }
+  const double sep[2] = {h_nmass(c, Z - 1, A - 1) + MP_D - h_nmass(c, Z, A), h_nmass(c, Z, A - 1) + MN_D - h_nmass(c, Z, A)};
+  for (int k = 0; k < NSHELL; ++k)
+    for (int t = 0; t < 2; ++t) {
+      const double frac = t == 0 ? (double)Z / A : (double)(A - Z) / A, m = t == 0 ? MP_D : MN_D;
+      const double rho = avg[k] * A / tot * frac, pF = 197.3269804 * std::cbrt(3 * PI_D * PI_D * rho);
+      const double EF = std::sqrt(pF * pF + m * m) - m;
+      n.rho[t][k] = (float)rho; n.pF[t][k] = (float)pF; n.EF[t][k] = (float)EF; n.V[t][k] = (float)(EF + sep[t]);
+    }
+  n.rmax = (float)rmax; n.coulomb = (float)(1.44 * (Z - 1) / rmax); n.mass = h_nmass(c, Z, A);
+  return n;
+}
+
+std::vector<float> to_f(const std::vector<double> &v, double scale = 1.0) {
+  std::vector<float> o(v.size());
+  for (size_t i = 0; i < v.size(); ++i) o[i] = (float)(v[i] * scale);
+  return o;
+}
+
+// (re)build every device table that depends on tables + materials + options
+int sync_tables(pmc_ctx *c) {
+  if (!c->tables_dirty) return PMC_OK;
+  cudaStream_t s = c->stream;
+  Tables &T = c->T;
+  T.n_e = c->n_e; T.n_r = c->n_r; T.n_sr = c->n_sr; T.n_elem = c->n_elem; T.zdim = c->zdim; T.adim = c->adim;
+  const double dlne = (std::log(c->e_max) - std::log(c->e_min)) / (c->n_e - 1);
+  T.ln_emin = (float)std::log(c->e_min); T.ln_emax = (float)std::log(c->e_max); T.inv_dlne = (float)(1.0 / dlne);
+  T.e_min = (float)c->e_min; T.e_max = (float)c->e_max;
+  T.e_cut = (float)c->e_cut; T.highland = (float)c->highland; T.kappa_g = (float)c->kappa_g; T.s_max = (float)c->s_max;
+  T.opt_strag = c->opt_strag; T.opt_mcs = c->opt_mcs; T.opt_el = c->opt_el; T.opt_ne = c->opt_ne;
+  CK(c->d_lnR.upload(to_f(c->h_lnR), s)); CK(c->d_lnR2.upload(to_f(c->h_lnR2, dlne * dlne / 6.0), s));
+  std::vector<float> e2(c->h_lnE2.size());
+  for (int t = 0; t < c->n_sr; ++t) {
+    const double h = (c->h_lnrhi[t] - c->h_lnrlo[t]) / (c->n_r - 1);
+    T.lnr_lo[t] = (float)c->h_lnrlo[t]; T.lnr_hi[t] = (float)c->h_lnrhi[t]; T.inv_hr[t] = (float)(1.0 / h);
+    for (int i = 0; i < c->n_r; ++i) e2[(size_t)t * c->n_r + i] = (float)(c->h_lnE2[(size_t)t * c->n_r + i] * h * h / 6.0);
+  }
+  CK(c->d_lnE.upload(to_f(c->h_lnE), s)); CK(c->d_lnE2.upload(e2, s));
+  CK(c->d_sel.upload(to_f(c->h_sel), s)); CK(c->d_sne.upload(to_f(c->h_sne), s));
+  CK(c->d_mass.upload(c->h_mass, s)); CK(c->d_ek.upload(to_f(c->h_ek), s)); CK(c->d_ec.upload(to_f(c->h_ec), s));
+  CK(c->d_nuc.upload(c->h_nuc, s));
+  T.lnR = c->d_lnR.p; T.lnR2 = c->d_lnR2.p; T.lnE = c->d_lnE.p; T.lnE2 = c->d_lnE2.p; T.sig_el = c->d_sel.p; T.sig_ne = c->d_sne.p;
+  T.mass = c->d_mass.p; T.evap_k = c->d_ek.p; T.evap_c = c->d_ec.p; T.nuc = c->d_nuc.p;
+  for (int i = 0; i < MAX_ELEM; ++i) { T.elem_z[i] = i < c->n_elem ? c->ez[i] : 0; T.elem_a[i] = i < c->n_elem ? c->ea[i] : 1; }
+  T.nbins = (int)c->mats.size();
+  if (c->have_mats) {
+    const int nb = T.nbins;
+    std::vector<MatBin> bins(nb); std::vector<float> sig((size_t)nb * c->n_e);
+    for (int b = 0; b < nb; ++b) {
+      const pmc_hu_bin &h = c->mats[b].b; MatBin &m = bins[b];
+      m.hu_lo = (float)h.hu_lo; m.dhu = (float)((double)h.hu_hi - h.hu_lo); m.inv_dhu = (float)(1.0 / ((double)h.hu_hi - h.hu_lo));
+      m.rho_lo = (float)h.rho_lo; m.drho = (float)(h.rho_hi - h.rho_lo);
+      m.wet = h.table_id == 0 ? (float)h.f_m : 1.0f; m.inv_x0 = (float)(1.0 / h.x0_gcm2); m.zoa = (float)c->mats[b].zoa; m.table = h.table_id;
+      for (int i = 0; i < MAX_ELEM; ++i) m.nfac[i] = i < c->n_elem ? (float)(NAVO * h.w[i] / c->ea[i] * 1e-27) : 0.f;
+      // macroscopic cross-section per unit density: a sum of tables that are linear in ln E is linear in ln E
+      for (int k = 0; k < c->n_e; ++k) {
+        double acc = 0;
+        for (int i = 0; i < c->n_elem; ++i) {
+          const double nf = NAVO * h.w[i] / c->ea[i] * 1e-27;
+          if (c->opt_el) acc += nf * c->h_sel[(size_t)i * c->n_e + k];
+          if (c->opt_ne) acc += nf * c->h_sne[(size_t)i * c->n_e + k];
+        }
+        sig[(size_t)b * c->n_e + k] = (float)acc;
+      }
+    }
+    // HU -> bin lookup table over [first bin's upper edge - 1, last bin's lower edge]; HU outside is clamped (L49)
+    const int lo = nb > 1 ? c->mats.front().b.hu_hi - 1 : c->mats.front().b.hu_lo;
+    const int hi = nb > 1 ? c->mats.back().b.hu_lo : c->mats.front().b.hu_lo;
+    std::vector<uint8_t> lut((size_t)(hi - lo + 1));
+    for (int hu = lo, b = 0; hu <= hi; ++hu) { while (b < nb - 1 && hu >= c->mats[b].b.hu_hi) ++b; lut[hu - lo] = (uint8_t)b; }
+    T.hu_lut_lo = lo; T.hu_lut_n = (int)lut.size();
+    CK(c->d_bins.upload(bins, s)); CK(c->d_sigbin.upload(sig, s)); CK(c->d_lut.upload(lut, s));
+    T.bins = c->d_bins.p; T.sig_bin = c->d_sigbin.p; T.hu_lut = c->d_lut.p;
+    c->smem_transport = ((size_t)2 * c->n_sr * c->n_e + (size_t)2 * c->n_sr * c->n_r + (size_t)nb * c->n_e) * 4 + (size_t)nb * sizeof(MatBin) +
+                        lut.size() + 16;
+    if (c->smem_transport > 200 * 1024) return fail(c, PMC_E_UNSUPPORTED, "tables too large for shared-memory staging");
+    CK(cudaFuncSetAttribute(transport_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_transport));
+  }
+  CK(cudaStreamSynchronize(s));
+  c->tables_dirty = false;
+  return PMC_OK;
+}
+
+int ensure_scratch(pmc_ctx *c, uint64_t chunk) {
+  const uint32_t cap = (uint32_t)std::max<uint64_t>(chunk + chunk / 4 + 4096, 8192);
+  if (cap > c->qcap) {
+    CK(c->qa.alloc(cap)); CK(c->qb.alloc(cap)); CK(c->qel.alloc(cap)); CK(c->qne.alloc(cap)); CK(c->qres.alloc(cap));
+    CK(c->d_resza.alloc(cap)); CK(c->d_resp.alloc((size_t)cap * 3));
+    c->qcap = cap;
+  }
+  CK(c->d_head.alloc(1)); CK(c->d_cnt.alloc(1));
+  if (!c->h_pinned) CK(cudaMallocHost(&c->h_pinned, 64));
+  if (!c->ev[0]) { CK(cudaEventCreate(&c->ev[0])); CK(cudaEventCreate(&c->ev[1])); }
+  return PMC_OK;
+}
+
+ResQueue res_queue(pmc_ctx *c) {
+  ResQueue r; r.q = c->qres.q; r.za = c->d_resza.p; r.px = c->d_resp.p; r.py = c->d_resp.p + c->qcap; r.pz = c->d_resp.p + 2ull * c->qcap;
+  return r;
+}
+
+int prepare_spots(pmc_ctx *c, const pmc_spot *spots, int nspots) {
+  std::vector<SpotDev> sd(nspots); std::vector<double> cdf(nspots);
+  double tot = 0;
+  for (int i = 0; i < nspots; ++i) { if (!(spots[i].weight >= 0)) return fail(c, PMC_E_INVALID_ARG, "negative spot weight"); tot += spots[i].weight; }
+  if (!(tot > 0)) return fail(c, PMC_E_INVALID_ARG, "spot weights sum to zero");
+  double acc = 0;
+  for (int i = 0; i < nspots; ++i) {
+    const pmc_spot &s = spots[i]; SpotDev &d = sd[i];
+    double n = std::sqrt(s.dir[0] * s.dir[0] + s.dir[1] * s.dir[1] + s.dir[2] * s.dir[2]);
+    if (!(n > 0)) return fail(c, PMC_E_INVALID_ARG, "zero spot direction");
+    for (int k = 0; k < 3; ++k) d.ax[k] = s.dir[k] / n;
+    const double a[3] = {0.0, std::fabs(d.ax[2]) >= 0.9 ? 1.0 : 0.0, std::fabs(d.ax[2]) >= 0.9 ? 0.0 : 1.0};
+    double ex[3] = {a[1] * d.ax[2] - a[2] * d.ax[1], a[2] * d.ax[0] - a[0] * d.ax[2], a[0] * d.ax[1] - a[1] * d.ax[0]};
+    n = std::sqrt(ex[0] * ex[0] + ex[1] * ex[1] + ex[2] * ex[2]);
+    for (int k = 0; k < 3; ++k) d.ex[k] = ex[k] / n;
+    d.ey[0] = d.ax[1] * d.ex[2] - d.ax[2] * d.ex[1]; d.ey[1] = d.ax[2] * d.ex[0] - d.ax[0] * d.ex[2]; d.ey[2] = d.ax[0] * d.ex[1] - d.ax[1] * d.ex[0];
+    for (int k = 0; k < 3; ++k) d.pos[k] = s.pos_cm[k];
+    d.e = s.e_mev; d.sigma_e = s.sigma_e_mev; d.sx = s.sigma_x_cm; d.sy = s.sigma_y_cm; d.divx = s.div_x_rad; d.divy = s.div_y_rad;
+    acc += s.weight; cdf[i] = acc / tot;
+  }
+  cdf[nspots - 1] = 1.0;
+  CK(c->d_spots.upload(sd, c->stream)); CK(c->d_cdf.upload(cdf, c->stream));
+  return PMC_OK;
+}
+
+struct Timer {
+  pmc_ctx *c; float *acc; bool on;
+  Timer(pmc_ctx *c_, float *a, bool on_) : c(c_), acc(a), on(on_) { if (on) cudaEventRecord(c->ev[0], c->stream); }
+  ~Timer() { if (on) { cudaEventRecord(c->ev[1], c->stream); cudaEventSynchronize(c->ev[1]); float ms = 0; cudaEventElapsedTime(&ms, c->ev[0], c->ev[1]); *acc += ms; } }
+};
+
+// The event-based scheduler (north_star; replaces the paper's transport kernel + Thrust collect/sort, L136):
+// generation loop over compacted queues until every queue is empty.
+int run_generations(pmc_ctx *c, RunParams P, uint32_t n0, bool profile) {
+  cudaStream_t s = c->stream;
+  QueueMem *cur = &c->qa, *nxt = &c->qb;
+  uint32_t n_in = n0;
+  const int grid_t = c->n_sm * 2, grid_e = c->n_sm * 4;
+  ResQueue rq = res_queue(c);
+  while (n_in > 0) {
+    c->counters.n_generations++;
+    CK(cudaMemsetAsync(c->d_head.p, 0, 4, s)); CK(cudaMemsetAsync(nxt->q.count, 0, 4, s));
+    CK(cudaMemsetAsync(c->qel.q.count, 0, 4, s)); CK(cudaMemsetAsync(c->qne.q.count, 0, 4, s)); CK(cudaMemsetAsync(c->qres.q.count, 0, 4, s));
+    { Timer t(c, &c->timing.transport_ms, profile);
+      transport_kernel<<<grid_t, 256, c->smem_transport, s>>>(c->T, c->G, P, cur->q, n_in, c->d_head.p, c->qel.q, c->qne.q, c->d_tally.p, c->d_cnt.p); }
+    c->timing.launches_total++; c->timing.launches_transport++;
+    if (P.dbg_out) break;
+    { Timer t(c, &c->timing.elastic_ms, profile);
+      elastic_kernel<<<grid_e, 256, 0, s>>>(c->T, P, c->qel.q, nxt->q, c->d_tally.p, c->d_cnt.p); }
+    { Timer t(c, &c->timing.inc_ms, profile);
+      inc_kernel<<<c->n_sm * 8, 128, 0, s>>>(c->T, P, c->qne.q, nxt->q, rq, c->d_tally.p, c->d_cnt.p); }
+    { Timer t(c, &c->timing.evaporation_ms, profile);
+      evap_kernel<<<c->n_sm * 8, 128, 0, s>>>(c->T, P, rq, nxt->q, c->d_tally.p, c->d_cnt.p); }
+    c->timing.launches_total += 3;
+    CK(cudaMemcpyAsync(c->h_pinned, nxt->q.count, 4, cudaMemcpyDeviceToHost, s));
+    CK(cudaStreamSynchronize(s));
+    n_in = c->h_pinned[0];
+    if (n_in > c->qcap) return fail(c, PMC_E_CAPACITY, "particle queue overflow (raise chunk capacity / lower chunk_histories)");
+    std::swap(cur, nxt);
+  }
+  return PMC_OK;
+}
+
+int fetch_counters(pmc_ctx *c) {
+  Counters h{};
+  CK(cudaMemcpyAsync(&h, c->d_cnt.p, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  pmc_counters &o = c->counters;
+  o.n_steps = h.n_steps; o.n_elastic = h.n_elastic; o.n_nonelastic = h.n_nonelastic; o.n_secondary_protons = h.n_secondary;
+  o.n_missed = h.n_missed; o.n_inc_tries = h.n_inc_tries; o.n_zab_violations = h.n_zab_bad;
+  o.e_source = h.e_source; o.e_deposit = h.e_deposit; o.e_escape = h.e_escape; o.e_neutron = h.e_neutron; o.e_gamma = h.e_gamma;
+  o.e_q = h.e_q; o.e_air = h.e_air;
+  if (h.overflow) { char b[96]; snprintf(b, sizeof b, "internal queue overflow (mask 0x%x)", h.overflow); return fail(c, PMC_E_CAPACITY, b); }
+  return PMC_OK;
+}
+
+int air_params(pmc_ctx *c, float &rho, float &wf, float &inv_x0, float &zoa, int &table) {
+  // material of HU -1000 (air between the nozzle exit and the CT volume)
+  const HostMat *m = &c->mats.front();
+  for (const HostMat &h : c->mats) if (-1000 >= h.b.hu_lo && -1000 < h.b.hu_hi) m = &h;
+  if (-1000 >= c->mats.back().b.hu_hi) m = &c->mats.back();
+  const int hh = std::min(std::max(-1000, m->b.hu_lo), m->b.hu_hi);
+  const double r = m->b.rho_lo + (m->b.rho_hi - m->b.rho_lo) * (double)(hh - m->b.hu_lo) / (double)(m->b.hu_hi - m->b.hu_lo);
+  rho = (float)r; wf = (float)(m->b.table_id == 0 ? r * m->b.f_m : r); inv_x0 = (float)(1.0 / m->b.x0_gcm2); zoa = (float)m->zoa; table = m->b.table_id;
+  return PMC_OK;
+}
+
+int load_ct_common(pmc_ctx *c, const int16_t *hu_dev, int nx, int ny, int nz, double dx, double dy, double dz, const double *origin) {
+  c->G.hu = hu_dev; c->G.nx = nx; c->G.ny = ny; c->G.nz = nz; c->G.d[0] = (float)dx; c->G.d[1] = (float)dy; c->G.d[2] = (float)dz;
+  c->G.vol = (float)(dx * dy * dz);
+  for (int k = 0; k < 3; ++k) c->G.d[k] = (float)(k == 0 ? dx : k == 1 ? dy : dz);
+  for (int k = 0; k < 3; ++k) c->origin[k] = origin ? origin[k] : 0.0;   // applied on the host to the spot positions
+  c->have_ct = true;
+  return PMC_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int pmc_create(pmc_ctx **out, int device, void *cuda_stream) {
+  if (!out) return PMC_E_INVALID_ARG;
+  *out = nullptr;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev <= 0 || device < 0 || device >= ndev) return PMC_E_CUDA;   // no CPU fallback
+  if (cudaSetDevice(device) != cudaSuccess) return PMC_E_CUDA;
+  pmc_ctx *c = new pmc_ctx();
+  c->device = device; c->stream = (cudaStream_t)cuda_stream;
+  cudaDeviceProp prop{};
+  if (cudaGetDeviceProperties(&prop, device) == cudaSuccess) c->n_sm = prop.multiProcessorCount;
+  *out = c;
+  return PMC_OK;
+}
+
+void pmc_destroy(pmc_ctx *c) {
+  if (!c) return;
+  cudaSetDevice(c->device);
+  cudaStreamSynchronize(c->stream);
+  c->d_lnR.release(); c->d_lnR2.release(); c->d_lnE.release(); c->d_lnE2.release(); c->d_sel.release(); c->d_sne.release();
+  c->d_sigbin.release(); c->d_ek.release(); c->d_ec.release(); c->d_mass.release(); c->d_bins.release(); c->d_lut.release();
+  c->d_nuc.release(); c->d_nuc1.release(); c->d_hu_own.release();
+  c->qa.release(); c->qb.release(); c->qel.release(); c->qne.release(); c->qres.release(); c->d_resza.release(); c->d_resp.release();
+  c->d_head.release(); c->d_cnt.release(); c->d_tally.release(); c->d_mean.release(); c->d_m2.release(); c->d_out.release();
+  c->d_spots.release(); c->d_cdf.release(); c->d_slots.release(); c->d_counts.release(); c->d_base.release();
+  if (c->h_pinned) cudaFreeHost(c->h_pinned);
+  if (c->ev[0]) { cudaEventDestroy(c->ev[0]); cudaEventDestroy(c->ev[1]); }
+  delete c;
+}
+
+const char *pmc_last_error(pmc_ctx *c) { return c ? c->err.c_str() : "null context"; }
+
+int pmc_load_physics_tables(pmc_ctx *c, const pmc_tables *t) {
+  if (!c || !t) return fail(c, PMC_E_INVALID_ARG, "null argument");
+  if (!t->stop_mass || !t->ln_range || !t->ln_range_d2 || !t->ln_r_lo || !t->ln_r_hi || !t->ln_energy || !t->ln_energy_d2 ||
+      !t->elem_z || !t->elem_a || !t->sigma_ne_mb || !t->sigma_el_mb || !t->nuclear_mass || !t->evap_k || !t->evap_c)
+    return fail(c, PMC_E_INVALID_ARG, "null table pointer");
+  if (t->n_e < 4 || t->n_r < 4 || t->n_sr < 1 || t->n_sr > 4 || t->n_elem < 1 || t->n_elem > PMC_MAX_ELEM || t->mass_zdim < 3 ||
+      t->mass_adim < 5 || !(t->e_min > 0) || !(t->e_max > t->e_min))
+    return fail(c, PMC_E_INVALID_ARG, "bad table sizes");
+  cudaSetDevice(c->device);
+  c->n_e = t->n_e; c->n_r = t->n_r; c->n_sr = t->n_sr; c->n_elem = t->n_elem; c->zdim = t->mass_zdim; c->adim = t->mass_adim;
+  c->e_min = t->e_min; c->e_max = t->e_max;
+  auto cp = [](std::vector<double> &v, const double *p, size_t n) { v.assign(p, p + n); };
+  cp(c->h_lnR, t->ln_range, (size_t)c->n_sr * c->n_e); cp(c->h_lnR2, t->ln_range_d2, (size_t)c->n_sr * c->n_e);
+  cp(c->h_lnrlo, t->ln_r_lo, c->n_sr); cp(c->h_lnrhi, t->ln_r_hi, c->n_sr);
+  cp(c->h_lnE, t->ln_energy, (size_t)c->n_sr * c->n_r); cp(c->h_lnE2, t->ln_energy_d2, (size_t)c->n_sr * c->n_r);
+  cp(c->h_sne, t->sigma_ne_mb, (size_t)c->n_elem * c->n_e); cp(c->h_sel, t->sigma_el_mb, (size_t)c->n_elem * c->n_e);
+  cp(c->h_mass, t->nuclear_mass, (size_t)c->zdim * c->adim); cp(c->h_ek, t->evap_k, (size_t)6 * c->zdim); cp(c->h_ec, t->evap_c, (size_t)6 * c->zdim);
+  c->ez.assign(t->elem_z, t->elem_z + c->n_elem); c->ea.assign(t->elem_a, t->elem_a + c->n_elem);
+  for (int s = 0; s < c->n_sr; ++s) {
+    for (int i = 1; i < c->n_e; ++i)
+      if (!(c->h_lnR[(size_t)s * c->n_e + i] > c->h_lnR[(size_t)s * c->n_e + i - 1])) return fail(c, PMC_E_INVALID_ARG, "range table not monotone");
+    if (!(c->h_lnrhi[s] > c->h_lnrlo[s])) return fail(c, PMC_E_INVALID_ARG, "inverse range table abscissa not increasing");
+  }
+  c->e_cut = t->e_cut; c->highland = t->highland_factor; c->kappa_g = t->kappa_gauss; c->s_max = t->s_max_wet_cm; c->n_batches = t->n_batches;
+  c->h_nuc.assign(c->n_elem, Nucleus{});
+  for (int i = 0; i < c->n_elem; ++i) {
+    if (c->ea[i] < 1 || c->ez[i] < 0 || c->ez[i] > c->ea[i]) return fail(c, PMC_E_INVALID_ARG, "bad element");
+    if (h_nmass(c, c->ez[i], c->ea[i]) <= 0) return fail(c, PMC_E_INVALID_ARG, "element missing from mass table");
+    if (c->ea[i] > 1) {
+      if (h_nmass(c, c->ez[i] - 1, c->ea[i] - 1) <= 0 || h_nmass(c, c->ez[i], c->ea[i] - 1) <= 0)
+        return fail(c, PMC_E_INVALID_ARG, "element's neighbours missing from mass table");
+      c->h_nuc[i] = build_nucleus(c, c->ez[i], c->ea[i]);
+    }
+  }
+  c->have_tables = true; c->have_mats = false; c->mats.clear(); c->tables_dirty = true;
+  return sync_tables(c);
+}
+
+int pmc_set_hu_materials(pmc_ctx *c, const pmc_hu_bin *b, int n) {
+  if (!c || !b || n < 1) return fail(c, PMC_E_INVALID_ARG, "null/empty materials");
+  if (!c->have_tables) return fail(c, PMC_E_STATE, "load physics tables first");
+  if (n > 255) return fail(c, PMC_E_UNSUPPORTED, "at most 255 HU bins");
+  cudaSetDevice(c->device);
+  std::vector<HostMat> mats;
+  for (int i = 0; i < n; ++i) {
+    if (b[i].hu_hi <= b[i].hu_lo || (i > 0 && b[i].hu_lo != b[i - 1].hu_hi)) return fail(c, PMC_E_INVALID_ARG, "bins must be sorted and contiguous");
+    double sw = 0; for (int k = 0; k < PMC_MAX_ELEM; ++k) { if (b[i].w[k] < 0) return fail(c, PMC_E_INVALID_ARG, "negative mass fraction"); sw += b[i].w[k]; }
+    if (std::fabs(sw - 1) > 1e-6) return fail(c, PMC_E_INVALID_ARG, "mass fractions must sum to 1");
+    for (int k = c->n_elem; k < PMC_MAX_ELEM; ++k) if (b[i].w[k] != 0) return fail(c, PMC_E_INVALID_ARG, "mass fraction on an element without cross-section rows");
+    if (b[i].table_id < 0 || b[i].table_id >= c->n_sr) return fail(c, PMC_E_INVALID_ARG, "bad table id");
+    if (!(b[i].rho_lo > 0) || !(b[i].rho_hi > 0) || !(b[i].x0_gcm2 > 0) || (b[i].table_id == 0 && !(b[i].f_m > 0))) return fail(c, PMC_E_INVALID_ARG, "non-positive density, f_m or X0");
+    HostMat m; m.b = b[i]; m.zoa = 0;
+    for (int k = 0; k < c->n_elem; ++k) m.zoa += b[i].w[k] * c->ez[k] / c->ea[k];
+    mats.push_back(m);
+  }
+  if ((long long)mats.back().b.hu_lo - mats.front().b.hu_hi > 70000) return fail(c, PMC_E_UNSUPPORTED, "HU span too large");
+  c->mats = mats; c->have_mats = true; c->tables_dirty = true;
+  return sync_tables(c);
+}
+
+static int check_grid(pmc_ctx *c, const void *hu, int nx, int ny, int nz, double dx, double dy, double dz) {
+  if (!c || !hu) return fail(c, PMC_E_INVALID_ARG, "null argument");
+  if (nx < 1 || ny < 1 || nz < 1 || !(dx > 0) || !(dy > 0) || !(dz > 0) || (double)nx * ny * nz >= 2147483648.0) return fail(c, PMC_E_INVALID_ARG, "bad grid");
+  return PMC_OK;
+}
+
+int pmc_load_ct(pmc_ctx *c, const int16_t *hu_dev, int nx, int ny, int nz, double dx, double dy, double dz, const double *origin) {
+  int rc = check_grid(c, hu_dev, nx, ny, nz, dx, dy, dz); if (rc) return rc;
+  cudaSetDevice(c->device);
+  cudaPointerAttributes attr{};
+  if (cudaPointerGetAttributes(&attr, hu_dev) != cudaSuccess || (attr.type != cudaMemoryTypeDevice && attr.type != cudaMemoryTypeManaged)) {
+    cudaGetLastError();
+    return fail(c, PMC_E_INVALID_ARG, "pmc_load_ct needs a device pointer (use pmc_load_ct_host for host arrays)");
+  }
+  return load_ct_common(c, hu_dev, nx, ny, nz, dx, dy, dz, origin);
+}
+
+int pmc_load_ct_host(pmc_ctx *c, const int16_t *hu_host, int nx, int ny, int nz, double dx, double dy, double dz, const double *origin) {
+  int rc = check_grid(c, hu_host, nx, ny, nz, dx, dy, dz); if (rc) return rc;
+  cudaSetDevice(c->device);
+  const size_t nv = (size_t)nx * ny * nz;
+  CK(c->d_hu_own.alloc(nv));
+  CK(cudaMemcpyAsync(c->d_hu_own.p, hu_host, nv * sizeof(int16_t), cudaMemcpyHostToDevice, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  return load_ct_common(c, c->d_hu_own.p, nx, ny, nz, dx, dy, dz, origin);
+}
+
+int pmc_set_option(pmc_ctx *c, const char *key, double v) {
+  if (!c || !key) return fail(c, PMC_E_INVALID_ARG, "null argument");
+  const std::string k(key);
+  if (k == "straggling") c->opt_strag = v != 0; else if (k == "mcs") c->opt_mcs = v != 0;
+  else if (k == "elastic") c->opt_el = v != 0; else if (k == "nonelastic") c->opt_ne = v != 0;
+  else if (k == "s_max_wet_cm") c->s_max = v; else if (k == "n_batches") { if (v < 2) return fail(c, PMC_E_INVALID_ARG, "need >= 2 batches"); c->n_batches = (int)v; }
+  else if (k == "chunk_histories") { if (v < 1 || v > 67108864.0) return fail(c, PMC_E_INVALID_ARG, "chunk_histories out of range"); c->chunk = (uint64_t)v; }
+  else if (k == "history_offset") { if (v < 0) return fail(c, PMC_E_INVALID_ARG, "negative offset"); c->history_offset = (uint64_t)v; }
+  else if (k == "dose_aggregate") c->aggregate = v != 0;
+  else return fail(c, PMC_E_INVALID_ARG, "unknown option");
+  c->tables_dirty = true;
+  return PMC_OK;
+}
+
+static int simulate_impl(pmc_ctx *c, const pmc_spot *spots_in, int nspots, uint64_t n, uint64_t seed, float *dose_dev, float *sigma_dev,
+                         int max_steps, float *dbg_out) {
+  if (!c || !spots_in || nspots < 1) return fail(c, PMC_E_INVALID_ARG, "null argument");
+  if (!c->have_tables || !c->have_mats || !c->have_ct) return fail(c, PMC_E_STATE, "call order: tables, materials, ct, simulate");
+  if (n >= 4294967296ull) return fail(c, PMC_E_UNSUPPORTED, "n_histories must be < 2^32 per call");
+  cudaSetDevice(c->device);
+  int rc = sync_tables(c); if (rc) return rc;
+  const int B = dbg_out ? 1 : c->n_batches;
+  if (!dbg_out && B < 2) return fail(c, PMC_E_INVALID_ARG, "need >= 2 batches");
+  // spot positions into the grid frame
+  std::vector<pmc_spot> spots(spots_in, spots_in + nspots);
+  for (auto &s : spots) for (int k = 0; k < 3; ++k) s.pos_cm[k] -= c->origin[k];
+  rc = prepare_spots(c, spots.data(), nspots); if (rc) return rc;
+  const uint64_t per_batch = (n + B - 1) / B;
+  const uint64_t chunk = std::max<uint64_t>(1, std::min<uint64_t>(c->chunk, std::max<uint64_t>(per_batch, 1)));
+  rc = ensure_scratch(c, chunk); if (rc) return rc;
+  const uint32_t nvox = (uint32_t)((size_t)c->G.nx * c->G.ny * c->G.nz);
+  CK(c->d_tally.alloc(nvox)); CK(c->d_mean.alloc(nvox)); CK(c->d_m2.alloc(nvox));
+  cudaStream_t s = c->stream;
+  CK(cudaMemsetAsync(c->d_tally.p, 0, (size_t)nvox * 4, s)); CK(cudaMemsetAsync(c->d_cnt.p, 0, sizeof(Counters), s));
+  c->counters = pmc_counters{}; c->timing = pmc_timing{};
+  float air_rho, air_wf, air_ix0, air_zoa; int air_tab; air_params(c, air_rho, air_wf, air_ix0, air_zoa, air_tab);
+  const bool profile = false;
+  cudaEvent_t e0, e1; CK(cudaEventCreate(&e0)); CK(cudaEventCreate(&e1));
+  CK(cudaEventRecord(e0, s));
+  const int grid_v = c->n_sm * 8;
+  for (int b = 0; b < B; ++b) {                                  // PAPER.md:L134 "10 groups of N/10"
+    const uint64_t h0 = (uint64_t)(((unsigned __int128)b * n + B - 1) / B), h1 = (uint64_t)(((unsigned __int128)(b + 1) * n + B - 1) / B);
+    for (uint64_t cs = h0; cs < h1; cs += chunk) {               // sub-groups (L134)
+      const uint32_t nc = (uint32_t)std::min<uint64_t>(chunk, h1 - cs);
+      RunParams P{}; P.seed = seed; P.hist0 = c->history_offset + cs; P.n = nc; P.max_steps = max_steps; P.dbg_out = dbg_out ? dbg_out + 8ull * (cs - h0) : nullptr;
+      P.aggregate = c->aggregate;
+      CK(cudaMemsetAsync(c->qa.q.count, 0, 4, s));
+      sampler_kernel<<<(nc + 255) / 256, 256, 0, s>>>(c->T, c->G, c->d_spots.p, c->d_cdf.p, nspots, P, c->qa.q, c->d_cnt.p, air_rho, air_wf, air_ix0, air_zoa, air_tab);
+      c->timing.launches_total++;
+      CK(cudaMemcpyAsync(c->h_pinned, c->qa.q.count, 4, cudaMemcpyDeviceToHost, s));
+      CK(cudaStreamSynchronize(s));
+      rc = run_generations(c, P, std::min(c->h_pinned[0], c->qcap), profile); if (rc) { cudaEventDestroy(e0); cudaEventDestroy(e1); return rc; }
+    }
+    if (!dbg_out) {
+      const float inv_nb = h1 > h0 ? (float)(1.0 / (double)(h1 - h0)) : 0.f;
+      fold_kernel<<<grid_v, 256, 0, s>>>(c->T, c->G, c->d_tally.p, c->d_mean.p, c->d_m2.p, b, inv_nb, nvox);
+      c->timing.launches_total++;
+    }
+  }
+  if (!dbg_out) { finish_kernel<<<grid_v, 256, 0, s>>>(c->d_mean.p, c->d_m2.p, dose_dev, sigma_dev, B, nvox); c->timing.launches_total++; }
+  CK(cudaEventRecord(e1, s));
+  CK(cudaGetLastError());
+  rc = fetch_counters(c);
+  float ms = 0; cudaEventElapsedTime(&ms, e0, e1); c->timing.total_ms = ms;
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  return rc;
+}
+
+int pmc_simulate(pmc_ctx *c, const pmc_spot *spots, int nspots, uint64_t n, uint64_t seed, float *dose_dev, float *sigma_dev) {
+  if (!dose_dev || !sigma_dev) return fail(c, PMC_E_INVALID_ARG, "null output");
+  return simulate_impl(c, spots, nspots, n, seed, dose_dev, sigma_dev, 0, nullptr);
+}
+
+int pmc_simulate_host(pmc_ctx *c, const pmc_spot *spots, int nspots, uint64_t n, uint64_t seed, float *dose_host, float *sigma_host) {
+  if (!c || !dose_host || !sigma_host) return fail(c, PMC_E_INVALID_ARG, "null output");
+  if (!c->have_ct) return fail(c, PMC_E_STATE, "call order: tables, materials, ct, simulate");
+  cudaSetDevice(c->device);
+  const size_t nvox = (size_t)c->G.nx * c->G.ny * c->G.nz;
+  CK(c->d_out.alloc(2 * nvox));
+  int rc = simulate_impl(c, spots, nspots, n, seed, c->d_out.p, c->d_out.p + nvox, 0, nullptr); if (rc) return rc;
+  CK(cudaMemcpyAsync(dose_host, c->d_out.p, nvox * 4, cudaMemcpyDeviceToHost, c->stream));
+  CK(cudaMemcpyAsync(sigma_host, c->d_out.p + nvox, nvox * 4, cudaMemcpyDeviceToHost, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  return PMC_OK;
+}
+
+int pmc_first_steps(pmc_ctx *c, const pmc_spot *spot, uint64_t n, uint64_t seed, int max_steps, float *out_dev) {
+  if (!out_dev || max_steps < 1) return fail(c, PMC_E_INVALID_ARG, "bad argument");
+  if (c) { cudaSetDevice(c->device); cudaMemsetAsync(out_dev, 0, n * 8 * sizeof(float), c->stream); }
+  return simulate_impl(c, spot, 1, n, seed, nullptr, nullptr, max_steps, out_dev);
+}
+
+int pmc_nonelastic(pmc_ctx *c, int Z, int A, double e_mev, uint64_t n, uint64_t seed, pmc_secondary *out_dev, uint64_t capacity,
+                   uint32_t *off_dev, uint64_t *n_out_host) {
+  if (!c || !off_dev || !n_out_host || (!out_dev && capacity > 0)) return fail(c, PMC_E_INVALID_ARG, "null argument");
+  if (!c->have_tables) return fail(c, PMC_E_STATE, "load physics tables first");
+  if (A < 2 || h_nmass(c, Z, A) <= 0 || h_nmass(c, Z - 1, A - 1) <= 0 || h_nmass(c, Z, A - 1) <= 0) return fail(c, PMC_E_UNSUPPORTED, "unsupported target");
+  if (!(e_mev > 0)) return fail(c, PMC_E_INVALID_ARG, "non-positive energy");
+  cudaSetDevice(c->device);
+  int rc = sync_tables(c); if (rc) return rc;
+  cudaStream_t s = c->stream;
+  std::vector<Nucleus> hn(1, build_nucleus(c, Z, A));
+  CK(c->d_nuc1.upload(hn, s));
+  const uint32_t CH = 1u << 17;
+  CK(c->d_slots.alloc((size_t)CH * MAX_SEC)); CK(c->d_counts.alloc(CH)); CK(c->d_base.alloc(1)); CK(c->d_cnt.alloc(1));
+  CK(cudaMemsetAsync(c->d_cnt.p, 0, sizeof(Counters), s)); CK(cudaMemsetAsync(c->d_base.p, 0, 8, s));
+  c->counters = pmc_counters{};
+  for (uint64_t ev0 = 0; ev0 < n; ev0 += CH) {
+    const uint32_t nc = (uint32_t)std::min<uint64_t>(CH, n - ev0);
+    nonelastic_kernel<<<(nc + 127) / 128, 128, 0, s>>>(c->T, c->d_nuc1.p, (float)e_mev, seed, ev0, nc, c->d_slots.p, c->d_counts.p, c->d_cnt.p);
+    scan_kernel<<<1, 1024, 0, s>>>(c->d_counts.p, nc, off_dev + ev0, c->d_base.p);
+    compact_kernel<<<(nc + 255) / 256, 256, 0, s>>>(c->d_slots.p, c->d_counts.p, off_dev + ev0, nc, reinterpret_cast<SecRec *>(out_dev), capacity);
+  }
+  unsigned long long total = 0;
+  CK(cudaMemcpyAsync(&total, c->d_base.p, 8, cudaMemcpyDeviceToHost, s));
+  CK(cudaStreamSynchronize(s));
+  if (total >= 4294967296ull) return fail(c, PMC_E_UNSUPPORTED, "more than 2^32 records: split the call");
+  const uint32_t t32 = (uint32_t)total;
+  CK(cudaMemcpyAsync(off_dev + n, &t32, 4, cudaMemcpyHostToDevice, s));
+  CK(cudaStreamSynchronize(s));
+  CK(cudaGetLastError());
+  *n_out_host = total;
+  rc = fetch_counters(c); if (rc) return rc;
+  c->counters.n_nonelastic = n;
+  if (total > capacity) return fail(c, PMC_E_CAPACITY, "capacity too small");
+  return PMC_OK;
+}
+
+int pmc_get_counters(pmc_ctx *c, pmc_counters *o) { if (!c || !o) return PMC_E_INVALID_ARG; *o = c->counters; return PMC_OK; }
+int pmc_get_timing(pmc_ctx *c, pmc_timing *o) { if (!c || !o) return PMC_E_INVALID_ARG; *o = c->timing; return PMC_OK; }
+
+// ---- sub-step entry points
+int pmc_philox4x32_10(pmc_ctx *c, const uint32_t *in_dev, uint64_t n, uint32_t *out_dev) {
+  if (!c || !in_dev || !out_dev) return fail(c, PMC_E_INVALID_ARG, "null argument");
+  cudaSetDevice(c->device);
+  if (n) philox_kernel<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(in_dev, n, out_dev);
+  CK(cudaStreamSynchronize(c->stream)); CK(cudaGetLastError());
+  return PMC_OK;
+}
+static int range_impl(pmc_ctx *c, int table, const float *in, uint64_t n, float *out, int inverse) {
+  if (!c || !in || !out) return fail(c, PMC_E_INVALID_ARG, "null argument");
+  if (!c->have_tables) return fail(c, PMC_E_STATE, "load physics tables first");
+  if (table < 0 || table >= c->n_sr) return fail(c, PMC_E_INVALID_ARG, "bad table id");
+  cudaSetDevice(c->device);
+  int rc = sync_tables(c); if (rc) return rc;
+  if (n) range_kernel<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(c->T, table, in, n, out, inverse);
+  CK(cudaStreamSynchronize(c->stream)); CK(cudaGetLastError());
+  return PMC_OK;
+}
+int pmc_range_of_energy(pmc_ctx *c, int table, const float *e_dev, uint64_t n, float *r_dev) { return range_impl(c, table, e_dev, n, r_dev, 0); }
+int pmc_energy_of_range(pmc_ctx *c, int table, const float *r_dev, uint64_t n, float *e_dev) { return range_impl(c, table, r_dev, n, e_dev, 1); }
+
+int pmc_straggle(pmc_ctx *c, double e, double mean, double rhoL, double zoa, uint64_t n, uint64_t seed, float *out_dev) {
+  if (!c || !out_dev) return fail(c, PMC_E_INVALID_ARG, "null argument");
+  if (!c->have_tables) return fail(c, PMC_E_STATE, "load physics tables first");
+  cudaSetDevice(c->device);
+  int rc = sync_tables(c); if (rc) return rc;
+  if (n) straggle_kernel<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(c->T, (float)e, (float)mean, (float)rhoL, (float)zoa, n, seed, out_dev);
+  CK(cudaStreamSynchronize(c->stream)); CK(cudaGetLastError());
+  return PMC_OK;
+}
+
+}  // extern "C"
+
+namespace pmc {
+__global__ void elastic_test_kernel(int A, float M, float tk, uint64_t n, uint64_t seed, float *out) {
+  const uint64_t i = blockIdx.x * (uint64_t)blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  Rng g; g.init(seed, i, 0u, 0u);
+  const ElasticOut o = elastic_event(A, M, tk, g.next4());
+  out[4 * i] = o.t_gev2; out[4 * i + 1] = o.T_out; out[4 * i + 2] = o.T_rec;
+  out[4 * i + 3] = acosf(fminf(1.f, fmaxf(-1.f, dot(o.dir_out, o.dir_rec))));
+}
+}  // namespace pmc
+
+extern "C" int pmc_elastic(pmc_ctx *c, int Z, int A, double t_mev, uint64_t n, uint64_t seed, float *out_dev) {
+  if (!c || !out_dev) return fail(c, PMC_E_INVALID_ARG, "null argument");
+  if (!c->have_tables) return fail(c, PMC_E_STATE, "load physics tables first");
+  if (h_nmass(c, Z, A) <= 0) return fail(c, PMC_E_UNSUPPORTED, "unsupported target");
+  cudaSetDevice(c->device);
+  if (n) pmc::elastic_test_kernel<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(A, (float)h_nmass(c, Z, A), (float)t_mev, n, seed, out_dev);
+  CK(cudaStreamSynchronize(c->stream)); CK(cudaGetLastError());
+  return PMC_OK;
+}

@@ -1,0 +1,291 @@
+// pmc_device.cuh — device-side building blocks shared by the kernels of libpmc (sm_100a).
+//
+// Philox4x32-10 counter-based RNG, fp32 table evaluation (range spline and its inverse, cross-section lerp),
+// direction rotation, Lorentz boosts, the SoA particle queue with warp-aggregated push, and the energy-loss
+// straggling sampler.  Citations: PAPER.md line + section; "Reading Rk" = DESIGN.md.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace pmc {
+
+constexpr float MP = 938.27208816f, MN = 939.56542052f, ME = 0.51099895f;
+constexpr double MP_D = 938.27208816, MN_D = 939.56542052;
+constexpr float HBARC = 197.3269804f;           // MeV fm
+constexpr float KBETHE = 0.307075f;             // MeV cm2/mol
+constexpr float TWO_PI = 6.2831853071795865f;
+constexpr int NSHELL = 15;                      // PAPER.md:L77 "15 constant density shells"
+constexpr int MAX_ELEM = 8;
+constexpr float BIG = 1e30f;
+
+// ------------------------------------------------------------------ Philox4x32-10 (north_star; Reading R0)
+__device__ __forceinline__ uint4 philox4x32_10(uint4 c, uint2 k) {
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    const uint64_t p0 = (uint64_t)0xD2511F53u * c.x, p1 = (uint64_t)0xCD9E8D57u * c.z;
+    c = make_uint4((uint32_t)(p1 >> 32) ^ c.y ^ k.x, (uint32_t)p1, (uint32_t)(p0 >> 32) ^ c.w ^ k.y, (uint32_t)p0);
+    k.x += 0x9E3779B9u; k.y += 0xBB67AE85u;
+  }
+  return c;
+}
+
+// Per-particle stream: key = seed, counter = (history_lo, history_hi, particle id, block number).  Draws are
+// handed out a block (4 words) at a time, so the only state that travels with a particle is `blk`.
+struct Rng {
+  uint2 key; uint32_t h0, h1, pid, blk;
+  __device__ __forceinline__ void init(uint64_t seed, uint64_t hist, uint32_t pid_, uint32_t blk_) {
+    key = make_uint2((uint32_t)seed, (uint32_t)(seed >> 32));
+    h0 = (uint32_t)hist; h1 = (uint32_t)(hist >> 32); pid = pid_; blk = blk_;
+  }
+  __device__ __forceinline__ uint4 next4() { return philox4x32_10(make_uint4(h0, h1, pid, blk++), key); }
+  // id of the k-th product of this particle's current event: a block with the top counter bit set is never a
+  // draw block (blk < 2^31), so the child stream is decorrelated from every draw of the parent.
+  __device__ __forceinline__ uint32_t child_id(uint32_t k) const {
+    return philox4x32_10(make_uint4(h0, h1, pid, 0x80000000u | blk), key).x ^ (k + 1u);
+  }
+};
+__device__ __forceinline__ float u01(uint32_t x) { return ((float)(x >> 8) + 0.5f) * (1.0f / 16777216.0f); }   // (0,1)
+
+// ------------------------------------------------------------------ device tables
+struct MatBin {                 // one HU bin, 16 floats
+  float hu_lo, inv_dhu, dhu, rho_lo, drho;
+  float wet;                    // f_m of Eq.1/Eq.2 (L55-63) for table 0, 1 for own tables
+  float inv_x0, zoa;
+  int table;
+  float nfac[MAX_ELEM];         // N_A w_i / A_i * 1e-27 : (cm^2/g) per mb of element i
+};
+
+struct Nucleus {                // PAPER.md:L77, Reading R6.1; type 0 = proton, 1 = neutron
+  int Z, A, nshell;
+  float rmax, coulomb;
+  float rout[NSHELL], rho[2][NSHELL], pF[2][NSHELL], EF[2][NSHELL], V[2][NSHELL];
+  double mass;                  // target ground-state mass
+  int pauli; float const_sigma_mb;
+};
+
+struct Tables {
+  int n_e, n_r, n_sr, n_elem, nbins, zdim, adim;
+  float ln_emin, ln_emax, inv_dlne, e_min, e_max;
+  float e_cut, highland, kappa_g, s_max;
+  float lnr_lo[4], lnr_hi[4], inv_hr[4];
+  int hu_lut_lo, hu_lut_n;
+  int opt_strag, opt_mcs, opt_el, opt_ne;
+  const float *lnR, *lnR2;      // [n_sr][n_e]; y'' pre-multiplied by h^2/6
+  const float *lnE, *lnE2;      // [n_sr][n_r]
+  const float *sig_el, *sig_ne; // [n_elem][n_e] mb
+  const float *sig_bin;         // [nbins][n_e] total macroscopic cross-section per unit density, cm^2/g
+  const MatBin *bins;           // [nbins]
+  const uint8_t *hu_lut;        // [hu_lut_n] HU -> bin
+  const Nucleus *nuc;           // [n_elem]
+  const double *mass;           // [zdim][adim]
+  const float *evap_k, *evap_c; // [6][zdim]
+  int elem_z[MAX_ELEM], elem_a[MAX_ELEM];
+};
+
+struct Grid {                   // PAPER.md:L144 "CT geometry in global memory"
+  const int16_t *hu; int nx, ny, nz; float d[3]; float vol;   // voxel volume, cm^3
+};
+
+// energy-grid lookup shared by the range spline and the cross-section lerp
+struct EIdx { int i; float b; };
+__device__ __forceinline__ EIdx e_index(const Tables &T, float lnE) {
+  float t = (lnE - T.ln_emin) * T.inv_dlne;
+  int i = min(max((int)floorf(t), 0), T.n_e - 2);
+  return {i, t - (float)i};
+}
+// natural cubic spline on uniform knots, y'' pre-scaled by h^2/6
+__device__ __forceinline__ float spline_eval(const float *y, const float *y2, int i, float b) {
+  const float a = 1.0f - b;
+  return a * y[i] + b * y[i + 1] + ((a * a * a - a) * y2[i] + (b * b * b - b) * y2[i + 1]);
+}
+__device__ __forceinline__ float ln_range(const Tables &T, const float *lnR, const float *lnR2, int tab, EIdx k) {
+  return spline_eval(lnR + tab * T.n_e, lnR2 + tab * T.n_e, k.i, k.b);
+}
+// ln E of the inverse table at ln R = x (clamped like the forward table)
+__device__ __forceinline__ float ln_energy_of(const Tables &T, const float *lnE, const float *lnE2, int tab, float x) {
+  if (x <= T.lnr_lo[tab]) return T.ln_emin;
+  if (x >= T.lnr_hi[tab]) return T.ln_emax;
+  float t = (x - T.lnr_lo[tab]) * T.inv_hr[tab];
+  int i = min(max((int)floorf(t), 0), T.n_r - 2);
+  return spline_eval(lnE + tab * T.n_r, lnE2 + tab * T.n_r, i, t - (float)i);
+}
+__device__ __forceinline__ float lerp_tab(const float *tab, EIdx k) { return (1.0f - k.b) * tab[k.i] + k.b * tab[k.i + 1]; }
+
+// ------------------------------------------------------------------ small vector helpers
+struct V3 { float x, y, z; };
+__device__ __forceinline__ V3 operator+(V3 a, V3 b) { return {a.x + b.x, a.y + b.y, a.z + b.z}; }
+__device__ __forceinline__ V3 operator-(V3 a, V3 b) { return {a.x - b.x, a.y - b.y, a.z - b.z}; }
+__device__ __forceinline__ V3 operator*(float s, V3 a) { return {s * a.x, s * a.y, s * a.z}; }
+__device__ __forceinline__ float dot(V3 a, V3 b) { return a.x * b.x + a.y * b.y + a.z * b.z; }
+__device__ __forceinline__ V3 unit(V3 a) { float n = rsqrtf(dot(a, a)); return {a.x * n, a.y * n, a.z * n}; }
+// components (a,b,c) in the frame whose z axis is the unit vector d -> lab frame
+__device__ __forceinline__ V3 to_lab(V3 d, float a, float b, float c) {
+  const float s2 = d.x * d.x + d.y * d.y;
+  if (s2 < 1e-14f) { const float sg = d.z >= 0.f ? 1.0f : -1.0f; return {a, sg * b, sg * c}; }
+  const float is = rsqrtf(s2), s = s2 * is;
+  return {a * d.x * d.z * is - b * d.y * is + c * d.x, a * d.y * d.z * is + b * d.x * is + c * d.y, -a * s + c * d.z};
+}
+__device__ __forceinline__ V3 isotropic(uint32_t r0, uint32_t r1) {
+  const float c = 2.0f * u01(r0) - 1.0f, s = sqrtf(fmaxf(0.f, 1.0f - c * c));
+  float sp, cp; sincospif(2.0f * u01(r1), &sp, &cp);
+  return {s * cp, s * sp, c};
+}
+// Lorentz transformation of (p,E) from a frame moving with velocity beta
+__device__ __forceinline__ void boost(V3 beta, V3 &p, float &E) {
+  const float b2 = dot(beta, beta);
+  if (b2 <= 0.f) return;
+  const float gam = rsqrtf(1.0f - b2), bp = dot(beta, p);
+  const float f = gam * gam / (gam + 1.0f) * bp + gam * E;      // (gam-1)/b2 = gam^2/(gam+1)
+  p = p + f * beta;
+  E = gam * (E + bp);
+}
+
+// ------------------------------------------------------------------ SoA particle queue (PAPER.md:L144 D1)
+struct Queue {
+  float *x, *y, *z, *u, *v, *w, *e;    // position is voxel-local (cm from the voxel's lower corner)
+  int *vox;                            // linear voxel index
+  uint32_t *hist, *pid, *blk, *aux;    // RNG stream; aux = element index (event queues) / product counter
+  uint32_t *count; uint32_t cap;
+};
+struct Particle { V3 r, d; float e; int vox; uint32_t hist, pid, blk, aux; };
+
+__device__ __forceinline__ Particle queue_load(const Queue &q, uint32_t i) {
+  Particle p;
+  p.r = {q.x[i], q.y[i], q.z[i]}; p.d = {q.u[i], q.v[i], q.w[i]}; p.e = q.e[i]; p.vox = q.vox[i];
+  p.hist = q.hist[i]; p.pid = q.pid[i]; p.blk = q.blk[i]; p.aux = q.aux[i];
+  return p;
+}
+// warp-aggregated slot allocation: the lanes that reach this point together share one atomicAdd
+__device__ __forceinline__ uint32_t warp_alloc(uint32_t *counter) {
+  const unsigned m = __activemask();
+  const int lane = threadIdx.x & 31, leader = __ffs(m) - 1;
+  uint32_t base = 0;
+  if (lane == leader) base = atomicAdd(counter, (uint32_t)__popc(m));
+  base = __shfl_sync(m, base, leader);
+  return base + (uint32_t)__popc(m & ((1u << lane) - 1u));
+}
+// returns false on overflow (the caller raises the sticky overflow flag)
+__device__ __forceinline__ bool queue_push(const Queue &q, const Particle &p) {
+  const uint32_t i = warp_alloc(q.count);
+  if (i >= q.cap) return false;
+  q.x[i] = p.r.x; q.y[i] = p.r.y; q.z[i] = p.r.z; q.u[i] = p.d.x; q.v[i] = p.d.y; q.w[i] = p.d.z; q.e[i] = p.e;
+  q.vox[i] = p.vox; q.hist[i] = p.hist; q.pid[i] = p.pid; q.blk[i] = p.blk; q.aux[i] = p.aux;
+  return true;
+}
+
+// ------------------------------------------------------------------ global counters / ledger
+struct Counters {
+  unsigned long long n_steps, n_elastic, n_nonelastic, n_secondary, n_missed, n_inc_tries, n_zab_bad;
+  double e_source, e_deposit, e_escape, e_neutron, e_gamma, e_q, e_air;
+  unsigned int overflow;
+};
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+__device__ __forceinline__ unsigned long long warp_sum(unsigned long long v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+// all 32 lanes must call
+__device__ __forceinline__ void flush(double *dst, double v) { v = warp_sum(v); if ((threadIdx.x & 31) == 0 && v != 0.0) atomicAdd(dst, v); }
+__device__ __forceinline__ void flush(unsigned long long *dst, unsigned long long v) { v = warp_sum(v); if ((threadIdx.x & 31) == 0 && v) atomicAdd(dst, v); }
+
+// ------------------------------------------------------------------ straggling (Reading R4)
+// Vavilov(kappa, beta^2) as its defining compound-Poisson process, shifted to the CSDA mean loss.  The collision
+// spectrum xi/T^2 (1 - beta^2 T/Tmax) is split at T_c: collisions above T_c are sampled one by one (Poisson
+// number by inversion, thinning for the (1 - beta^2 T/Tmax) factor); the many soft ones below T_c are replaced
+// by a Cornish-Fisher-corrected normal deviate carrying their exact 2nd, 3rd and 4th cumulants.  T_c is chosen
+// so that about MU_HARD hard collisions are expected (never below the oracle's own cut).  kappa >= kappa_G:
+// plain Gaussian of variance xi Tmax (1 - beta^2/2).
+constexpr float MU_HARD = 4.0f;
+__device__ __forceinline__ float gauss_pair(uint32_t a, uint32_t b) {
+  return sqrtf(-2.0f * __logf(u01(a))) * cospif(2.0f * u01(b));
+}
+__device__ float straggle(const Tables &T, Rng &g, float e_start, float mean_loss, float rhoL, float zoa) {
+  if (rhoL <= 0.f || mean_loss <= 0.f) return mean_loss;
+  const float gam = 1.0f + e_start * (1.0f / MP), b2 = 1.0f - 1.0f / (gam * gam), bg2 = b2 * gam * gam;
+  const float tmax = 2.0f * ME * bg2 / (1.0f + 2.0f * gam * (ME / MP) + (ME / MP) * (ME / MP));
+  const float xi = 0.5f * KBETHE * zoa * rhoL / b2;
+  float loss;
+  uint4 r = g.next4();
+  const float z = gauss_pair(r.x, r.y);
+  if (xi >= T.kappa_g * tmax) {
+    loss = mean_loss + sqrtf(xi * tmax * (1.0f - 0.5f * b2)) * z;
+  } else {
+    const float itmax = 1.0f / tmax;
+    float tc = fmaxf(fminf(1e-3f, 0.01f * tmax), 1.0f / (MU_HARD / xi + itmax));
+    tc = fminf(tc, tmax);
+    const float itc = 1.0f / tc, ltc = __logf(tmax * itc);
+    const float mu_c = xi * (itc - itmax);                                   // candidates (before thinning)
+    const float mean_hard = xi * (ltc - b2 * (1.0f - tc * itmax));
+    // Poisson(mu_c) by inversion with one uniform
+    float pk = __expf(-mu_c), cdf = pk; const float up = u01(r.z);
+    int n = 0;
+    while (up > cdf && n < 64) { ++n; pk *= mu_c / (float)n; cdf += pk; }
+    float hard = 0.f;
+    uint4 q = make_uint4(0, 0, 0, 0);
+    for (int k = 0; k < n; ++k) {
+      if ((k & 1) == 0) q = g.next4();
+      const uint32_t ra = (k & 1) ? q.z : q.x, rb = (k & 1) ? q.w : q.y;
+      const float t = 1.0f / (itc - u01(ra) * (itc - itmax));
+      if (u01(rb) < 1.0f - b2 * t * itmax) hard += t;
+    }
+    // soft part: cumulants k2 = xi tc (1 - b2 tc/2Tmax), k3 = xi tc^2 (1/2 - b2 tc/3Tmax), k4 = xi tc^3 (1/3 - b2 tc/4Tmax)
+    const float x = b2 * tc * itmax;
+    const float k2 = xi * tc * (1.0f - 0.5f * x);
+    const float g1 = xi * tc * tc * (0.5f - x * (1.0f / 3.0f)) / (k2 * sqrtf(k2));
+    const float g2 = xi * tc * tc * tc * ((1.0f / 3.0f) - 0.25f * x) / (k2 * k2);
+    const float z2 = z * z;
+    const float cf = z + g1 * (1.0f / 6.0f) * (z2 - 1.0f) + g2 * (1.0f / 24.0f) * z * (z2 - 3.0f)
+                     - g1 * g1 * (1.0f / 36.0f) * z * (2.0f * z2 - 5.0f);
+    loss = mean_loss + (hard - mean_hard) + sqrtf(k2) * cf;
+  }
+  return fminf(fmaxf(loss, 0.f), e_start);
+}
+
+// ------------------------------------------------------------------ Cugnon NN parameterisation (PAPER.md:L77 ref [20]; Reading R6)
+// p in GeV/c, sigma in mb
+__device__ __forceinline__ float cug_sigma_pp(float p) {
+  if (p < 0.44f) return 34.0f * __powf(p * 2.5f, -2.104f);
+  if (p < 0.8f) { float d = p - 0.7f; d *= d; return 23.5f + 1000.0f * d * d; }
+  if (p < 2.0f) return 1250.0f / (p + 50.0f) - 4.0f * (p - 1.3f) * (p - 1.3f);
+  return 77.0f / (p + 1.5f);
+}
+__device__ __forceinline__ float cug_sigma_np(float p) {
+  if (p < 0.446f) { const float l = __logf(p); return 6.3555f * __expf(-3.2481f * l - 0.377f * l * l); }
+  if (p < 0.8f) { const float a = fabsf(p - 0.95f); return 33.0f + 196.0f * a * a * sqrtf(a); }
+  if (p < 2.0f) return 31.0f * rsqrtf(p);
+  return 77.0f / (p + 1.5f);
+}
+__device__ __forceinline__ float cug_b_pp(float p) {
+  if (p < 2.0f) { float p2 = p * p, p4 = p2 * p2, p8 = p4 * p4; return 5.5f * p8 / (7.7f + p8); }
+  return 5.334f + 0.67f * (p - 2.0f);
+}
+__device__ __forceinline__ float cug_b_np(float p) {
+  if (p < 0.225f) return 0.f;
+  if (p < 0.6f) return 16.53f * (p - 0.225f);
+  if (p < 1.6f) return -1.63f * p + 7.16f;
+  return cug_b_pp(p);
+}
+__device__ __forceinline__ float cug_a_np(float p) { return p < 0.8f ? 1.0f : 0.64f / (p * p); }
+
+// |t| from exp(-B t) truncated to [0, tmax]
+__device__ __forceinline__ float trunc_exp(float B, float tmax, float u) {
+  if (B * tmax < 1e-6f) return u * tmax;
+  return -__logf(1.0f - u * (1.0f - __expf(-B * tmax))) / B;
+}
+// cos(theta_cm) of NN elastic scattering: dsigma/dt ~ exp(B t) (+ a exp(B u) for np).  Uses 2 uniforms.
+__device__ __forceinline__ float sample_nn_cos(bool same, float p_lab_gev, float pcm_mev, uint32_t r0, uint32_t r1) {
+  const float tmax = 4.0f * pcm_mev * pcm_mev * 1e-6f;
+  const float B = same ? cug_b_pp(p_lab_gev) : cug_b_np(p_lab_gev);
+  bool backward = false;
+  if (!same) { const float a = cug_a_np(p_lab_gev); backward = u01(r0) < a / (1.0f + a); }
+  const float t = trunc_exp(B, tmax, u01(r1));
+  const float c = 1.0f - 2.0f * t / tmax;
+  return backward ? -c : c;
+}
+
+}  // namespace pmc

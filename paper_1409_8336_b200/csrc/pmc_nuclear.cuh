@@ -1,0 +1,406 @@
+// pmc_nuclear.cuh — non-elastic proton-nucleus collisions: Bertini-style intranuclear cascade (
+// Reading R6) followed by evaporation (Reading R7), as device functions plus the event-queue
+// kernels of the transport scheduler and the standalone kernel behind pmc_nonelastic.
+//
+// Precision: cascade geometry, sampling and NN kinematics run in fp32; the conservation bookkeeping (sums of
+// outgoing four-momenta, residual excitation energy, two-body decay of the compound nucleus, separation
+// energies) runs in fp64 because it subtracts nuclear masses of 1e4 MeV to get MeV-scale answers.  Charge and
+// baryon number are integers throughout.
+#pragma once
+#include "pmc_device.cuh"
+
+namespace pmc {
+
+constexpr int CASC_STACK = 48;      // cascade nucleons waiting to be tracked (an attempt that needs more fails)
+constexpr int MAX_INC_OUT = 32;     // nucleons leaving the nucleus in one cascade
+constexpr int MAX_SEC = 48;         // records per event in the standalone kernel's slot buffer (INC + evaporation + residual)
+constexpr int NQ = 64;              // quadrature bins of the evaporation spectrum (Reading R7)
+
+struct SecRec { int16_t Z, A; uint8_t origin, pad[3]; float ke; float dir[3]; };   // == pmc_secondary (24 B)
+static_assert(sizeof(SecRec) == 24, "pmc_secondary layout");
+
+struct OutNuc { int type; float ke; V3 dir; double p[3]; };                      // type 0 proton, 1 neutron
+struct Residual { int Z, A; double estar; double P[3]; double mass_gs; };
+struct CascNucleon { V3 r, p; int type, shell; };
+
+__device__ __forceinline__ float nucleon_mass(int type) { return type == 0 ? MP : MN; }
+__device__ __forceinline__ double nmass(const Tables &T, int z, int a) {
+  return (z < 0 || a < 1 || z >= T.zdim || a >= T.adim || z > a) ? 0.0 : T.mass[z * T.adim + a];
+}
+
+// one cascade attempt; false if no Pauli-allowed collision happened or the outcome is invalid (L75)
+__device__ bool inc_attempt(const Tables &T, const Nucleus &N, float t_in, Rng &g, OutNuc *out, int &n_out_ret,
+                            Residual &res) {
+  const int ns = N.nshell;
+  CascNucleon stack[CASC_STACK]; int sp = 0;
+  int ncoll = 0, n_out = 0, np_out = 0;
+  double e_out_sum = 0, pxs = 0, pys = 0, pzs = 0;
+  {
+    // entry: uniform over the disc of radius rmax, travelling along +z (L75 "random point of entry");
+    // refraction into the outermost shell: gains V, tangential momentum conserved
+    const uint4 r = g.next4();
+    const float b = N.rmax * sqrtf(u01(r.x)); float sph, cph; sincospif(2.0f * u01(r.y), &sph, &cph);
+    const V3 r0{b * cph, b * sph, -sqrtf(fmaxf(0.f, N.rmax * N.rmax - b * b))};
+    const float Tn = t_in + N.V[0][ns - 1], p0 = sqrtf(t_in * (t_in + 2.0f * MP)), p1 = sqrtf(Tn * (Tn + 2.0f * MP));
+    const V3 nh = unit(r0), pv{0.f, 0.f, p0};
+    const float pr = dot(pv, nh); const V3 pt = pv - pr * nh;
+    const float pr2 = p1 * p1 - dot(pt, pt);
+    stack[sp++] = {r0, pt + (-sqrtf(fmaxf(pr2, 0.f))) * nh, 0, ns - 1};
+  }
+  int guard = 0;
+  while (sp > 0) {
+    CascNucleon c = stack[--sp];
+    bool alive = true;
+    while (alive) {
+      if (++guard > 20000) return false;
+      const int k = c.shell, ty = c.type;
+      const float m = nucleon_mass(ty), p2 = dot(c.p, c.p), E = sqrtf(p2 + m * m), Tk = p2 / (E + m);
+      const V3 d = rsqrtf(p2) * c.p;
+      // candidate collisions with a proton and with a neutron of the Fermi sea (Reading R6.3)
+      float dbest = BIG, plab_best = 0.f; int tbest = -1; V3 qbest{0.f, 0.f, 0.f};
+#pragma unroll
+      for (int tp = 0; tp < 2; ++tp) {
+        if (N.rho[tp][k] <= 0.f) continue;
+        const uint4 r = g.next4();
+        const float mq = nucleon_mass(tp), qmag = N.pF[tp][k] * cbrtf(u01(r.x));
+        const V3 q = qmag * isotropic(r.y, r.z);
+        const float Eq = sqrtf(qmag * qmag + mq * mq);
+        const float e1 = (E * Eq - dot(c.p, q)) / mq;                       // projectile energy in the partner rest frame
+        const float plab = sqrtf(fmaxf(e1 * e1 - m * m, 0.f));
+        const float sig = N.const_sigma_mb >= 0.f ? N.const_sigma_mb
+                                                  : (tp == ty ? cug_sigma_pp(plab * 1e-3f) : cug_sigma_np(plab * 1e-3f));
+        const float dist = -__logf(u01(r.w)) / (N.rho[tp][k] * sig * 0.1f);  // 1 mb = 0.1 fm^2
+        if (dist < dbest) { dbest = dist; tbest = tp; qbest = q; plab_best = plab; }
+      }
+      // distance to the shell boundaries along d
+      const float rr = dot(c.r, c.r), bq = dot(c.r, d), r_out = N.rout[k], r_in = k > 0 ? N.rout[k - 1] : 0.f;
+      float dbound = -bq + sqrtf(fmaxf(bq * bq - (rr - r_out * r_out), 0.f)); bool inward = false;
+      if (k > 0 && bq < 0.f) {
+        const float disc = bq * bq - (rr - r_in * r_in);
+        if (disc > 0.f) { const float s_in = -bq - sqrtf(disc); if (s_in < dbound) { dbound = fmaxf(s_in, 0.f); inward = true; } }
+      }
+      if (dbest < dbound) {
+        // ---- collision attempt (Reading R6.4)
+        c.r = c.r + dbest * d;
+        const int tp = tbest; const float mq = nucleon_mass(tp);
+        const V3 q = qbest; const float Eq = sqrtf(dot(q, q) + mq * mq);
+        const V3 Pt = c.p + q; const float Et = E + Eq; const V3 beta = (1.0f / Et) * Pt;
+        const float s = Et * Et - dot(Pt, Pt);
+        const float pcm = sqrtf(fmaxf((s - (m + mq) * (m + mq)) * (s - (m - mq) * (m - mq)), 0.f) / (4.0f * s));
+        V3 p1 = c.p; float E1 = E; boost(-1.0f * beta, p1, E1);             // projectile in the CM
+        const V3 ax = unit(p1);
+        const uint4 r = g.next4();
+        const float ct = sample_nn_cos(tp == ty, plab_best * 1e-3f, pcm, r.x, r.y), st = sqrtf(fmaxf(0.f, 1.0f - ct * ct));
+        float sph, cph; sincospif(2.0f * u01(r.z), &sph, &cph);
+        V3 n1 = pcm * to_lab(ax, st * cph, st * sph, ct), n2 = -1.0f * n1;
+        float En1 = sqrtf(pcm * pcm + m * m), En2 = sqrtf(pcm * pcm + mq * mq);
+        boost(beta, n1, En1); boost(beta, n2, En2);
+        const float T1 = En1 - m, T2 = En2 - mq;
+        const bool ok = !N.pauli || (T1 > N.EF[ty][k] && T2 > N.EF[tp][k]);  // L77 Pauli blocking
+        if (!ok) continue;                                                   // blocked: go on unchanged
+        ncoll++;
+        // trapping (Reading R6.4): outside energy eps = T - V <= B_C stays in the nucleus
+        const float bc2 = tp == 0 ? N.coulomb : 0.f, bc1 = ty == 0 ? N.coulomb : 0.f;
+        if (T2 - N.V[tp][k] > bc2) { if (sp >= CASC_STACK) return false; stack[sp++] = {c.r, n2, tp, k}; }
+        if (T1 - N.V[ty][k] > bc1) c.p = n1; else alive = false;
+        continue;
+      }
+      // ---- shell boundary (L77 "reflection and refraction"; Reading R6.5)
+      c.r = c.r + dbound * d;
+      const float rb = inward ? r_in : r_out;
+      c.r = (rb * rsqrtf(dot(c.r, c.r))) * c.r;
+      const V3 nh = (1.0f / rb) * c.r;
+      const float pr = dot(c.p, nh); const V3 pt = c.p - pr * nh;
+      const int k2 = inward ? k - 1 : k + 1;
+      const float Vnew = k2 >= ns ? 0.f : N.V[ty][k2], T2 = Tk + (Vnew - N.V[ty][k]);
+      const float pn2 = T2 > 0.f ? T2 * (T2 + 2.0f * m) : -1.0f, pr2 = pn2 - dot(pt, pt);
+      if (pn2 <= 0.f || pr2 <= 0.f) { c.p = pt - pr * nh; continue; }         // specular reflection
+      const V3 pnew = pt + ((pr > 0.f ? 1.0f : -1.0f) * sqrtf(pr2)) * nh;
+      if (k2 >= ns) {                                                       // leaves the nucleus with KE = eps
+        if (n_out >= MAX_INC_OUT) return false;
+        OutNuc &o = out[n_out++];
+        o.type = ty; o.ke = T2; o.dir = unit(pnew); o.p[0] = pnew.x; o.p[1] = pnew.y; o.p[2] = pnew.z;
+        e_out_sum += (double)T2 + (ty == 0 ? MP_D : MN_D); pxs += pnew.x; pys += pnew.y; pzs += pnew.z;
+        if (ty == 0) np_out++;
+        alive = false;
+      } else { c.p = pnew; c.shell = k2; }
+    }
+  }
+  if (ncoll == 0) return false;                                             // L75: need >= 1 allowed collision
+  // ---- residual nucleus (Reading R6.7): exact integers, relativistic invariant mass, fp64
+  const int Ar = N.A + 1 - n_out, Zr = N.Z + 1 - np_out;
+  const double Mgs = nmass(T, Zr, Ar);
+  if (Ar < 1 || Zr < 0 || Zr > Ar || Mgs <= 0) return false;
+  const double tin = (double)t_in, pin = sqrt(tin * (tin + 2 * MP_D));
+  const double Eres = (tin + MP_D + N.mass) - e_out_sum, Px = -pxs, Py = -pys, Pz = pin - pzs;
+  const double M2 = Eres * Eres - (Px * Px + Py * Py + Pz * Pz);
+  if (Eres <= 0 || M2 <= 0) return false;
+  const double estar = sqrt(M2) - Mgs;
+  if (estar < 0) return false;
+  if (Ar == 1 && estar > 1e-4) return false;                                // a lone nucleon cannot be excited
+  res.Z = Zr; res.A = Ar; res.estar = estar; res.P[0] = Px; res.P[1] = Py; res.P[2] = Pz; res.mass_gs = Mgs;
+  n_out_ret = n_out;
+  return true;
+}
+
+__device__ void inc_event(const Tables &T, const Nucleus &N, float t_in, Rng &g, OutNuc *out, int &n_out, Residual &res,
+                          unsigned long long &tries) {
+  for (int it = 0; it < 100000; ++it) {                 // L75 "This is repeated until ..."
+    tries++;
+    if (inc_attempt(T, N, t_in, g, out, n_out, res)) return;
+  }
+  // Reading R6.8 (never reached in the configs): form the compound nucleus (Z+1, A+1)
+  n_out = 0;
+  const double tin = (double)t_in, pin = sqrt(tin * (tin + 2 * MP_D)), Et = tin + MP_D + N.mass, Mgs = nmass(T, N.Z + 1, N.A + 1);
+  res.Z = N.Z + 1; res.A = N.A + 1; res.estar = sqrt(Et * Et - pin * pin) - Mgs; res.P[0] = 0; res.P[1] = 0; res.P[2] = pin; res.mass_gs = Mgs;
+}
+
+// ------------------------------------------------------------------ evaporation (Reading R7)
+__constant__ int EJ_Z[6] = {0, 1, 1, 1, 2, 2};
+__constant__ int EJ_A[6] = {1, 1, 2, 3, 3, 4};
+__constant__ float EJ_SPIN_G[6] = {2.f, 2.f, 3.f, 2.f, 2.f, 1.f};
+__device__ __forceinline__ float pairing(int Z, int A) {
+  const int N = A - Z; const float d = 12.0f * rsqrtf((float)A);
+  return (Z % 2 == 0 && N % 2 == 0) ? 2.0f * d : ((Z % 2) != (N % 2) ? d : 0.f);
+}
+struct Chan { float S, emin, emax, kV, cj, pref, alpha, beta, ad; int Zd, Ad; double Md, mj; };
+__device__ bool chan_setup(const Tables &T, int Z, int A, float estar, double Mpar, int j, Chan &c) {
+  const int Zd = Z - EJ_Z[j], Ad = A - EJ_A[j];
+  if (Ad < 2 || Zd < 0) return false;
+  const double Md = nmass(T, Zd, Ad), mj = nmass(T, EJ_Z[j], EJ_A[j]);
+  if (Md <= 0) return false;
+  c.Zd = Zd; c.Ad = Ad; c.Md = Md; c.mj = mj; c.S = (float)(Md + mj - Mpar);
+  const float a13 = cbrtf((float)Ad);
+  c.kV = 0.f; c.cj = 0.f;
+  if (j > 0) {
+    const float rhoj = j == 1 ? 0.f : 1.2f, V = 1.44f * EJ_Z[j] * Zd / (1.5f * a13 + rhoj);
+    c.kV = T.evap_k[j * T.zdim + Zd] * V; c.cj = T.evap_c[j * T.zdim + Zd];
+  }
+  c.emin = c.kV; c.emax = estar - c.S - pairing(Zd, Ad);
+  if (c.emax <= c.emin) return false;
+  c.alpha = 0.76f + 2.2f / a13; c.beta = (2.12f / (a13 * a13) - 0.050f) / c.alpha; c.ad = Ad * 0.125f;
+  c.pref = EJ_SPIN_G[j] * (float)mj * a13 * a13;
+  return true;
+}
+__device__ __forceinline__ float chan_f(const Chan &c, int j, float e, float ref) {
+  const float sinv = j == 0 ? c.alpha * (1.0f + c.beta / e) : (1.0f + c.cj) * (1.0f - c.kV / e);
+  return c.pref * sinv * e * __expf(2.0f * sqrtf(c.ad * (c.emax - e)) - ref);
+}
+struct Emission { int j; float ke; V3 dir; };
+// one emission from R (updated in place); returns false when no channel is open
+__device__ bool evap_emit(const Tables &T, Residual &R, Rng &g, uint32_t mask, Emission &em, float *eps_out, float *cos_out) {
+  const float estar = (float)R.estar;
+  const float ref = 2.0f * sqrtf(R.A * 0.125f * fmaxf(estar, 0.f));
+  float width[6]; float tot = 0.f;
+#pragma unroll 1
+  for (int j = 0; j < 6; ++j) {
+    width[j] = 0.f;
+    Chan c;
+    if (!((mask >> j) & 1u) || !chan_setup(T, R.Z, R.A, estar, R.mass_gs, j, c)) continue;
+    const float de = (c.emax - c.emin) * (1.0f / NQ);
+    float w = 0.f;
+    for (int i = 0; i < NQ; ++i) w += chan_f(c, j, c.emin + (i + 0.5f) * de, ref);
+    width[j] = w * de; tot += width[j];
+  }
+  if (!(tot > 0.f)) return false;
+  const uint4 r = g.next4();
+  float u = u01(r.x) * tot; int j = -1;
+#pragma unroll
+  for (int q = 0; q < 6; ++q) if (width[q] > 0.f && (j < 0 || u >= 0.f)) { j = q; u -= width[q]; }
+  Chan c; chan_setup(T, R.Z, R.A, estar, R.mass_gs, j, c);
+  const float de = (c.emax - c.emin) * (1.0f / NQ);
+  float v = u01(r.y) * width[j] / de; int bin = NQ - 1;
+  for (int i = 0; i < NQ; ++i) { const float f = chan_f(c, j, c.emin + (i + 0.5f) * de, ref); if (v < f) { bin = i; break; } v -= f; }
+  const float eps = c.emin + ((float)bin + u01(r.z)) * de;                  // total CM kinetic energy released
+  // relativistic two-body decay of M* -> m_j + M_d* (isotropic in the nucleus rest frame, L79), fp64
+  const uint4 r2 = g.next4();
+  const V3 dirc = isotropic(r2.x, r2.y);
+  const double mj = c.mj, Mstar = R.mass_gs + R.estar, Ud = R.estar - (c.Md + mj - R.mass_gs) - (double)eps, Md = c.Md + Ud;
+  const double pc2 = (Mstar * Mstar - (mj + Md) * (mj + Md)) * (Mstar * Mstar - (mj - Md) * (mj - Md)) / (4 * Mstar * Mstar);
+  const double pc = sqrt(fmax(pc2, 0.0));
+  double pj[3] = {pc * dirc.x, pc * dirc.y, pc * dirc.z};
+  double Ej = sqrt(pc * pc + mj * mj), Ed = sqrt(pc * pc + Md * Md);
+  const double Epar = sqrt(R.P[0] * R.P[0] + R.P[1] * R.P[1] + R.P[2] * R.P[2] + Mstar * Mstar);
+  const double bx = R.P[0] / Epar, by = R.P[1] / Epar, bz = R.P[2] / Epar, b2 = bx * bx + by * by + bz * bz;
+  double pd[3] = {-pj[0], -pj[1], -pj[2]};
+  if (b2 > 0) {
+    const double gam = 1.0 / sqrt(1.0 - b2);
+    const double bpj = bx * pj[0] + by * pj[1] + bz * pj[2], fj = (gam - 1.0) * bpj / b2 + gam * Ej;
+    pj[0] += fj * bx; pj[1] += fj * by; pj[2] += fj * bz; Ej = gam * (Ej + bpj);
+    const double bpd = -bpj + 0.0, fd = (gam - 1.0) * bpd / b2 + gam * Ed;
+    pd[0] += fd * bx; pd[1] += fd * by; pd[2] += fd * bz; Ed = gam * (Ed + bpd);
+  }
+  const double pn = sqrt(pj[0] * pj[0] + pj[1] * pj[1] + pj[2] * pj[2]);
+  em.j = j; em.ke = (float)(Ej - mj);
+  em.dir = pn > 0 ? V3{(float)(pj[0] / pn), (float)(pj[1] / pn), (float)(pj[2] / pn)} : V3{0.f, 0.f, 1.f};
+  R.Z = c.Zd; R.A = c.Ad; R.estar = Ud; R.P[0] = pd[0]; R.P[1] = pd[1]; R.P[2] = pd[2]; R.mass_gs = c.Md;
+  if (eps_out) *eps_out = eps;
+  if (cos_out) *cos_out = dirc.z;
+  return true;
+}
+__device__ __forceinline__ double residual_ke(const Residual &R) {
+  const double Mres = R.mass_gs + R.estar, p2 = R.P[0] * R.P[0] + R.P[1] * R.P[1] + R.P[2] * R.P[2];
+  return p2 / (sqrt(p2 + Mres * Mres) + Mres);
+}
+
+// ------------------------------------------------------------------ event-queue kernels of the transport scheduler
+struct ResQueue { Queue q; uint32_t *za; float *px, *py, *pz; };   // q.e = E*, q.aux = next product index
+
+// K3: one cascade per thread over the non-elastic queue (PAPER.md:L128(3), L136)
+__global__ void __launch_bounds__(128) inc_kernel(Tables T, RunParams P, Queue in, Queue out, ResQueue rq, float *tally,
+                                                  Counters *cnt) {
+  const uint32_t n = min(*in.count, in.cap);
+  double c_dep = 0, c_neu = 0, c_q = 0; unsigned long long c_sec = 0, c_tries = 0;
+  for (uint32_t i0 = blockIdx.x * blockDim.x; i0 < n; i0 += gridDim.x * blockDim.x) {
+    const uint32_t i = i0 + threadIdx.x;
+    if (i < n) {
+      Particle p = queue_load(in, i);
+      Rng g; g.init(P.seed, P.hist0 + p.hist, p.pid, p.blk);
+      const Nucleus &N = T.nuc[p.aux];
+      OutNuc outn[MAX_INC_OUT]; int n_out = 0; Residual R;
+      inc_event(T, N, p.e, g, outn, n_out, R, c_tries);
+      float dep = 0.f; uint32_t kchild = 0; double msum = 0;
+      for (int k = 0; k < n_out; ++k) {
+        const OutNuc &o = outn[k];
+        msum += o.type == 0 ? MP_D : MN_D;
+        if (o.type == 0) {                                                   // L79: only protons are followed
+          if (o.ke > T.e_cut) {
+            Particle s = p; s.d = unit(to_lab(p.d, o.dir.x, o.dir.y, o.dir.z)); s.e = o.ke;
+            s.pid = g.child_id(kchild++); s.blk = 0u; s.aux = 0u; c_sec++;
+            if (!queue_push(out, s)) atomicOr(&cnt->overflow, 16u);
+          } else dep += o.ke;
+        } else c_neu += (double)o.ke;                                        // neutrons: not transported
+      }
+      c_q += msum + R.mass_gs - MP_D - N.mass;
+      if (dep != 0.f) { atomicAdd(tally + p.vox, dep); c_dep += (double)dep; }
+      // residual -> evaporation queue (keeps the event frame: p.d is the incident direction)
+      const uint32_t slot = warp_alloc(rq.q.count);
+      if (slot >= rq.q.cap) atomicOr(&cnt->overflow, 32u);
+      else {
+        const Queue &q = rq.q;
+        q.x[slot] = p.r.x; q.y[slot] = p.r.y; q.z[slot] = p.r.z; q.u[slot] = p.d.x; q.v[slot] = p.d.y; q.w[slot] = p.d.z;
+        q.e[slot] = (float)R.estar; q.vox[slot] = p.vox; q.hist[slot] = p.hist; q.pid[slot] = p.pid; q.blk[slot] = g.blk;
+        q.aux[slot] = kchild; rq.za[slot] = ((uint32_t)R.Z << 16) | (uint32_t)R.A;
+        rq.px[slot] = (float)R.P[0]; rq.py[slot] = (float)R.P[1]; rq.pz[slot] = (float)R.P[2];
+      }
+    }
+  }
+  flush(&cnt->e_deposit, c_dep); flush(&cnt->e_neutron, c_neu); flush(&cnt->e_q, c_q);
+  flush(&cnt->n_secondary, c_sec); flush(&cnt->n_inc_tries, c_tries);
+}
+
+// K4: one nuclear de-excitation per thread over the residual queue (PAPER.md:L128(4), L136)
+__global__ void __launch_bounds__(128) evap_kernel(Tables T, RunParams P, ResQueue rq, Queue out, float *tally, Counters *cnt) {
+  const uint32_t n = min(*rq.q.count, rq.q.cap);
+  double c_dep = 0, c_neu = 0, c_q = 0, c_gam = 0; unsigned long long c_sec = 0;
+  for (uint32_t i0 = blockIdx.x * blockDim.x; i0 < n; i0 += gridDim.x * blockDim.x) {
+    const uint32_t i = i0 + threadIdx.x;
+    if (i < n) {
+      Particle p = queue_load(rq.q, i);
+      Rng g; g.init(P.seed, P.hist0 + p.hist, p.pid, p.blk);
+      Residual R; R.Z = (int)(rq.za[i] >> 16); R.A = (int)(rq.za[i] & 0xffffu); R.estar = (double)p.e;
+      R.P[0] = rq.px[i]; R.P[1] = rq.py[i]; R.P[2] = rq.pz[i]; R.mass_gs = nmass(T, R.Z, R.A);
+      const double m0 = R.mass_gs; double msum = 0;
+      uint32_t kchild = p.aux; float dep = 0.f;
+      for (int it = 0; it < 200; ++it) {
+        Emission em;
+        if (!evap_emit(T, R, g, 0x3Fu, em, nullptr, nullptr)) break;
+        msum += nmass(T, EJ_Z[em.j], EJ_A[em.j]);
+        if (em.j == 1) {
+          if (em.ke > T.e_cut) {
+            Particle s = p; s.d = unit(to_lab(p.d, em.dir.x, em.dir.y, em.dir.z)); s.e = em.ke;
+            s.pid = g.child_id(kchild++); s.blk = 0u; s.aux = 0u; c_sec++;
+            if (!queue_push(out, s)) atomicOr(&cnt->overflow, 64u);
+          } else dep += em.ke;
+        } else if (em.j == 0) c_neu += (double)em.ke;
+        else dep += em.ke;                                                   // d, t, 3He, alpha: local (L79)
+      }
+      const double kres = residual_ke(R);
+      if (R.A == 1 && R.Z == 0) c_neu += kres; else dep += (float)kres;
+      c_gam += R.estar;                                                     // L79: no photon evaporation
+      c_q += msum + R.mass_gs - m0;
+      if (dep != 0.f) { atomicAdd(tally + p.vox, dep); c_dep += (double)dep; }
+    }
+  }
+  flush(&cnt->e_deposit, c_dep); flush(&cnt->e_neutron, c_neu); flush(&cnt->e_q, c_q); flush(&cnt->e_gamma, c_gam);
+  flush(&cnt->n_secondary, c_sec);
+}
+
+// ------------------------------------------------------------------ standalone non-elastic events (pmc_nonelastic; Table I)
+__global__ void __launch_bounds__(128) nonelastic_kernel(Tables T, const Nucleus *nuc, float t_in, uint64_t seed, uint64_t ev0,
+                                                         uint32_t n, SecRec *slots, uint32_t *counts, Counters *cnt) {
+  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  unsigned long long c_tries = 0, c_bad = 0; double c_gam = 0;
+  if (i < n) {
+    const Nucleus &N = *nuc;
+    Rng g; g.init(seed, ev0 + i, 0u, 0u);
+    OutNuc outn[MAX_INC_OUT]; int n_out = 0; Residual R;
+    inc_event(T, N, t_in, g, outn, n_out, R, c_tries);
+    SecRec *s = slots + (size_t)i * MAX_SEC; int ns = 0, zs = 0, as = 0;
+    for (int k = 0; k < n_out; ++k) {
+      SecRec rec{}; rec.Z = outn[k].type == 0 ? 1 : 0; rec.A = 1; rec.origin = 0; rec.ke = outn[k].ke;
+      rec.dir[0] = outn[k].dir.x; rec.dir[1] = outn[k].dir.y; rec.dir[2] = outn[k].dir.z;
+      zs += rec.Z; as += 1; s[ns++] = rec;
+    }
+    for (int it = 0; it < 200; ++it) {
+      Emission em;
+      if (!evap_emit(T, R, g, 0x3Fu, em, nullptr, nullptr)) break;
+      SecRec rec{}; rec.Z = (int16_t)EJ_Z[em.j]; rec.A = (int16_t)EJ_A[em.j]; rec.origin = 1; rec.ke = em.ke;
+      rec.dir[0] = em.dir.x; rec.dir[1] = em.dir.y; rec.dir[2] = em.dir.z;
+      zs += rec.Z; as += rec.A;
+      if (ns < MAX_SEC - 1) s[ns++] = rec; else atomicOr(&cnt->overflow, 128u);
+    }
+    {
+      const double pn = sqrt(R.P[0] * R.P[0] + R.P[1] * R.P[1] + R.P[2] * R.P[2]);
+      SecRec rec{}; rec.Z = (int16_t)R.Z; rec.A = (int16_t)R.A; rec.origin = 2; rec.ke = (float)residual_ke(R);
+      if (pn > 0) { rec.dir[0] = (float)(R.P[0] / pn); rec.dir[1] = (float)(R.P[1] / pn); rec.dir[2] = (float)(R.P[2] / pn); }
+      else { rec.dir[2] = 1.f; }
+      zs += R.Z; as += R.A; s[ns++] = rec;
+    }
+    if (zs != N.Z + 1 || as != N.A + 1) c_bad++;
+    counts[i] = (uint32_t)ns; c_gam = R.estar;
+  }
+  flush(&cnt->n_inc_tries, c_tries); flush(&cnt->n_zab_bad, c_bad); flush(&cnt->e_gamma, c_gam);
+}
+
+// exclusive scan of counts[n] -> off[n+1] shifted by base (single block; n <= a few 1e5)
+__global__ void __launch_bounds__(1024) scan_kernel(const uint32_t *counts, uint32_t n, uint32_t *off, unsigned long long *base_io) {
+  __shared__ unsigned long long part[1024];
+  const uint32_t per = (n + blockDim.x - 1) / blockDim.x, b = threadIdx.x * per, e = min(b + per, n);
+  unsigned long long s = 0;
+  for (uint32_t i = b; i < e; ++i) s += counts[i];
+  part[threadIdx.x] = s; __syncthreads();
+  if (threadIdx.x == 0) { unsigned long long acc = *base_io; for (int t = 0; t < (int)blockDim.x; ++t) { unsigned long long v = part[t]; part[t] = acc; acc += v; } *base_io = acc; }
+  __syncthreads();
+  unsigned long long acc = part[threadIdx.x];
+  for (uint32_t i = b; i < e; ++i) { off[i] = (uint32_t)acc; acc += counts[i]; }
+}
+__global__ void __launch_bounds__(256) compact_kernel(const SecRec *slots, const uint32_t *counts, const uint32_t *off, uint32_t n,
+                                                      SecRec *out, unsigned long long capacity) {
+  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const uint32_t c = counts[i]; const unsigned long long o = off[i];
+  for (uint32_t k = 0; k < c; ++k) if (o + k < capacity) out[o + k] = slots[(size_t)i * MAX_SEC + k];
+}
+
+// ------------------------------------------------------------------ sub-step test kernels
+__global__ void philox_kernel(const uint32_t *in, uint64_t n, uint32_t *out) {
+  const uint64_t i = blockIdx.x * (uint64_t)blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const uint4 r = philox4x32_10(make_uint4(in[6 * i], in[6 * i + 1], in[6 * i + 2], in[6 * i + 3]), make_uint2(in[6 * i + 4], in[6 * i + 5]));
+  out[4 * i] = r.x; out[4 * i + 1] = r.y; out[4 * i + 2] = r.z; out[4 * i + 3] = r.w;
+}
+__global__ void range_kernel(Tables T, int tab, const float *in, uint64_t n, float *out, int inverse) {
+  const uint64_t i = blockIdx.x * (uint64_t)blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  if (!inverse) { const float x = logf(fminf(fmaxf(in[i], T.e_min), T.e_max)); out[i] = expf(ln_range(T, T.lnR, T.lnR2, tab, e_index(T, x))); }
+  else out[i] = expf(ln_energy_of(T, T.lnE, T.lnE2, tab, logf(fmaxf(in[i], 1e-30f))));
+}
+__global__ void straggle_kernel(Tables T, float e, float mean, float rhoL, float zoa, uint64_t n, uint64_t seed, float *out) {
+  const uint64_t i = blockIdx.x * (uint64_t)blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  Rng g; g.init(seed, i, 0u, 0u);
+  out[i] = straggle(T, g, e, mean, rhoL, zoa);
+}
+
+}  // namespace pmc

@@ -1,0 +1,427 @@
+// pmc_transport.cuh — beam-spot sampler, condensed-history step kernel, nuclear-elastic kernel and the
+// batch-statistics kernels.
+#pragma once
+#include "pmc_device.cuh"
+
+namespace pmc {
+
+struct SpotDev {                 // pmc_spot, prepared on the host (axis normalised, transverse basis built)
+  double pos[3]; double ax[3], ex[3], ey[3];
+  double e, sigma_e, sx, sy, divx, divy;
+};
+
+struct RunParams {
+  uint64_t seed; uint64_t hist0;      // first history id of this launch
+  uint32_t n;                         // histories in this launch
+  int max_steps; float *dbg_out;      // pmc_first_steps: stop after max_steps, write [hist][8]
+  int aggregate;                      // warp-aggregated dose atomics
+};
+
+// ------------------------------------------------------------------ material of a voxel
+struct VoxMat { float rho, wf, inv_x0, zoa; int table, bin; };
+__device__ __forceinline__ int hu_to_bin(const Tables &T, const uint8_t *lut, int hu) {
+  return lut[min(max(hu - T.hu_lut_lo, 0), T.hu_lut_n - 1)];
+}
+__device__ __forceinline__ float bin_density(const MatBin &m, int hu) {
+  const float t = fminf(fmaxf((float)hu - m.hu_lo, 0.f), m.dhu);
+  return m.rho_lo + m.drho * (t * m.inv_dhu);
+}
+
+// distance along d to the first face of the voxel (voxel-local r in [0, size]); ties: x before y before z
+__device__ __forceinline__ float dist_to_face(const V3 &r, const V3 &d, const float *sz, int &axis, int &sgn) {
+  float best = BIG; axis = -1; sgn = 0;
+  const float rr[3] = {r.x, r.y, r.z}, dd[3] = {d.x, d.y, d.z};
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    if (dd[a] != 0.f) {
+      const float t = fmaxf(((dd[a] > 0.f ? sz[a] : 0.f) - rr[a]) / dd[a], 0.f);
+      if (t < best) { best = t; axis = a; sgn = dd[a] > 0.f ? 1 : -1; }
+    }
+  }
+  return best;
+}
+
+// Highland theta0 with the paper's factor; t = mass thickness / X0
+__device__ __forceinline__ float highland(const Tables &T, float e, float t) {
+  if (t <= 0.f) return 0.f;
+  const float pc2 = e * (e + 2.0f * MP), bcp = pc2 / (e + MP);
+  return T.highland * 13.6f / bcp * sqrtf(t) * fmaxf(0.f, 1.0f + 0.038f * __logf(t));
+}
+// one MCS deflection: two independent projected Gaussians of width theta0 (Reading R3.4)
+__device__ __forceinline__ V3 deflect(V3 d, float theta0, uint32_t r0, uint32_t r1) {
+  const float th = theta0 * sqrtf(-2.0f * __logf(u01(r0)));
+  float st, ct, sp, cp;
+  sincosf(th, &st, &ct); sincospif(2.0f * u01(r1), &sp, &cp);
+  return unit(to_lab(d, st * cp, st * sp, ct));
+}
+
+// mean energy loss over water-equivalent path dr (g/cm2 of the table medium) from the range table
+// (Eq.2): E - E(R(E) - dr), written with expm1 so that a vanishing step loses nothing.
+__device__ __forceinline__ float mean_loss(const Tables &T, const float *lnE, const float *lnE2, int tab,
+                                           float e, float lnEv, float lnRv, float Rg, float dr) {
+  const float r1 = Rg - dr;
+  float lnE1 = T.ln_emin;
+  if (r1 > 0.f) lnE1 = ln_energy_of(T, lnE, lnE2, tab, lnRv + log1pf(-dr / Rg));
+  const float m = -e * expm1f(lnE1 - lnEv);
+  return fminf(fmaxf(m, 0.f), e);
+}
+
+// ------------------------------------------------------------------ K1: beam-spot sampler (Reading R2)
+__device__ __forceinline__ double u01d(uint32_t x) { return ((double)x + 0.5) * (1.0 / 4294967296.0); }
+
+__global__ void __launch_bounds__(256) sampler_kernel(Tables T, Grid G, const SpotDev *spots, const double *cdf, int nspots,
+                                                     RunParams P, Queue out, Counters *cnt, float air_rho, float air_wf,
+                                                     float air_inv_x0, float air_zoa, int air_table) {
+  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  double e_src = 0, e_esc = 0, e_air = 0; unsigned long long missed = 0;
+  if (i < P.n) {
+    const uint64_t hist = P.hist0 + i;
+    Rng g; g.init(P.seed, hist, 0u, 0u);
+    uint4 r = g.next4();
+    // spot ~ weight: first cdf entry >= u
+    const double us = u01d(r.x);
+    int lo = 0, hi = nspots - 1;
+    while (lo < hi) { int mid = (lo + hi) >> 1; if (cdf[mid] < us) lo = mid + 1; else hi = mid; }
+    const SpotDev sp = spots[lo];
+    const double rr = sqrt(-2.0 * log(u01d(r.y)));
+    double s2, c2; sincospi(2.0 * u01d(r.z), &s2, &c2);
+    double pos[3], dir[3];
+    for (int k = 0; k < 3; ++k) { pos[k] = sp.pos[k] + sp.sx * rr * c2 * sp.ex[k] + sp.sy * rr * s2 * sp.ey[k]; dir[k] = sp.ax[k]; }
+    if (sp.divx > 0 || sp.divy > 0) {
+      uint4 q = g.next4();
+      const double r2 = sqrt(-2.0 * log(u01d(q.x))); double s4, c4; sincospi(2.0 * u01d(q.y), &s4, &c4);
+      double n2 = 0;
+      for (int k = 0; k < 3; ++k) { dir[k] = sp.ax[k] + sp.divx * r2 * c4 * sp.ex[k] + sp.divy * r2 * s4 * sp.ey[k]; n2 += dir[k] * dir[k]; }
+      n2 = 1.0 / sqrt(n2); for (int k = 0; k < 3; ++k) dir[k] *= n2;
+    }
+    double E = sp.e;
+    if (sp.sigma_e > 0) { uint4 q = g.next4(); E += sp.sigma_e * sqrt(-2.0 * log(u01d(q.x))) * cospi(2.0 * u01d(q.y)); }
+    E = fmax(E, 0.0);
+    e_src = E;
+    const double size[3] = {G.nx * (double)G.d[0], G.ny * (double)G.d[1], G.nz * (double)G.d[2]};
+    auto ray_box = [&](const double *o, const double *dd, double &tin) {
+      double t0 = 0, t1 = 1e300;
+      for (int k = 0; k < 3; ++k) {
+        if (dd[k] == 0) { if (o[k] < 0 || o[k] > size[k]) return false; continue; }
+        double ta = (0 - o[k]) / dd[k], tb = (size[k] - o[k]) / dd[k];
+        if (ta > tb) { double s = ta; ta = tb; tb = s; }
+        t0 = fmax(t0, ta); t1 = fmin(t1, tb);
+      }
+      tin = t0; return t0 < t1;
+    };
+    double tin; bool ok = ray_box(pos, dir, tin);
+    if (!ok) { e_esc = E; missed = 1; }
+    else if (tin > 0) {
+      // single air step to the CT edge: hinge, Highland, mean loss + straggling
+      uint4 q = g.next4();
+      const double tau = u01d(q.x) * tin;
+      double rh[3]; for (int k = 0; k < 3; ++k) rh[k] = pos[k] + tau * dir[k];
+      double dn[3] = {dir[0], dir[1], dir[2]};
+      if (T.opt_mcs) {
+        V3 d1 = deflect(V3{(float)dir[0], (float)dir[1], (float)dir[2]}, highland(T, (float)E, (float)tin * air_rho * air_inv_x0), q.y, q.z);
+        dn[0] = d1.x; dn[1] = d1.y; dn[2] = d1.z;
+      }
+      double t2;
+      if (!ray_box(rh, dn, t2)) { e_esc = E; missed = 1; ok = false; }
+      else {
+        const double L = tau + t2;
+        for (int k = 0; k < 3; ++k) { pos[k] = rh[k] + t2 * dn[k]; dir[k] = dn[k]; }
+        const float ef = (float)E, lnEv = logf(fminf(fmaxf(ef, T.e_min), T.e_max));
+        const float lnRv = ln_range(T, T.lnR, T.lnR2, air_table, e_index(T, lnEv)), Rg = expf(lnRv);
+        float loss = mean_loss(T, T.lnE, T.lnE2, air_table, ef, lnEv, lnRv, Rg, (float)L * air_wf);
+        if (T.opt_strag) loss = straggle(T, g, ef, loss, (float)L * air_rho, air_zoa);
+        e_air = loss; E -= loss;
+        if (E <= T.e_cut) { e_air += E; ok = false; }
+      }
+    }
+    if (ok) {
+      Particle p; int idx[3]; const int nn[3] = {G.nx, G.ny, G.nz}; float loc[3];
+      for (int k = 0; k < 3; ++k) {
+        const double rv = fmin(fmax(pos[k], 0.0), size[k]), dk = (double)G.d[k];
+        int ii = (int)floor(rv / dk);
+        if (ii * dk == rv && dir[k] < 0) ii -= 1;
+        ii = min(max(ii, 0), nn[k] - 1);
+        idx[k] = ii; loc[k] = (float)fmin(fmax(rv - ii * dk, 0.0), dk);
+      }
+      p.r = {loc[0], loc[1], loc[2]}; p.d = unit(V3{(float)dir[0], (float)dir[1], (float)dir[2]}); p.e = (float)E;
+      p.vox = (idx[2] * G.ny + idx[1]) * G.nx + idx[0];
+      p.hist = i; p.pid = 0u; p.blk = g.blk; p.aux = 0u;
+      if (!queue_push(out, p)) atomicOr(&cnt->overflow, 1u);
+    }
+  }
+  flush(&cnt->e_source, e_src); flush(&cnt->e_escape, e_esc); flush(&cnt->e_air, e_air); flush(&cnt->n_missed, missed);
+}
+
+// ------------------------------------------------------------------ dose deposit (atomics)
+// Lanes of a warp that score into the same voxel in the same iteration are merged (warp match) so that a
+// single RED reaches the L2; with a pencil beam the lanes advance slab by slab and collide often.
+__device__ __forceinline__ void deposit(float *tally, int vox, float e, bool on, int aggregate) {
+  if (!aggregate) { if (on && e != 0.f) atomicAdd(tally + vox, e); return; }
+  const unsigned act = __ballot_sync(0xffffffffu, on);
+  if (!on) return;
+  const unsigned peers = __match_any_sync(act, vox);
+  const int lane = threadIdx.x & 31, leader = __ffs(peers) - 1;
+  float sum = e;
+  if (peers != (1u << lane)) {
+    // segmented reduction over the peer set
+    sum = 0.f;
+    unsigned m = peers;
+    while (m) { const int src = __ffs(m) - 1; m &= m - 1; sum += __shfl_sync(peers, e, src); }
+  }
+  if (lane == leader && sum != 0.f) atomicAdd(tally + vox, sum);
+}
+
+// ------------------------------------------------------------------ K2: condensed-history step kernel (Reading R3)
+// Persistent kernel: every lane pulls a particle from the input queue, steps it in registers until it stops,
+// leaves the grid or reaches a discrete nuclear event, then refills from the queue (warp-aggregated fetch).
+// Particles that reach an event are appended to the elastic or non-elastic queue; nothing else is written back.
+struct TransportSmem { int dummy; };
+
+__global__ void __launch_bounds__(256, 2) transport_kernel(Tables T, Grid G, RunParams P, Queue in, uint32_t n_in,
+                                                           uint32_t *head, Queue q_el, Queue q_ne, float *tally,
+                                                           Counters *cnt) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  // shared-memory staging of the stopping-power/range and cross-section tables (PAPER.md:L144 used textures)
+  float *s_lnR = reinterpret_cast<float *>(smem_raw);
+  float *s_lnR2 = s_lnR + T.n_sr * T.n_e;
+  float *s_lnE = s_lnR2 + T.n_sr * T.n_e;
+  float *s_lnE2 = s_lnE + T.n_sr * T.n_r;
+  float *s_sig = s_lnE2 + T.n_sr * T.n_r;
+  MatBin *s_bins = reinterpret_cast<MatBin *>(s_sig + T.nbins * T.n_e);
+  uint8_t *s_lut = reinterpret_cast<uint8_t *>(s_bins + T.nbins);
+  for (int i = threadIdx.x; i < T.n_sr * T.n_e; i += blockDim.x) { s_lnR[i] = T.lnR[i]; s_lnR2[i] = T.lnR2[i]; }
+  for (int i = threadIdx.x; i < T.n_sr * T.n_r; i += blockDim.x) { s_lnE[i] = T.lnE[i]; s_lnE2[i] = T.lnE2[i]; }
+  for (int i = threadIdx.x; i < T.nbins * T.n_e; i += blockDim.x) s_sig[i] = T.sig_bin[i];
+  for (int i = threadIdx.x; i < T.nbins * (int)(sizeof(MatBin) / 4); i += blockDim.x)
+    reinterpret_cast<uint32_t *>(s_bins)[i] = reinterpret_cast<const uint32_t *>(T.bins)[i];
+  for (int i = threadIdx.x; i < T.hu_lut_n; i += blockDim.x) s_lut[i] = T.hu_lut[i];
+  __syncthreads();
+
+  const float sz[3] = {G.d[0], G.d[1], G.d[2]};
+  const int lane = threadIdx.x & 31;
+  bool active = false, exhausted = false;
+  Particle p; Rng g; int ix = 0, iy = 0, iz = 0, nstep = 0; float path = 0.f;
+  unsigned long long c_steps = 0, c_el = 0, c_ne = 0;
+  double c_dep = 0, c_esc = 0;
+  const bool nuclear = T.opt_el || T.opt_ne;
+
+  while (true) {
+    // ---- refill idle lanes
+    const unsigned need = __ballot_sync(0xffffffffu, !active && !exhausted);
+    if (need) {
+      uint32_t base = 0;
+      if (lane == __ffs(need) - 1) base = atomicAdd(head, (uint32_t)__popc(need));
+      base = __shfl_sync(0xffffffffu, base, __ffs(need) - 1);
+      if (!active && !exhausted) {
+        const uint32_t idx = base + (uint32_t)__popc(need & ((1u << lane) - 1u));
+        if (idx < n_in) {
+          p = queue_load(in, idx);
+          g.init(P.seed, P.hist0 + p.hist, p.pid, p.blk);
+          ix = p.vox % G.nx; const int t = p.vox / G.nx; iy = t % G.ny; iz = t / G.ny;
+          active = true; nstep = 0; path = 0.f;
+        } else exhausted = true;
+      }
+    }
+    if (!__any_sync(0xffffffffu, active)) break;
+
+    float dep = 0.f; int dep_vox = p.vox;
+    if (active) {
+      // ---- material of the current voxel
+      const int hu = G.hu[p.vox];
+      const int bin = hu_to_bin(T, s_lut, hu);
+      const MatBin &m = s_bins[bin];
+      const float rho = bin_density(m, hu), wf = rho * m.wet;
+      const int tab = m.table;
+      c_steps++;
+      const uint4 r = g.next4();
+      // ---- 1. nuclear distance, face distance, residual range
+      const float e0 = p.e, lnEv = logf(fminf(fmaxf(e0, T.e_min), T.e_max));
+      const EIdx k = e_index(T, lnEv);
+      float lam = BIG;
+      if (nuclear) { const float Sig = rho * lerp_tab(s_sig + bin * T.n_e, k); if (Sig > 0.f) lam = -__logf(u01(r.x)) / Sig; }
+      int ax, sg; const float dface = dist_to_face(p.r, p.d, sz, ax, sg);
+      const float lnRv = ln_range(T, s_lnR, s_lnR2, tab, k), Rg = expf(lnRv);
+      const float R = Rg / wf, smax = T.s_max > 0.f ? T.s_max / wf : BIG;
+      // ---- 2. step = min (Reading R3.2)
+      float dx = lam; int lim = 2;
+      if (dface < dx) { dx = dface; lim = 1; }
+      if (R < dx) { dx = R; lim = 3; }
+      if (smax < dx) { dx = smax; lim = 0; }
+      // ---- 3-5. random hinge (PAPER.md:L69 ref [19]): first leg tau, deflect, second leg
+      float tau = 0.f; V3 dnew = p.d;
+      if (T.opt_mcs && dx > 0.f) {
+        tau = u01(r.y) * dx;
+        p.r = p.r + tau * p.d;
+        dnew = deflect(p.d, highland(T, e0, dx * rho * m.inv_x0), r.z, r.w);
+      }
+      const float ell = dx - tau; int ax2, sg2; const float d2 = dist_to_face(p.r, dnew, sz, ax2, sg2);
+      float L; int cls;
+      if (ell >= d2) { L = tau + d2; p.r = p.r + d2 * dnew; cls = 1; }
+      else { L = dx; p.r = p.r + ell * dnew; cls = (lim == 1) ? 0 : lim; }
+      p.r.x = fminf(fmaxf(p.r.x, 0.f), sz[0]); p.r.y = fminf(fmaxf(p.r.y, 0.f), sz[1]); p.r.z = fminf(fmaxf(p.r.z, 0.f), sz[2]);
+      p.d = dnew; path += L;
+      // ---- 6. energy loss from the range table (Eq.2) + straggling (L61)
+      float loss;
+      if (cls == 3) loss = e0;                                  // 7. range-out: everything stays here (L71)
+      else if (L <= 0.f) loss = 0.f;
+      else {
+        loss = mean_loss(T, s_lnE, s_lnE2, tab, e0, lnEv, lnRv, Rg, L * wf);
+        if (T.opt_strag) loss = straggle(T, g, e0, loss, L * rho, m.zoa);
+      }
+      p.e = e0 - loss; dep = loss;
+      bool alive = cls != 3;
+      if (alive && p.e <= T.e_cut) { dep += p.e; p.e = 0.f; alive = false; }           // L71 (2)
+      c_dep += (double)dep;
+      if (alive && cls == 1) {                                                        // boundary: next voxel
+        int nidx, nmax;
+        if (ax2 == 0) { ix += sg2; nidx = ix; nmax = G.nx; p.r.x = sg2 > 0 ? 0.f : sz[0]; }
+        else if (ax2 == 1) { iy += sg2; nidx = iy; nmax = G.ny; p.r.y = sg2 > 0 ? 0.f : sz[1]; }
+        else { iz += sg2; nidx = iz; nmax = G.nz; p.r.z = sg2 > 0 ? 0.f : sz[2]; }
+        if (nidx < 0 || nidx >= nmax) { c_esc += (double)p.e; alive = false; }         // L71 (3)
+        else p.vox = (iz * G.ny + iy) * G.nx + ix;
+      }
+      ++nstep;
+      if (alive && cls == 2) {
+        // ---- 8. discrete nuclear event at the end point (L71, L75; Reading R5): class, then target element
+        const float lnE1 = logf(fminf(fmaxf(p.e, T.e_min), T.e_max));
+        const EIdx k1 = e_index(T, lnE1);
+        float pel[MAX_ELEM], pne[MAX_ELEM], sel = 0.f, sne = 0.f;
+#pragma unroll
+        for (int i = 0; i < MAX_ELEM; ++i) {
+          pel[i] = 0.f; pne[i] = 0.f;
+          if (i < T.n_elem && m.nfac[i] > 0.f) {
+            if (T.opt_el) pel[i] = m.nfac[i] * lerp_tab(T.sig_el + i * T.n_e, k1);
+            if (T.opt_ne) pne[i] = m.nfac[i] * lerp_tab(T.sig_ne + i * T.n_e, k1);
+          }
+          sel += pel[i]; sne += pne[i];
+        }
+        if (sel + sne > 0.f) {
+          const uint4 q = g.next4();
+          const bool is_el = u01(q.x) * (sel + sne) < sel;
+          float u = u01(q.y) * (is_el ? sel : sne); int el = -1;
+#pragma unroll
+          for (int i = 0; i < MAX_ELEM; ++i) {
+            const float w = is_el ? pel[i] : pne[i];
+            if (w > 0.f && (el < 0 || u >= 0.f)) { el = i; u -= w; }
+          }
+          p.aux = (uint32_t)el; p.blk = g.blk; p.vox = dep_vox;
+          if (P.dbg_out == nullptr) {
+            if (is_el) { c_el++; if (!queue_push(q_el, p)) atomicOr(&cnt->overflow, 2u); }
+            else { c_ne++; if (!queue_push(q_ne, p)) atomicOr(&cnt->overflow, 4u); }
+            alive = false;
+          }
+        }
+      }
+      if (alive && P.max_steps > 0 && nstep >= P.max_steps) alive = false;
+      if (!alive) {
+        active = false;
+        if (P.dbg_out && p.pid == 0u) {
+          float *o = P.dbg_out + 8ull * p.hist;
+          o[0] = ix * sz[0] + p.r.x; o[1] = iy * sz[1] + p.r.y; o[2] = iz * sz[2] + p.r.z;
+          o[3] = p.d.x; o[4] = p.d.y; o[5] = p.d.z; o[6] = p.e; o[7] = path;
+        }
+      }
+    }
+    deposit(tally, dep_vox, dep, dep != 0.f, P.aggregate);
+  }
+  flush(&cnt->n_steps, c_steps); flush(&cnt->n_elastic, c_el); flush(&cnt->n_nonelastic, c_ne);
+  flush(&cnt->e_deposit, c_dep); flush(&cnt->e_escape, c_esc);
+}
+
+// ------------------------------------------------------------------ nuclear elastic (Eq.3; Reading R5)
+struct ElasticOut { float t_gev2, T_out, T_rec; V3 dir_out, dir_rec; };
+// proton of kinetic energy Tk along +z on nucleus of mass M (MeV); r = 4 random words
+__device__ __forceinline__ ElasticOut elastic_event(int A, float M, float Tk, uint4 r) {
+  const float E = Tk + MP, plab = sqrtf(Tk * (Tk + 2.0f * MP));
+  const float s = MP * MP + M * M + 2.0f * M * E, irs = rsqrtf(s), pcm = M * plab * irs;
+  const float tmax = 4.0f * pcm * pcm * 1e-6f;
+  float t;
+  if (A == 1) {
+    t = trunc_exp(cug_b_pp(plab * 1e-3f), tmax, u01(r.y));                  // p-p: Cugnon angular law
+  } else {
+    const float lA = __logf((float)A);
+    float a1, b1, a2, b2 = 10.0f;
+    if (A <= 62) { a1 = __expf(1.63f * lA); b1 = 14.5f * __expf(0.66f * lA); a2 = 1.4f * __expf(0.33f * lA); }
+    else { a1 = __expf(1.33f * lA); b1 = 60.0f * __expf(0.33f * lA); a2 = 0.4f * __expf(0.4f * lA); }
+    const float w1 = a1 * (1.0f - __expf(-b1 * tmax)) / b1, w2 = a2 * (1.0f - __expf(-b2 * tmax)) / b2;
+    const float bb = u01(r.x) * (w1 + w2) < w1 ? b1 : b2;
+    t = trunc_exp(bb, tmax, u01(r.y));                                      // |t|, truncated exponential
+  }
+  const float ct = 1.0f - 2.0f * t / tmax, st = sqrtf(fmaxf(0.f, 1.0f - ct * ct));
+  float sp, cp; sincospif(2.0f * u01(r.z), &sp, &cp);
+  // boost of the CM momenta along z with beta = plab/(E+M)
+  const float beta = plab / (E + M), gam = rsqrtf(1.0f - beta * beta);
+  const float Ep = sqrtf(pcm * pcm + MP * MP), Er = sqrtf(pcm * pcm + M * M);
+  V3 po{pcm * st * cp, pcm * st * sp, gam * (pcm * ct + beta * Ep)};
+  V3 pr{-po.x, -po.y, gam * (-pcm * ct + beta * Er)};
+  ElasticOut o;
+  o.t_gev2 = t;
+  o.T_rec = t * 1e6f / (2.0f * M);            // invariant: t = -2 M T_rec, free of the E - M cancellation
+  o.T_out = Tk - o.T_rec;
+  o.dir_out = unit(po);
+  o.dir_rec = dot(pr, pr) > 0.f ? unit(pr) : V3{0.f, 0.f, 1.f};
+  return o;
+}
+
+// K-elastic: one event per thread over the elastic queue; the scattered proton (and, for hydrogen, the recoil
+// proton) go to the next-generation transport queue; recoil nuclei deposit locally (L79 policy).
+__global__ void __launch_bounds__(256) elastic_kernel(Tables T, RunParams P, Queue in, Queue out, float *tally, Counters *cnt) {
+  const uint32_t n = min(*in.count, in.cap);
+  double c_dep = 0; unsigned long long c_sec = 0;
+  for (uint32_t i0 = blockIdx.x * blockDim.x; i0 < n; i0 += gridDim.x * blockDim.x) {
+    const uint32_t i = i0 + threadIdx.x;
+    if (i < n) {
+      Particle p = queue_load(in, i);
+      Rng g; g.init(P.seed, P.hist0 + p.hist, p.pid, p.blk);
+      const int el = (int)p.aux, Z = T.elem_z[el], A = T.elem_a[el];
+      const float M = (float)T.mass[Z * T.adim + A];
+      const ElasticOut o = elastic_event(A, M, p.e, g.next4());
+      const V3 d0 = p.d;
+      float dep = 0.f;
+      Particle s = p;
+      p.d = unit(to_lab(d0, o.dir_out.x, o.dir_out.y, o.dir_out.z)); p.e = o.T_out; p.aux = 0u;
+      bool push_rec = false;
+      if (A == 1 && o.T_rec > T.e_cut) {
+        s.d = unit(to_lab(d0, o.dir_rec.x, o.dir_rec.y, o.dir_rec.z)); s.e = o.T_rec;
+        s.pid = g.child_id(0u); s.blk = 0u; s.aux = 0u; push_rec = true; c_sec++;
+      } else dep += o.T_rec;
+      p.blk = g.blk;
+      const bool push_p = p.e > T.e_cut;
+      if (!push_p) dep += p.e;
+      if (push_p) { if (!queue_push(out, p)) atomicOr(&cnt->overflow, 8u); }
+      if (push_rec) { if (!queue_push(out, s)) atomicOr(&cnt->overflow, 8u); }
+      if (dep != 0.f) { atomicAdd(tally + p.vox, dep); c_dep += (double)dep; }
+    }
+  }
+  flush(&cnt->e_deposit, c_dep); flush(&cnt->n_secondary, c_sec);
+}
+
+// ------------------------------------------------------------------ K5: batch statistics (Reading R8)
+// After each batch: dose of the batch (Gy per primary) folded into a running mean and sum of squared
+// deviations (Welford), tally cleared.
+__global__ void __launch_bounds__(256) fold_kernel(Tables T, Grid G, float *tally, float *mean, float *m2, int b,
+                                                   float inv_nb, uint32_t nvox) {
+  for (uint32_t v = blockIdx.x * blockDim.x + threadIdx.x; v < nvox; v += gridDim.x * blockDim.x) {
+    const float t = tally[v];
+    float d = 0.f;
+    if (t != 0.f) {
+      const int hu = G.hu[v];
+      const MatBin &m = T.bins[hu_to_bin(T, T.hu_lut, hu)];
+      d = t / (bin_density(m, hu) * G.vol) * inv_nb * 1.602176634e-10f;
+      tally[v] = 0.f;
+    }
+    const float mu = b == 0 ? 0.f : mean[v], s = b == 0 ? 0.f : m2[v];
+    const float delta = d - mu, mu1 = mu + delta / (float)(b + 1);
+    mean[v] = mu1; m2[v] = s + delta * (d - mu1);
+  }
+}
+__global__ void __launch_bounds__(256) finish_kernel(const float *mean, const float *m2, float *dose, float *sigma,
+                                                     int B, uint32_t nvox) {
+  for (uint32_t v = blockIdx.x * blockDim.x + threadIdx.x; v < nvox; v += gridDim.x * blockDim.x) {
+    dose[v] = mean[v];
+    const float var = m2[v] / ((float)B * (float)(B - 1));
+    sigma[v] = var > 0.f ? sqrtf(var) : 0.f;
+  }
+}
+
+}  // namespace pmc
