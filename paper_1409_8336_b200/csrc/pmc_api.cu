@@ -70,7 +70,7 @@ struct pmc_ctx {
   std::vector<double> h_lnR, h_lnR2, h_lnrlo, h_lnrhi, h_lnE, h_lnE2, h_sne, h_sel, h_mass, h_ek, h_ec;
   std::vector<int> ez, ea;
   double e_cut = 0.1, highland = 1.07, kappa_g = 10, s_max = 0.2; int n_batches = 10;
-  bool opt_strag = true, opt_mcs = true, opt_el = true, opt_ne = true; int aggregate = 1;
+  bool opt_strag = true, opt_mcs = true, opt_el = true, opt_ne = true; int aggregate = 1; bool profile = false;
   uint64_t chunk = 1u << 21, history_offset = 0;
   std::vector<HostMat> mats;
   // device tables
@@ -445,6 +445,7 @@ int pmc_set_option(pmc_ctx *c, const char *key, double v) {
   else if (k == "chunk_histories") { if (v < 1 || v > 67108864.0) return fail(c, PMC_E_INVALID_ARG, "chunk_histories out of range"); c->chunk = (uint64_t)v; }
   else if (k == "history_offset") { if (v < 0) return fail(c, PMC_E_INVALID_ARG, "negative offset"); c->history_offset = (uint64_t)v; }
   else if (k == "dose_aggregate") c->aggregate = v != 0;
+  else if (k == "profile") c->profile = v != 0;
   else return fail(c, PMC_E_INVALID_ARG, "unknown option");
   c->tables_dirty = true;
   return PMC_OK;
@@ -472,7 +473,7 @@ static int simulate_impl(pmc_ctx *c, const pmc_spot *spots_in, int nspots, uint6
   CK(cudaMemsetAsync(c->d_tally.p, 0, (size_t)nvox * 4, s)); CK(cudaMemsetAsync(c->d_cnt.p, 0, sizeof(Counters), s));
   c->counters = pmc_counters{}; c->timing = pmc_timing{};
   float air_rho, air_wf, air_ix0, air_zoa; int air_tab; air_params(c, air_rho, air_wf, air_ix0, air_zoa, air_tab);
-  const bool profile = false;
+  const bool profile = c->profile;
   cudaEvent_t e0, e1; CK(cudaEventCreate(&e0)); CK(cudaEventCreate(&e1));
   CK(cudaEventRecord(e0, s));
   const int grid_v = c->n_sm * 8;
@@ -483,7 +484,8 @@ static int simulate_impl(pmc_ctx *c, const pmc_spot *spots_in, int nspots, uint6
       RunParams P{}; P.seed = seed; P.hist0 = c->history_offset + cs; P.n = nc; P.max_steps = max_steps; P.dbg_out = dbg_out ? dbg_out + 8ull * (cs - h0) : nullptr;
       P.aggregate = c->aggregate;
       CK(cudaMemsetAsync(c->qa.q.count, 0, 4, s));
-      sampler_kernel<<<(nc + 255) / 256, 256, 0, s>>>(c->T, c->G, c->d_spots.p, c->d_cdf.p, nspots, P, c->qa.q, c->d_cnt.p, air_rho, air_wf, air_ix0, air_zoa, air_tab);
+      { Timer t(c, &c->timing.sampler_ms, profile);
+        sampler_kernel<<<(nc + 255) / 256, 256, 0, s>>>(c->T, c->G, c->d_spots.p, c->d_cdf.p, nspots, P, c->qa.q, c->d_cnt.p, air_rho, air_wf, air_ix0, air_zoa, air_tab); }
       c->timing.launches_total++;
       CK(cudaMemcpyAsync(c->h_pinned, c->qa.q.count, 4, cudaMemcpyDeviceToHost, s));
       CK(cudaStreamSynchronize(s));
@@ -491,7 +493,8 @@ static int simulate_impl(pmc_ctx *c, const pmc_spot *spots_in, int nspots, uint6
     }
     if (!dbg_out) {
       const float inv_nb = h1 > h0 ? (float)(1.0 / (double)(h1 - h0)) : 0.f;
-      fold_kernel<<<grid_v, 256, 0, s>>>(c->T, c->G, c->d_tally.p, c->d_mean.p, c->d_m2.p, b, inv_nb, nvox);
+      { Timer t(c, &c->timing.statistics_ms, profile);
+        fold_kernel<<<grid_v, 256, 0, s>>>(c->T, c->G, c->d_tally.p, c->d_mean.p, c->d_m2.p, b, inv_nb, nvox); }
       c->timing.launches_total++;
     }
   }
