@@ -1,0 +1,309 @@
+#!/usr/bin/env python
+"""bench.py — proton histories/s of the full-physics hot path (pmc_simulate) on config C4, with roofline,
+end-to-end (host-buffer) throughput and the fp64 CPU oracle timed beside it.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload c4|c1|c3_150|c5]
+
+One "step" = one pmc_simulate call: the whole hot path (spot sampler, condensed-history transport, elastic, INC,
+evaporation, 10-batch statistics) over `--histories` primaries (default: the workload's own count, 1e7 for C4).
+N > 1 (torchrun, one rank per GPU): weak scaling, every rank simulates the same number of histories with
+disjoint global history ids; the per-rank doses are combined with one NCCL all-reduce per step.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "proton histories/sec (full physics, dose on CT grid)"
+UNIT = "histories/s"
+# algorithmic thread-instructions of one condensed-history step of the transport kernel
+ALGO_INST_PER_STEP = 520.0
+ISSUE_LANES_PER_SM_PER_CLK = 128.0     # 4 schedulers x 32 lanes
+N_SM = 148
+
+
+def _env_int(k, d):
+    try:
+        return int(os.environ.get(k, d))
+    except ValueError:
+        return d
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md clocks line)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.idx = gpu_index
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+
+    def start(self):
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(self.idx), f"--query-gpu={self.Q}",
+                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                      stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush(); self.f.seek(0)
+        sm, mx, reasons = [], [], set()
+        for line in self.f.read().splitlines():
+            c = [x.strip() for x in line.split(",")]
+            if len(c) < 9:
+                continue
+            try:
+                sm.append(float(c[1])); mx.append(float(c[2]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), c[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        try:
+            os.unlink(self.f.name)
+        except OSError:
+            pass
+        if sm:
+            sm.sort()
+            out.update(sm_mhz=sm[len(sm) // 2], sm_max_mhz=max(mx), reasons=sorted(reasons), samples=len(sm))
+        return out
+
+
+def _cores():
+    try:
+        return len(os.sched_getaffinity(0))
+    except AttributeError:
+        return os.cpu_count() or 1
+
+
+def time_oracle(w, tables, target_s, seed):
+    """The oracle as it stands on the host cores, on a bounded sample of the workload -> (hist/s, n, seconds)."""
+    from oracle import Oracle
+    o = Oracle(tables, w["materials"])
+    o.load_ct(w["hu"], w["vox"])
+    n = 20000
+    t0 = time.perf_counter(); o.simulate(w["spots"], n, seed); dt = time.perf_counter() - t0
+    rate = n / dt
+    n2 = int(min(max(rate * target_s, 20000), 5_000_000))
+    if n2 > 2 * n:
+        t0 = time.perf_counter(); o.simulate(w["spots"], n2, seed + 1); dt = time.perf_counter() - t0
+        n = n2
+    return n / dt, n, dt
+
+
+def run_reference(args, rank):
+    """--impl reference: the fp64 oracle on the host cores, bounded sample per step (rank 0 only)."""
+    if rank != 0:
+        return
+    import inputs
+    w = inputs.workload(args.workload)
+    tables = inputs.make_physics_tables()
+    from oracle import Oracle
+    o = Oracle(tables, w["materials"]); o.load_ct(w["hu"], w["vox"])
+    n = 20000
+    t0 = time.perf_counter(); o.simulate(w["spots"], n, 1000); dt = time.perf_counter() - t0
+    budget = 150.0 / max(1, args.steps + args.warmup)
+    n_step = int(min(max(n / dt * min(budget, 20.0), 5000), 2_000_000))
+    for i in range(args.warmup):
+        o.simulate(w["spots"], n_step, 2000 + i)
+    t0 = time.perf_counter()
+    for i in range(args.steps):
+        o.simulate(w["spots"], n_step, 3000 + i)
+    dt = time.perf_counter() - t0
+    v = n_step * args.steps / dt
+    sample = f"{n_step} histories of {w['name']} per step (of {w['n_histories']})"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": w["label"], "histories_per_step": n_step, "n_spots": w["n_spots"]},
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": _cores(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="c4")
+    ap.add_argument("--histories", type=int, default=0, help="histories per step and per rank (0 = the workload's)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    args = ap.parse_args()
+    rank, local_rank, world = _env_int("RANK", 0), _env_int("LOCAL_RANK", 0), _env_int("WORLD_SIZE", 1)
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    import inputs
+    from paper_1409_8336_b200 import Pmc
+    from paper_1409_8336_b200.sharding import weak_shard, combine_dose
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=dev)
+
+    w = inputs.workload(args.workload)
+    tables = inputs.make_physics_tables()
+    n_hist = args.histories or w["n_histories"]
+    stream = torch.cuda.Stream(device=dev)
+    pm = Pmc(local_rank, stream=stream)
+    pm.load_physics_tables(tables)
+    pm.set_hu_materials(w["materials"])
+    hu_dev = torch.as_tensor(w["hu"], device=dev)
+    pm.load_ct(hu_dev, w["vox"])
+    offset, _ = weak_shard(n_hist, rank)
+    pm.set_option("history_offset", float(offset))
+    spots = w["spots"]
+    nvox = int(w["hu"].size)
+    dose = torch.empty(w["hu"].shape, dtype=torch.float32, device=dev)
+    sigma = torch.empty_like(dose)
+    l2_flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # > 126 MB L2
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    def step(i):
+        pm.simulate(spots, n_hist, w["seed"] + i, out=(dose, sigma))
+        if world > 1:
+            with torch.cuda.stream(stream):
+                combine_dose(dose, sigma, n_hist)
+
+    for i in range(args.warmup):
+        step(i)
+    barrier()
+
+    # ---- device-resident timing: K steps, CUDA events on the library's stream, L2 flushed between steps
+    sampler = ClockSampler(local_rank); sampler.start()
+    time.sleep(0.3)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    t_transport = 0.0; n_transport = 0; launches = 0; steps_total = 0
+    klass = {k: 0.0 for k in ("sampler_ms", "transport_ms", "elastic_ms", "inc_ms", "evaporation_ms", "statistics_ms")}
+    cnt_last = None
+    barrier()
+    for i in range(args.steps):
+        with torch.cuda.stream(stream):
+            l2_flush.fill_(i & 0xFF)
+        ev[i][0].record(stream)
+        step(args.warmup + i)
+        ev[i][1].record(stream)
+        tm, cnt_last = pm.timing(), pm.counters()
+        t_transport += tm["transport_ms"]; n_transport += tm["launches_transport"]; launches += tm["launches_total"]
+        steps_total += cnt_last["n_steps"]
+        for k in klass:
+            klass[k] += tm[k]
+    barrier()
+    clocks = sampler.stop()
+    ms = sum(a.elapsed_time(b) for a, b in ev)
+    t = torch.tensor([ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms = float(t.item())
+    value = world * n_hist * args.steps / (ms * 1e-3)
+
+    # ---- end to end through the C-ABI with HOST buffers: HU grid + spots host->device, dose + sigma device->host
+    hu_pin = torch.as_tensor(w["hu"]).pin_memory()
+    dose_h = torch.empty(w["hu"].shape, dtype=torch.float32).pin_memory()
+    sigma_h = torch.empty_like(dose_h).pin_memory()
+    e2e_steps = max(1, min(args.steps, 3))
+    pm.load_ct(hu_pin.numpy(), w["vox"]); pm.simulate_host(spots, n_hist, 99, dose_h.numpy(), sigma_h.numpy())   # warm
+    barrier()
+    t0 = time.perf_counter()
+    for i in range(e2e_steps):
+        pm.load_ct(hu_pin.numpy(), w["vox"])
+        pm.simulate_host(spots, n_hist, w["seed"] + 100 + i, dose_h.numpy(), sigma_h.numpy())
+    torch.cuda.synchronize(dev)
+    e2e_s = time.perf_counter() - t0
+    t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    e2e_value = world * n_hist * e2e_steps / float(t.item())
+    h2d = int(w["hu"].nbytes + spots.nbytes)
+    d2h = int(2 * nvox * 4)
+
+    if rank == 0:
+        # ---- roofline of the dominant kernel (transport_kernel): plain-ALU issue bound
+        sm_mhz = clocks["sm_mhz"] or 1965.0
+        peak = N_SM * ISSUE_LANES_PER_SM_PER_CLK * sm_mhz * 1e6 / 1e9            # G thread-inst/s at the clock seen
+        achieved = ALGO_INST_PER_STEP * steps_total / (t_transport * 1e-3) / 1e9 if t_transport > 0 else 0.0
+        roofline = {"bound": "alu", "kernel": "transport_kernel", "achieved": achieved, "peak": peak,
+                    "unit": "Gthread-inst/s", "frac": achieved / peak if peak else None, "traffic": None,
+                    "peak_source": "148 SMs x 4 schedulers x 32 lanes x median SM clock under load (derived, DESIGN.md)",
+                    "avg_launch_ms": t_transport / max(1, n_transport), "launches": n_transport,
+                    "algorithmic_inst_per_condensed_step": ALGO_INST_PER_STEP,
+                    "condensed_steps_per_history": steps_total / (n_hist * args.steps),
+                    "kernel_share_of_step": t_transport / ms if ms else None,
+                    "hbm_gbs_peak_measured": _measured_hbm()}
+        cpu = None
+        if not args.no_cpu_baseline:
+            v, n_s, dt = time_oracle(w, tables, args.cpu_seconds, 777)
+            cpu = {"value": v, "unit": UNIT, "cores": _cores(), "kind": "oracle",
+                   "sample": f"{n_s} histories of {w['name']} ({dt:.1f} s, OpenMP over histories, fp64)"}
+        out = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": w["label"], "histories_per_step_per_gpu": n_hist, "n_spots": w["n_spots"],
+                       "n_batches": 10, "l2": "flushed between timed steps (256 MiB write)",
+                       "parallelism": f"history-sharded x{world}"},
+            "clocks": {k: clocks[k] for k in ("sm_mhz", "sm_max_mhz", "reasons")},
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                    "steps": e2e_steps},
+            "gpu_launches": int(launches),
+            "roofline": roofline, "cpu_baseline": cpu,
+            "kernel_ms_per_step": {k: v / args.steps for k, v in klass.items()},
+            "counters_last_step": {k: cnt_last[k] for k in ("n_steps", "n_elastic", "n_nonelastic",
+                                                            "n_secondary_protons", "n_generations", "n_missed")},
+            "context": "paper: ~20 s per 1e7 histories on a GTX680 incl. transfers (PAPER.md:L15), i.e. ~5e5 hist/s",
+        }
+        print(json.dumps(out))
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def _measured_hbm():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return json.load(f).get("hbm_gbs")
+    except (OSError, ValueError):
+        return None
+
+
+if __name__ == "__main__":
+    main()

@@ -130,7 +130,8 @@ int  pmc_load_ct_host(pmc_ctx *ctx, const int16_t *hu_host, int nx, int ny, int 
 /* Options: "straggling" "mcs" "elastic" "nonelastic" (0/1), "s_max_wet_cm", "n_batches",
  * "chunk_histories" (histories per sub-group), "history_offset" (first history id, for sharding
  * a run over several GPUs), "dose_aggregate" (0/1 warp-aggregated dose atomics),
- * "profile" (0/1: time every kernel class with CUDA events into pmc_timing; serialises the launches). */
+ * "profile" (0/1, default 1: a CUDA-event pair is recorded on the context's stream around every kernel launch and
+ * resolved into pmc_timing at the end of the call; no extra synchronisation). */
 int  pmc_set_option(pmc_ctx *ctx, const char *key, double value);
 
 /* PAPER.md:L134-138 (Fig 2): simulate n_histories primaries drawn from the spot list (HOST, nspots entries),

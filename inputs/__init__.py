@@ -13,3 +13,4 @@ from .physics_tables import make_physics_tables, ELEMENTS  # noqa: F401
 from .materials import make_materials_c1, make_materials_24  # noqa: F401
 from .phantoms import phantom_c1, phantom_c3, phantom_c4, phantom_c5  # noqa: F401
 from .plans import plan_single_spot, plan_c4, plan_c5  # noqa: F401
+from .workloads import workload  # noqa: F401

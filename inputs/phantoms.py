@@ -48,8 +48,14 @@ def phantom_c4(seed=4, nx=256, ny=256, nz=120, vox=(0.1, 0.1, 0.25)):
     soft = np.clip(rng.normal(40.0, 20.0, size=shape), -100, 120).astype(np.int16)
     head_c, head_r = (cx, cy, 0.68 * lz), (8.0, 9.5, 0.30 * lz)
     neck_c, neck_r = (cx, cy + 0.5, 0.22 * lz), (5.5, 6.0, 0.30 * lz)
-    body = _ellipsoid_mask(shape, vox, head_c, head_r) | _ellipsoid_mask(shape, vox, neck_c, neck_r)
+    # shoulders (low slices): wide enough that a lateral field to the low-neck target needs ~20 cm WET (~190 MeV)
+    sh_c, sh_r = (cx, cy + 0.5, 0.0), (12.4, 7.0, 0.22 * lz)
+    body = (_ellipsoid_mask(shape, vox, head_c, head_r) | _ellipsoid_mask(shape, vox, neck_c, neck_r)
+            | _ellipsoid_mask(shape, vox, sh_c, sh_r))
     hu[body] = soft[body]
+    for sgn in (-1.0, 1.0):     # humeral heads
+        m = _ellipsoid_mask(shape, vox, (cx + sgn * 9.0, cy + 0.5, 0.05 * lz), (2.2, 2.2, 0.12 * lz))
+        hu[m] = rng.integers(700, 1501, size=int(m.sum())).astype(np.int16)
     # skull shell
     inner = _ellipsoid_mask(shape, vox, head_c, tuple(r - 0.7 for r in head_r))
     outer = _ellipsoid_mask(shape, vox, head_c, tuple(r - 0.2 for r in head_r))
@@ -70,8 +76,9 @@ def phantom_c4(seed=4, nx=256, ny=256, nz=120, vox=(0.1, 0.1, 0.25)):
         c = (cx + 3.2 * np.cos(ang), cy - 3.5 - 3.0 * np.sin(ang), 0.47 * lz)
         m = _ellipsoid_mask(shape, vox, c, (0.35, 0.35, 0.6))
         hu[m] = rng.integers(2000, 3001, size=int(m.sum())).astype(np.int16)
-    targets = [((cx - 2.5, cy + 0.5, 0.40 * lz), (1.6, 1.8, 2.2)),
-               ((cx + 3.0, cy - 1.0, 0.30 * lz), (1.2, 1.2, 1.6))]
+    targets = [((cx - 2.5, cy + 0.5, 0.40 * lz), (1.4, 1.5, 1.9)),
+               ((cx + 3.0, cy - 1.0, 0.30 * lz), (1.0, 1.0, 1.4)),
+               ((cx + 4.5, cy + 0.5, 0.09 * lz), (1.2, 1.2, 1.3))]      # low-neck node behind the shoulder
     return hu, vox, targets
 
 

@@ -70,7 +70,7 @@ struct pmc_ctx {
   std::vector<double> h_lnR, h_lnR2, h_lnrlo, h_lnrhi, h_lnE, h_lnE2, h_sne, h_sel, h_mass, h_ek, h_ec;
   std::vector<int> ez, ea;
   double e_cut = 0.1, highland = 1.07, kappa_g = 10, s_max = 0.2; int n_batches = 10;
-  bool opt_strag = true, opt_mcs = true, opt_el = true, opt_ne = true; int aggregate = 1; bool profile = false;
+  bool opt_strag = true, opt_mcs = true, opt_el = true, opt_ne = true; int aggregate = 1; bool profile = true;
   uint64_t chunk = 1u << 21, history_offset = 0;
   std::vector<HostMat> mats;
   // device tables
@@ -89,6 +89,7 @@ struct pmc_ctx {
   int n_sm = 148; size_t smem_transport = 0;
   pmc_counters counters{}; pmc_timing timing{};
   cudaEvent_t ev[2] = {nullptr, nullptr};
+  std::vector<cudaEvent_t> ev_pool; size_t ev_used = 0; std::vector<float *> ev_acc;
 };
 
 namespace {
@@ -243,11 +244,27 @@ int prepare_spots(pmc_ctx *c, const pmc_spot *spots, int nspots) {
   return PMC_OK;
 }
 
+// Always-on per-kernel-class timing: an event pair from a pool is recorded around every launch on the context's
+// stream (no synchronisation); the pairs are resolved once at the end of the call, after the stream is idle.
 struct Timer {
-  pmc_ctx *c; float *acc; bool on;
-  Timer(pmc_ctx *c_, float *a, bool on_) : c(c_), acc(a), on(on_) { if (on) cudaEventRecord(c->ev[0], c->stream); }
-  ~Timer() { if (on) { cudaEventRecord(c->ev[1], c->stream); cudaEventSynchronize(c->ev[1]); float ms = 0; cudaEventElapsedTime(&ms, c->ev[0], c->ev[1]); *acc += ms; } }
+  pmc_ctx *c; size_t i; bool on;
+  Timer(pmc_ctx *c_, float *a, bool on_) : c(c_), i(0), on(on_) {
+    if (!on) return;
+    if (c->ev_used + 2 > c->ev_pool.size()) {
+      for (int k = 0; k < 64; ++k) { cudaEvent_t e = nullptr; if (cudaEventCreate(&e) != cudaSuccess) { on = false; return; } c->ev_pool.push_back(e); }
+    }
+    i = c->ev_used; c->ev_used += 2; c->ev_acc.push_back(a);
+    cudaEventRecord(c->ev_pool[i], c->stream);
+  }
+  ~Timer() { if (on) cudaEventRecord(c->ev_pool[i + 1], c->stream); }
 };
+void resolve_timers(pmc_ctx *c) {       // stream must be idle
+  for (size_t k = 0; k < c->ev_acc.size(); ++k) {
+    float ms = 0;
+    if (cudaEventElapsedTime(&ms, c->ev_pool[2 * k], c->ev_pool[2 * k + 1]) == cudaSuccess) *c->ev_acc[k] += ms;
+  }
+  c->ev_used = 0; c->ev_acc.clear();
+}
 
 // The event-based scheduler (north_star; replaces the paper's transport kernel + Thrust collect/sort, L136):
 // generation loop over compacted queues until every queue is empty.
@@ -344,6 +361,7 @@ void pmc_destroy(pmc_ctx *c) {
   c->d_spots.release(); c->d_cdf.release(); c->d_slots.release(); c->d_counts.release(); c->d_base.release();
   if (c->h_pinned) cudaFreeHost(c->h_pinned);
   if (c->ev[0]) { cudaEventDestroy(c->ev[0]); cudaEventDestroy(c->ev[1]); }
+  for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
   delete c;
 }
 
@@ -474,6 +492,7 @@ static int simulate_impl(pmc_ctx *c, const pmc_spot *spots_in, int nspots, uint6
   c->counters = pmc_counters{}; c->timing = pmc_timing{};
   float air_rho, air_wf, air_ix0, air_zoa; int air_tab; air_params(c, air_rho, air_wf, air_ix0, air_zoa, air_tab);
   const bool profile = c->profile;
+  c->ev_used = 0; c->ev_acc.clear();
   cudaEvent_t e0, e1; CK(cudaEventCreate(&e0)); CK(cudaEventCreate(&e1));
   CK(cudaEventRecord(e0, s));
   const int grid_v = c->n_sm * 8;
@@ -502,6 +521,7 @@ static int simulate_impl(pmc_ctx *c, const pmc_spot *spots_in, int nspots, uint6
   CK(cudaEventRecord(e1, s));
   CK(cudaGetLastError());
   rc = fetch_counters(c);
+  resolve_timers(c);
   float ms = 0; cudaEventElapsedTime(&ms, e0, e1); c->timing.total_ms = ms;
   cudaEventDestroy(e0); cudaEventDestroy(e1);
   return rc;
