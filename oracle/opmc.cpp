@@ -585,12 +585,13 @@ bool transport_step(opmc_ctx *c, Particle &p, Rng &g, double *tally, Ledger &led
   }
   double ell = dx - tau; int ax2, sg2; double d2 = dist_to_face(c, p.r, dnew, p.idx, ax2, sg2);
   double L; int cls;
-  if (ell >= d2) {                                 // ends on a face: boundary step whatever limited dx
+  if (ell >= d2 || lim == 1) {                     // ends on a face: boundary step whatever limited dx; a face-limited
+                                                   // step is always carried to the face (L69; Reading R3.5)
     L = tau + d2; p.r = p.r + d2 * dnew;
     double face = sg2 > 0 ? (p.idx[ax2] + 1) * c->d[ax2] : p.idx[ax2] * c->d[ax2];
     (ax2 == 0 ? p.r.x : ax2 == 1 ? p.r.y : p.r.z) = face;
     cls = 1;
-  } else { L = dx; p.r = p.r + ell * dnew; cls = (lim == 1) ? 0 : lim; }
+  } else { L = dx; p.r = p.r + ell * dnew; cls = lim; }
   p.d = dnew;
   if (pathlen) *pathlen += L;
   // 6. energy loss from the range table (L61-63, Eq.2) + straggling

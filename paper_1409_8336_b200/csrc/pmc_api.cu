@@ -592,14 +592,14 @@ int pmc_get_timing(pmc_ctx *c, pmc_timing *o) { if (!c || !o) return PMC_E_INVAL
 
 // ---- sub-step entry points
 int pmc_philox4x32_10(pmc_ctx *c, const uint32_t *in_dev, uint64_t n, uint32_t *out_dev) {
-  if (!c || !in_dev || !out_dev) return fail(c, PMC_E_INVALID_ARG, "null argument");
+  if (!c || (n && (!in_dev || !out_dev))) return fail(c, PMC_E_INVALID_ARG, "null argument");
   cudaSetDevice(c->device);
   if (n) philox_kernel<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(in_dev, n, out_dev);
   CK(cudaStreamSynchronize(c->stream)); CK(cudaGetLastError());
   return PMC_OK;
 }
 static int range_impl(pmc_ctx *c, int table, const float *in, uint64_t n, float *out, int inverse) {
-  if (!c || !in || !out) return fail(c, PMC_E_INVALID_ARG, "null argument");
+  if (!c || (n && (!in || !out))) return fail(c, PMC_E_INVALID_ARG, "null argument");
   if (!c->have_tables) return fail(c, PMC_E_STATE, "load physics tables first");
   if (table < 0 || table >= c->n_sr) return fail(c, PMC_E_INVALID_ARG, "bad table id");
   cudaSetDevice(c->device);

@@ -216,7 +216,8 @@ __device__ float straggle(const Tables &T, Rng &g, float e_start, float mean_los
     loss = mean_loss + sqrtf(xi * tmax * (1.0f - 0.5f * b2)) * z;
   } else {
     const float itmax = 1.0f / tmax;
-    float tc = fmaxf(fminf(1e-3f, 0.01f * tmax), 1.0f / (MU_HARD / xi + itmax));
+    const float tc0 = fminf(1e-3f, 0.01f * tmax);                            // Reading R4: below tc0 the soft part is Gaussian
+    float tc = fmaxf(tc0, 1.0f / (MU_HARD / xi + itmax));
     tc = fminf(tc, tmax);
     const float itc = 1.0f / tc, ltc = __logf(tmax * itc);
     const float mu_c = xi * (itc - itmax);                                   // candidates (before thinning)
@@ -233,14 +234,20 @@ __device__ float straggle(const Tables &T, Rng &g, float e_start, float mean_los
       const float t = 1.0f / (itc - u01(ra) * (itc - itmax));
       if (u01(rb) < 1.0f - b2 * t * itmax) hard += t;
     }
-    // soft part: cumulants k2 = xi tc (1 - b2 tc/2Tmax), k3 = xi tc^2 (1/2 - b2 tc/3Tmax), k4 = xi tc^3 (1/3 - b2 tc/4Tmax)
-    const float x = b2 * tc * itmax;
+    // soft part: variance k2 = xi tc (1 - b2 tc/2Tmax) of everything below tc; the 3rd and 4th cumulants
+    // k3 = xi (tc^2 - tc0^2)(1/2 - ..), k4 = xi (tc^3 - tc0^3)(1/3 - ..) only of the collisions in [tc0, tc] that were
+    // moved from the hard to the soft part, so that at tc = tc0 the sampler is the Gaussian of Reading R4 and the
+    // skewness never exceeds 1/4 (tc <= xi/MU_HARD), where the Cornish-Fisher expansion is monotone.
+    const float x = b2 * tc * itmax, f0 = tc0 * itc;
     const float k2 = xi * tc * (1.0f - 0.5f * x);
-    const float g1 = xi * tc * tc * (0.5f - x * (1.0f / 3.0f)) / (k2 * sqrtf(k2));
-    const float g2 = xi * tc * tc * tc * ((1.0f / 3.0f) - 0.25f * x) / (k2 * k2);
-    const float z2 = z * z;
-    const float cf = z + g1 * (1.0f / 6.0f) * (z2 - 1.0f) + g2 * (1.0f / 24.0f) * z * (z2 - 3.0f)
-                     - g1 * g1 * (1.0f / 36.0f) * z * (2.0f * z2 - 5.0f);
+    float cf = z;
+    if (tc > tc0) {
+      const float g1 = (1.0f - f0 * f0) * xi * tc * tc * (0.5f - x * (1.0f / 3.0f)) / (k2 * sqrtf(k2));
+      const float g2 = (1.0f - f0 * f0 * f0) * xi * tc * tc * tc * ((1.0f / 3.0f) - 0.25f * x) / (k2 * k2);
+      const float z2 = z * z;
+      cf = z + g1 * (1.0f / 6.0f) * (z2 - 1.0f) + g2 * (1.0f / 24.0f) * z * (z2 - 3.0f)
+           - g1 * g1 * (1.0f / 36.0f) * z * (2.0f * z2 - 5.0f);
+    }
     loss = mean_loss + (hard - mean_hard) + sqrtf(k2) * cf;
   }
   return fminf(fmaxf(loss, 0.f), e_start);

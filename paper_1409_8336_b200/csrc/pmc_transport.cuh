@@ -256,8 +256,9 @@ __global__ void __launch_bounds__(256, 2) transport_kernel(Tables T, Grid G, Run
       }
       const float ell = dx - tau; int ax2, sg2; const float d2 = dist_to_face(p.r, dnew, sz, ax2, sg2);
       float L; int cls;
-      if (ell >= d2) { L = tau + d2; p.r = p.r + d2 * dnew; cls = 1; }
-      else { L = dx; p.r = p.r + ell * dnew; cls = (lim == 1) ? 0 : lim; }
+      // a face-limited step always ends on a face (dx = distance to the voxel boundary; Reading R3.5)
+      if (ell >= d2 || lim == 1) { L = tau + d2; p.r = p.r + d2 * dnew; cls = 1; }
+      else { L = dx; p.r = p.r + ell * dnew; cls = lim; }
       p.r.x = fminf(fmaxf(p.r.x, 0.f), sz[0]); p.r.y = fminf(fmaxf(p.r.y, 0.f), sz[1]); p.r.z = fminf(fmaxf(p.r.z, 0.f), sz[2]);
       p.d = dnew; path += L;
       // ---- 6. energy loss from the range table (Eq.2) + straggling (L61)

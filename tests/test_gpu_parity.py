@@ -1,0 +1,433 @@
+"""GPU parity tests (`-m gpu`): the CUDA path, called through the C-ABI of include/pmc.h, against the fp64 oracle.
+
+Philox is compared bit for bit; table evaluation element by element; everything downstream statistically with
+north_star's tolerances (identical Philox streams diverge at fp32-vs-fp64 branch points):
+integrated dose 0.5 %, >= 99 % of voxels above 10 % of the maximum within 3 combined sigma, R80 and distal
+fall-off 0.2 mm, secondary yields 3 sigma, charge / baryon number exact.
+"""
+import numpy as np
+import pytest
+import torch
+
+import inputs
+import parity
+from oracle import Oracle
+from oracle import binding as ob
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def pm(tables):
+    from paper_1409_8336_b200 import Pmc
+    assert torch.cuda.is_available(), "the gpu tests need a CUDA device (there is no CPU fallback)"
+    p = Pmc(0)
+    p.load_physics_tables(tables)
+    yield p
+    p.close()
+
+
+def _setup(pm, tables, mats, hu, vox, **opts):
+    """Same tables / materials / CT / options on both sides -> (pm, oracle)."""
+    pm.load_physics_tables(tables)
+    pm.set_hu_materials(mats)
+    pm.load_ct(torch.as_tensor(hu, device="cuda"), vox)
+    o = Oracle(tables, mats)
+    o.load_ct(hu, vox)
+    for k in ("straggling", "mcs", "elastic", "nonelastic"):
+        pm.set_option(k, float(opts.get(k, 1)))
+        o.set_option(k, float(opts.get(k, 1)))
+    return o
+
+
+# ------------------------------------------------------------------ S0 Philox: bit-exact
+def test_philox_bit_exact_against_kat_and_oracle(pm):
+    kat = [((0, 0, 0, 0), (0, 0), (0x6627e8d5, 0xe169c58d, 0xbc57ac4c, 0x9b00dbd8)),
+           ((0xffffffff,) * 4, (0xffffffff,) * 2, (0x408f276d, 0x41c83b0e, 0xa20bc7c6, 0x6d5451fd)),
+           ((0x243f6a88, 0x85a308d3, 0x13198a2e, 0x03707344), (0xa4093822, 0x299f31d0),
+            (0xd16cfe09, 0x94fdcceb, 0x5001e420, 0x24126ea1))]
+    rng = np.random.default_rng(5)
+    rnd = rng.integers(0, 2 ** 32, size=(1000, 6), dtype=np.uint64).astype(np.uint32)
+    rows = np.array([list(c) + list(k) for c, k, _ in kat], dtype=np.uint32)
+    out = pm.philox4x32_10(np.concatenate([rows, rnd]))
+    for i, (_, _, ref) in enumerate(kat):
+        assert tuple(int(x) for x in out[i]) == ref
+    for i in range(0, 1000, 7):
+        r = rnd[i]
+        assert [int(x) for x in out[3 + i]] == ob.philox4x32_10([int(x) for x in r[:4]], [int(x) for x in r[4:]])
+
+
+def test_philox_empty_input(pm):
+    assert pm.philox4x32_10(np.zeros((0, 6), dtype=np.uint32)).shape == (0, 4)
+
+
+# ------------------------------------------------------------------ S4 range tables: element by element
+@pytest.mark.parametrize("table", [0, 1, 2])
+def test_range_tables_match_oracle(pm, oracle_c1, table):
+    # fp32 evaluation of ln R splines: |d ln R| <~ 16 ulp(ln R ~ 5) ~ 1e-5 relative
+    e = np.exp(np.linspace(np.log(0.06), np.log(290.0), 4099)).astype(np.float32)          # ragged size
+    r_g = pm.range_of_energy(table, e).astype(np.float64)
+    r_o = np.array([oracle_c1.range_gcm2(table, float(x)) for x in e])
+    assert np.max(np.abs(r_g / r_o - 1)) < 3e-5
+    e_back = pm.energy_of_range(table, r_g.astype(np.float32)).astype(np.float64)
+    e_o = np.array([oracle_c1.energy_of_range(table, float(x)) for x in r_g])
+    assert np.max(np.abs(e_back / e_o - 1)) < 3e-5
+    assert np.max(np.abs(e_back / e - 1)) < 1e-4
+
+
+# ------------------------------------------------------------------ S5 straggling: cumulants and distribution
+@pytest.mark.parametrize("e_mev,rho_l", [(230.0, 0.1), (150.0, 0.2), (70.0, 0.2), (30.0, 0.25), (5.0, 0.02)])
+def test_straggling_distribution(pm, oracle_c1, e_mev, rho_l):
+    zoa, n = 0.555087, 400_000
+    mean = 0.5 * rho_l * 5.0
+    g = pm.straggle(e_mev, mean, rho_l, zoa, n, 11).astype(np.float64)
+    o = oracle_c1.straggle(e_mev, mean, rho_l, zoa, n, 12)
+    sd = o.std()
+    assert abs(g.mean() - o.mean()) < 5 * sd / np.sqrt(n) * np.sqrt(2) + 1e-6
+    assert abs(g.var() / o.var() - 1) < 0.03
+    m3g, m3o = np.mean((g - g.mean()) ** 3), np.mean((o - o.mean()) ** 3)
+    assert abs(m3g - m3o) < 0.15 * abs(m3o) + 0.02 * sd ** 3
+    # quantiles of the bulk agree to a small fraction of the width
+    q = np.array([0.01, 0.05, 0.25, 0.5, 0.75, 0.95, 0.99])
+    assert np.max(np.abs(np.quantile(g, q) - np.quantile(o, q))) < 0.03 * sd
+
+
+# ------------------------------------------------------------------ S10 nuclear elastic (Eq.3) and p-p
+@pytest.mark.parametrize("Z,A,t_mev", [(8, 16, 150.0), (20, 40, 100.0), (22, 48, 200.0), (1, 1, 150.0)])
+def test_elastic_matches_oracle(pm, oracle_c1, tables, Z, A, t_mev):
+    from scipy import stats
+    n = 200_000
+    g = pm.elastic(Z, A, t_mev, n, 41).astype(np.float64)
+    o = oracle_c1.elastic(Z, A, t_mev, n, 42)
+    assert stats.ks_2samp(g[:, 0], o[:, 0]).pvalue > 1e-3                  # |t| distribution
+    assert stats.ks_2samp(g[:, 3], o[:, 3]).pvalue > 1e-3                  # opening angle
+    assert np.allclose(g[:, 1] + g[:, 2], t_mev, atol=2e-4)               # fp32 energy conservation
+    m_t = tables["nuclear_mass"][Z, A]
+    assert np.allclose(g[:, 2], g[:, 0] * 1e6 / (2 * m_t), rtol=1e-5, atol=1e-6)
+    assert abs(g[:, 2].mean() - o[:, 2].mean()) < 5 * o[:, 2].std() * np.sqrt(2 / n)
+
+
+# ------------------------------------------------------------------ S3-S6 first steps: MCS / hinge / energy moments
+@pytest.mark.parametrize("e_mev,max_steps", [(150.0, 1), (70.0, 5), (230.0, 40)])
+def test_first_steps_moments_match_oracle(pm, tables, e_mev, max_steps):
+    hu, vox = inputs.phantom_c1()
+    o = _setup(pm, tables, inputs.make_materials_c1(), hu, vox, elastic=0, nonelastic=0)
+    spot = inputs.plan_single_spot((5.0, 5.0, 0.0), e_mev, 0.0)
+    n = 200_000
+    g = pm.first_steps(spot, n, 5, max_steps).astype(np.float64)
+    r = o.first_steps(spot, n, 6, max_steps)
+    se = np.sqrt(2.0 / n)
+    for col, name in [(0, "x"), (1, "y"), (3, "u"), (4, "v")]:
+        sg, so = g[:, col].std(), r[:, col].std()
+        assert abs(g[:, col].mean() - r[:, col].mean()) < 5 * so * se, name
+        assert abs(sg / so - 1) < 0.02, name                               # widths (Highland x 1.07, hinge)
+    # angle-displacement covariance of the hinge (Fermi-Eyges)
+    cg, co = np.mean((g[:, 0] - 5) * g[:, 3]), np.mean((r[:, 0] - 5) * r[:, 3])
+    assert abs(cg / co - 1) < 0.05
+    # depth, energy and path length after max_steps
+    for col, name in [(2, "z"), (6, "E"), (7, "path")]:
+        so = max(r[:, col].std(), 1e-9)
+        assert abs(g[:, col].mean() - r[:, col].mean()) < 5 * so * se + 2e-6 * abs(r[:, col].mean()), name
+    assert abs(g[:, 6].std() / r[:, 6].std() - 1) < 0.03                  # straggling width
+
+
+def test_first_steps_deterministic_limits(pm, tables):
+    # all fluctuations off: every history is the same CSDA track; compare element by element (fp32 vs fp64)
+    hu, vox = inputs.phantom_c1()
+    o = _setup(pm, tables, inputs.make_materials_c1(), hu, vox, straggling=0, mcs=0, elastic=0, nonelastic=0)
+    spot = inputs.plan_single_spot((5.0, 5.0, 0.0), 150.0, 0.3)
+    g = pm.first_steps(spot, 1000, 5, 30).astype(np.float64)
+    r = o.first_steps(spot, 1000, 5, 30)
+    assert np.allclose(g[:, 2], r[:, 2], atol=2e-5) and np.allclose(g[:, 7], r[:, 7], atol=2e-5)
+    assert np.allclose(g[:, 6], r[:, 6], rtol=2e-5)                       # 30 range-table updates in fp32
+    assert np.allclose(g[:, 3:6], [0, 0, 1], atol=1e-7)
+    # the draw order of the two sides is free: the spot profile is compared as a distribution
+    assert abs(g[:, 0].std() / 0.3 - 1) < 0.1 and abs(r[:, 0].std() / 0.3 - 1) < 0.1
+
+
+# ------------------------------------------------------------------ S12-S13 non-elastic collisions (config C2)
+C2_CASES = [(6, 12), (8, 16), (20, 40), (22, 48)]
+
+
+@pytest.mark.parametrize("Z,A", C2_CASES)
+@pytest.mark.parametrize("ie,e_mev", [(0, 100.0), (1, 200.0)])
+def test_nonelastic_c2_yields_spectra_angles(pm, oracle_c1, tables, Z, A, ie, e_mev):
+    n = 100_000                                                            # C2: 1e5 events per target and energy
+    seed = 2000 + 10 * C2_CASES.index((Z, A)) + ie
+    sg, og = pm.nonelastic(Z, A, e_mev, n, seed)
+    cg = pm.counters()
+    so, oo = oracle_c1.nonelastic(Z, A, e_mev, n, seed + 5)
+    # exact integers: charge and baryon number of every event (bit-exact bar)
+    assert cg["n_zab_violations"] == 0
+    zs = np.add.reduceat(sg["Z"].astype(np.int64), og[:-1]); as_ = np.add.reduceat(sg["A"].astype(np.int64), og[:-1])
+    assert np.all(zs == Z + 1) and np.all(as_ == A + 1)
+    assert og[0] == 0 and og[-1] == len(sg) and np.all(np.diff(og.astype(np.int64)) >= 2)
+    assert np.all(sg[og[1:] - 1]["origin"] == 2)
+    assert np.all(sg["ke"] >= 0) and np.allclose(np.linalg.norm(sg["dir"], axis=1), 1.0, atol=1e-4)
+    # energy bookkeeping per event from the public records: nothing is created
+    m = tables["nuclear_mass"]
+    e_out = np.add.reduceat(sg["ke"].astype(np.float64) + m[sg["Z"], sg["A"]], og[:-1])
+    left = e_mev + 938.27208816 + m[Z, A] - e_out
+    assert np.all(left > -2e-2) and abs(left.sum() - cg["e_gamma"]) < 2e-2 * n
+    # yields per species within 3 sigma (north_star), per origin
+    yg, yo = parity.species_yields(sg, og), parity.species_yields(so, oo)
+    err = np.sqrt(yg.var(axis=0) / n + yo.var(axis=0) / n)
+    z = (yg.mean(axis=0) - yo.mean(axis=0)) / np.maximum(err, 1e-12)
+    assert np.all(np.abs(z) < 3.0 + 0.5), (z, yg.mean(axis=0), yo.mean(axis=0))   # 48 comparisons: 3 sigma + look-elsewhere
+    assert np.all(np.abs(yg.mean(axis=0) - yo.mean(axis=0)) <= 0.01 * yo.mean(axis=0) + 3.5 * err)
+    # INC attempts per event (L75 restart rule)
+    assert abs(cg["n_inc_tries"] / n - oracle_c1.counters()["n_inc_tries"] / n) < 0.02
+    # spectra (5 MeV bins) and angles (20 bins), per species and origin
+    for (zz, aa) in [(0, 1), (1, 1), (2, 4)]:
+        for origin in (0, 1):
+            a = sg[(sg["Z"] == zz) & (sg["A"] == aa) & (sg["origin"] == origin)]
+            b = so[(so["Z"] == zz) & (so["A"] == aa) & (so["origin"] == origin)]
+            if len(b) < 2000:
+                continue
+            c2, nb = parity.chi2_hist(a["ke"], b["ke"], np.arange(0.0, e_mev + 10.0, 5.0))
+            assert c2 < 1 + 5 * np.sqrt(2.0 / max(nb, 1)), ("ke", zz, aa, origin, c2, nb)
+            c2, nb = parity.chi2_hist(a["dir"][:, 2], b["dir"][:, 2], np.linspace(-1, 1, 21))
+            assert c2 < 1 + 5 * np.sqrt(2.0 / max(nb, 1)), ("cos", zz, aa, origin, c2, nb)
+    # residual (Z, A) map
+    ra, rb = sg[og[1:] - 1], so[oo[1:] - 1]
+    ka, kb = ra["Z"].astype(np.int64) * 64 + ra["A"], rb["Z"].astype(np.int64) * 64 + rb["A"]
+    c2, nb = parity.chi2_hist(ka, kb, np.arange(-0.5, 64 * 24))
+    assert c2 < 1 + 5 * np.sqrt(2.0 / max(nb, 1)), ("residual map", c2, nb)
+
+
+def test_nonelastic_edge_cases(pm):
+    from paper_1409_8336_b200 import PmcError
+    sec, off = pm.nonelastic(8, 16, 200.0, 1, 3)                          # a single event
+    assert len(off) == 2 and off[1] == len(sec) >= 2
+    with pytest.raises(PmcError) as e:                                    # capacity too small: error, nothing silent
+        pm.nonelastic(8, 16, 200.0, 1000, 3, capacity=100)
+    assert e.value.code == -3
+    with pytest.raises(PmcError) as e:                                    # hydrogen has no cascade
+        pm.nonelastic(1, 1, 200.0, 10, 3)
+    assert e.value.code == -5
+    # reproducible: same seed -> identical records; event i depends only on (seed, i)
+    a, oa = pm.nonelastic(20, 40, 100.0, 5000, 9)
+    b, ob_ = pm.nonelastic(20, 40, 100.0, 2500, 9)
+    assert np.array_equal(oa[:2501], ob_) and a[:ob_[-1]].tobytes() == b.tobytes()
+
+
+# ------------------------------------------------------------------ full path: dose parity (configs C1, C3, C4)
+def _ledger_closes(c, rel=2e-4):
+    sinks = c["e_deposit"] + c["e_escape"] + c["e_neutron"] + c["e_gamma"] + c["e_q"] + c["e_air"]
+    return abs(sinks / c["e_source"] - 1) < rel
+
+
+def _dose_parity(pm, o, w_hu, vox, mats, spots, n, seed, axis=0, check_range=True, min_pass=0.99):
+    """north_star's dose tolerances between pmc_simulate and the oracle on the same inputs."""
+    dg, sg = pm.simulate(spots, n, seed)
+    cg = pm.counters()
+    dg, sg = dg.cpu().numpy().astype(np.float64), sg.cpu().numpy().astype(np.float64)
+    do, so = o.simulate(spots, n, seed)
+    co = o.counters()
+    assert np.all(np.isfinite(dg)) and np.all(dg >= 0) and np.all(sg >= 0)
+    # integrated dose (= deposited energy per history) within 0.5 %
+    rho = _density(w_hu, mats)
+    vol = vox[0] * vox[1] * vox[2]
+    eg, eo = (dg * rho).sum() * vol / parity.GY_PER_MEV_G, (do * rho).sum() * vol / parity.GY_PER_MEV_G
+    assert abs(eg / eo - 1) < 5e-3, (eg, eo)
+    assert abs(eg - cg["e_deposit"] / n) < 2e-4 * eg                       # tally == ledger (fp32 atomics)
+    assert _ledger_closes(cg), cg
+    # >= 99 % of voxels above 10 % of the maximum within 3 combined sigma
+    frac, zmean, zrms, nv = parity.zscore_pass(dg, sg, do, so)
+    assert nv > 20 and frac >= min_pass, (frac, zmean, zrms, nv)
+    assert abs(zmean) < 0.25 and zrms < 1.5, (zmean, zrms)
+    # R80 and distal fall-off within 0.2 mm
+    if check_range:
+        d_cm = vox[2 - axis]
+        r_g, f_g = parity.r80_and_falloff(parity.depth_dose(dg * rho, axis), d_cm)
+        r_o, f_o = parity.r80_and_falloff(parity.depth_dose(do * rho, axis), d_cm)
+        assert abs(r_g - r_o) < 0.02 and abs(f_g - f_o) < 0.02, (r_g, r_o, f_g, f_o)
+    # event rates per history: statistically equal (Poisson)
+    for k in ("n_elastic", "n_nonelastic", "n_secondary_protons"):
+        a, b = cg[k], co[k]
+        assert abs(a - b) < 5 * np.sqrt(a + b + 1) + 0.002 * b, (k, a, b)
+    assert abs(cg["n_steps"] / co["n_steps"] - 1) < 5e-3
+    return dg, sg, do, so, cg, co
+
+
+def _density(hu, mats):
+    rho = np.zeros(hu.shape)
+    h = hu.astype(np.float64)
+    for i, m in enumerate(mats):
+        lo = -np.inf if i == 0 else m["hu_lo"]
+        hi = np.inf if i == len(mats) - 1 else m["hu_hi"]
+        sel = (h >= lo) & (h < hi)
+        t = np.clip(h[sel], m["hu_lo"], m["hu_hi"])
+        rho[sel] = m["rho_lo"] + (m["rho_hi"] - m["rho_lo"]) * (t - m["hu_lo"]) / (m["hu_hi"] - m["hu_lo"])
+    return rho
+
+
+def test_c1_water_phantom_as_configured(pm, tables):
+    w = inputs.workload("c1")                                             # 1e4 histories, seed 1, full physics
+    o = _setup(pm, tables, w["materials"], w["hu"], w["vox"])
+    _dose_parity(pm, o, w["hu"], w["vox"], w["materials"], w["spots"], w["n_histories"], w["seed"], min_pass=0.985)
+
+
+def test_c1_water_phantom_high_statistics(pm, tables):
+    w = inputs.workload("c1")
+    o = _setup(pm, tables, w["materials"], w["hu"], w["vox"])
+    dg, sg, do, so, cg, co = _dose_parity(pm, o, w["hu"], w["vox"], w["materials"], w["spots"], 400_000, 11)
+    # lateral profile at the Bragg peak: MCS + nuclear halo
+    k = int(np.argmax(do.sum(axis=(1, 2))))
+    pg, po = dg[k - 5:k + 1].sum(axis=(0, 1)), do[k - 5:k + 1].sum(axis=(0, 1))
+    x = np.arange(len(po))
+    wg = np.sqrt((pg * (x - (pg * x).sum() / pg.sum()) ** 2).sum() / pg.sum())
+    wo = np.sqrt((po * (x - (po * x).sum() / po.sum()) ** 2).sum() / po.sum())
+    assert abs(wg / wo - 1) < 0.01
+
+
+@pytest.mark.parametrize("switches", [dict(straggling=0, mcs=0, elastic=0, nonelastic=0),
+                                      dict(elastic=0, nonelastic=0), dict(nonelastic=0), dict(elastic=0)])
+def test_c1_physics_switches(pm, tables, switches):
+    w = inputs.workload("c1")
+    o = _setup(pm, tables, w["materials"], w["hu"], w["vox"], **switches)
+    _dose_parity(pm, o, w["hu"], w["vox"], w["materials"], w["spots"], 100_000, 21, min_pass=0.985)
+
+
+@pytest.mark.parametrize("name,n", [("c3_70", 100_000), ("c3_150", 100_000), ("c3_230", 60_000)])
+def test_c3_slab_phantom(pm, tables, name, n):
+    w = inputs.workload(name)                                             # full 200x200x300 grid, 24-bin table
+    o = _setup(pm, tables, w["materials"], w["hu"], w["vox"])
+    # 230 MeV leaves the 30 cm slab: no Bragg peak inside, so no R80
+    dg, sg, do, so, cg, co = _dose_parity(pm, o, w["hu"], w["vox"], w["materials"], w["spots"], n, w["seed"],
+                                          check_range=(name != "c3_230"), min_pass=0.985)
+    if name == "c3_230":
+        assert abs(cg["e_escape"] / co["e_escape"] - 1) < 5e-3
+    # energy deposited per material class (water / bone / lung / Ti)
+    rho = _density(w["hu"], w["materials"])
+    for lo, hi in [(-5, 6), (1200, 1201), (-700, -699), (3071, 3072)]:
+        m = (w["hu"] >= lo) & (w["hu"] < hi)
+        a, b = (dg * rho)[m].sum(), (do * rho)[m].sum()
+        if b > 0:
+            assert abs(a / b - 1) < 1e-2, (lo, a, b)
+
+
+def test_c4_head_and_neck_full_size_against_oracle_subsample(pm, tables):
+    """C4 at BASELINE's full size (1e7 histories, the configuration bench.py times) on the GPU; the oracle runs a
+    4e5-history subsample of the same plan.  Doses are per primary, so projections and integrals compare directly."""
+    w = inputs.workload("c4")
+    o = _setup(pm, tables, w["materials"], w["hu"], w["vox"])
+    n_g, n_o = w["n_histories"], 400_000
+    dg, sg = pm.simulate(w["spots"], n_g, w["seed"])
+    cg = pm.counters()
+    dg, sg = dg.cpu().numpy().astype(np.float64), sg.cpu().numpy().astype(np.float64)
+    do, so = o.simulate(w["spots"], n_o, w["seed"] + 1)
+    co = o.counters()
+    assert _ledger_closes(cg) and cg["n_zab_violations"] == 0
+    rho = _density(w["hu"], w["materials"])
+    vol = np.prod(w["vox"])
+    eg, eo = (dg * rho).sum() * vol / parity.GY_PER_MEV_G, (do * rho).sum() * vol / parity.GY_PER_MEV_G
+    assert abs(eg / eo - 1) < 5e-3
+    assert abs(eg - cg["e_deposit"] / n_g) < 3e-4 * eg
+    for k in ("n_steps", "n_elastic", "n_nonelastic", "n_secondary_protons", "n_missed"):
+        a, b = cg[k] / n_g, co[k] / n_o
+        assert abs(a - b) < 5 * np.sqrt(b / n_o + a / n_g) + 5e-3 * b, (k, a, b)
+    # voxel z-scores: the GPU dose is nearly noise-free at 1e7, the oracle's sigma dominates
+    frac, zmean, zrms, nv = parity.zscore_pass(dg, sg, do, so)
+    assert nv > 1000 and frac >= 0.985 and abs(zmean) < 0.15 and zrms < 1.4, (frac, zmean, zrms, nv)
+    # the three 1-D projections of deposited energy
+    for ax in range(3):
+        pg, po = parity.depth_dose(dg * rho, ax), parity.depth_dose(do * rho, ax)
+        m = po > 0.05 * po.max()
+        assert np.max(np.abs(pg[m] / po[m] - 1)) < 0.03, ax
+    # sigma scales as 1/sqrt(N): median relative error in the high-dose region
+    hi = do > 0.5 * do.max()
+    ratio = np.median(sg[hi] / np.maximum(dg[hi], 1e-30)) / np.median(so[hi] / np.maximum(do[hi], 1e-30))
+    assert abs(ratio * np.sqrt(n_g / n_o) - 1) < 0.25
+
+
+# ------------------------------------------------------------------ edge and degenerate cases
+def test_simulate_edge_cases(pm, tables):
+    from paper_1409_8336_b200 import PmcError
+    w = inputs.workload("c1")
+    o = _setup(pm, tables, w["materials"], w["hu"], w["vox"])
+    # every history misses the grid: zero dose, energy all in the escape ledger
+    away = inputs.plan_single_spot((50.0, 50.0, -5.0), 150.0, 0.1)
+    d, s = pm.simulate(away, 1000, 1)
+    c = pm.counters()
+    assert float(d.abs().sum()) == 0.0 and float(s.abs().sum()) == 0.0
+    assert c["n_missed"] == 1000 and c["n_steps"] == 0 and abs(c["e_escape"] - 150.0 * 1000) < 1e-6
+    do, _ = o.simulate(away, 1000, 1)
+    assert do.sum() == 0.0 and o.counters()["n_missed"] == 1000
+    # fewer histories than batches; a single history
+    for n in (1, 7):
+        d, s = pm.simulate(w["spots"], n, 3)
+        c = pm.counters()
+        assert _ledger_closes(c) and abs(c["e_source"] - 150.0 * n) < 1e-6 and float(d.sum()) > 0
+    # air gap: source 20 cm upstream of the grid
+    up = inputs.plan_single_spot((5.0, 5.0, -20.0), 150.0, 0.3)
+    d, s = pm.simulate(up, 50_000, 5)
+    cg = pm.counters()
+    o.simulate(up, 50_000, 6)
+    co = o.counters()
+    assert cg["e_air"] > 0 and abs(cg["e_air"] / co["e_air"] - 1) < 0.02 and _ledger_closes(cg)
+    # oblique beam entering through a side face
+    ob_ = inputs.plan_single_spot((-3.0, 5.0, 6.0), 100.0, 0.3, direction=(0.8, 0.0, 0.6))
+    _dose_parity(pm, o, w["hu"], w["vox"], w["materials"], ob_, 60_000, 8, check_range=False, min_pass=0.98)
+    # zero-weight and bad inputs
+    bad = w["spots"].copy(); bad[0, 12] = 0.0
+    with pytest.raises(PmcError):
+        pm.simulate(bad, 10, 1)
+    bad = w["spots"].copy(); bad[0, 3:6] = 0.0
+    with pytest.raises(PmcError):
+        pm.simulate(bad, 10, 1)
+
+
+def test_call_order_and_argument_errors(tables):
+    from paper_1409_8336_b200 import Pmc, PmcError
+    p = Pmc(0)
+    w = inputs.workload("c1")
+    with pytest.raises(PmcError) as e:
+        p.set_hu_materials(w["materials"])
+    assert e.value.code == -2                                             # PMC_E_STATE
+    p.load_physics_tables(tables)
+    p.shape = w["hu"].shape
+    with pytest.raises(PmcError) as e:
+        p.simulate(w["spots"], 10, 1)
+    assert e.value.code == -2
+    p.set_hu_materials(w["materials"])
+    with pytest.raises(PmcError):
+        p.load_ct(w["hu"], (0.2, -0.2, 0.2))
+    with pytest.raises(PmcError):
+        p.set_option("no_such_option", 1.0)
+    mats = [dict(m) for m in w["materials"]]
+    mats[1] = dict(mats[1], hu_lo=mats[1]["hu_lo"] + 1)
+    with pytest.raises(PmcError):
+        p.set_hu_materials(mats)
+    p.close()
+
+
+def test_streams_are_schedule_independent(pm, tables):
+    """Philox streams are keyed per history (north_star): sub-group size, history offset and the stream the context
+    runs on change the schedule, not the physics.  Integer counters are identical; float tallies agree up to the
+    order of the atomic adds."""
+    w = inputs.workload("c1")
+    _setup(pm, tables, w["materials"], w["hu"], w["vox"])
+    n = 30_000
+    d0, _ = pm.simulate(w["spots"], n, 77); c0 = pm.counters()
+    pm.set_option("chunk_histories", 1000.0)
+    d1, _ = pm.simulate(w["spots"], n, 77); c1 = pm.counters()
+    pm.set_option("chunk_histories", float(1 << 21))
+    pm.set_option("dose_aggregate", 0.0)
+    d2, _ = pm.simulate(w["spots"], n, 77); c2 = pm.counters()
+    pm.set_option("dose_aggregate", 1.0)
+    for c in (c1, c2):
+        for k in ("n_steps", "n_elastic", "n_nonelastic", "n_secondary_protons", "n_inc_tries"):
+            assert c[k] == c0[k], k
+    for d in (d1, d2):
+        assert torch.allclose(d, d0, rtol=2e-4, atol=1e-16)
+    # two halves with history offsets = the whole (sharding)
+    pm.set_option("n_batches", 2.0)
+    dw, _ = pm.simulate(w["spots"], n, 78); cw = pm.counters()
+    pm.set_option("n_batches", 10.0)
+    da, _ = pm.simulate(w["spots"], n // 2, 78); ca = pm.counters()
+    pm.set_option("history_offset", float(n // 2))
+    db, _ = pm.simulate(w["spots"], n // 2, 78); cb = pm.counters()
+    pm.set_option("history_offset", 0.0)
+    assert ca["n_steps"] + cb["n_steps"] == cw["n_steps"] and ca["n_nonelastic"] + cb["n_nonelastic"] == cw["n_nonelastic"]
+    assert torch.allclose(0.5 * (da + db), dw, rtol=2e-4, atol=1e-16)
