@@ -575,7 +575,7 @@ bool transport_step(opmc_ctx *c, Particle &p, Rng &g, double *tally, Ledger &led
   double dx = lam; int lim = 2;
   if (dface < dx) { dx = dface; lim = 1; }
   if (R < dx) { dx = R; lim = 3; }
-  if (smax < dx) { dx = smax; lim = 0; }
+  if (smax < dx * (1 - 1e-6)) { dx = smax; lim = 0; }   // s_max binds only when shorter by more than rounding (R3.2)
   // 3-5. random hinge (L69 ref [19]): first leg tau, deflect, second leg
   double e0 = p.E, tau = 0; V3 dnew = p.d;
   if (c->opt_mcs && dx > 0) {

@@ -246,7 +246,7 @@ __global__ void __launch_bounds__(256, 2) transport_kernel(Tables T, Grid G, Run
       float dx = lam; int lim = 2;
       if (dface < dx) { dx = dface; lim = 1; }
       if (R < dx) { dx = R; lim = 3; }
-      if (smax < dx) { dx = smax; lim = 0; }
+      if (smax < dx * (1.0f - 1e-6f)) { dx = smax; lim = 0; }   // ties go to the face / event (Reading R3.2)
       // ---- 3-5. random hinge (PAPER.md:L69 ref [19]): first leg tau, deflect, second leg
       float tau = 0.f; V3 dnew = p.d;
       if (T.opt_mcs && dx > 0.f) {

@@ -34,11 +34,15 @@ def r80_and_falloff(dd, d_cm):
     return r80, r20 - r80
 
 
-def zscore_pass(d_a, s_a, d_b, s_b, frac_of_max=0.1, nsig=3.0):
-    """Fraction of voxels with d_b > frac*max within nsig combined sigma; also mean and rms z."""
+def zscore_pass(d_a, s_a, d_b, s_b, frac_of_max=0.1, nsig=3.0, region=None):
+    """Fraction of voxels with d_b > frac*max within nsig combined sigma; also mean and rms z.  `region` (bool grid)
+    restricts both the maximum and the voxels compared (e.g. to tissue, leaving out air voxels whose dose-to-medium
+    is a 1000x spike whenever a single proton stops in them)."""
     d_a = np.asarray(d_a, dtype=np.float64); d_b = np.asarray(d_b, dtype=np.float64)
     s = np.sqrt(np.asarray(s_a, dtype=np.float64) ** 2 + np.asarray(s_b, dtype=np.float64) ** 2)
-    m = (d_b > frac_of_max * d_b.max()) & (s > 0)
+    if region is None:
+        region = np.ones(d_b.shape, dtype=bool)
+    m = region & (d_b > frac_of_max * d_b[region].max()) & (s > 0)
     z = (d_a[m] - d_b[m]) / s[m]
     return float(np.mean(np.abs(z) <= nsig)), float(z.mean()), float(z.std()), int(m.sum())
 

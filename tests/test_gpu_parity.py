@@ -112,7 +112,9 @@ def test_elastic_matches_oracle(pm, oracle_c1, tables, Z, A, t_mev):
 def test_first_steps_moments_match_oracle(pm, tables, e_mev, max_steps):
     hu, vox = inputs.phantom_c1()
     o = _setup(pm, tables, inputs.make_materials_c1(), hu, vox, elastic=0, nonelastic=0)
-    spot = inputs.plan_single_spot((5.0, 5.0, 0.0), e_mev, 0.0)
+    # the pencil starts at a voxel centre: on a voxel face (x = 5.0) the first deflection decides the voxel and the
+    # one-step x distribution is one-sided, with the side set by how 5.0/0.2 rounds in fp32 vs fp64
+    spot = inputs.plan_single_spot((5.1, 5.1, 0.0), e_mev, 0.0)
     n = 200_000
     g = pm.first_steps(spot, n, 5, max_steps).astype(np.float64)
     r = o.first_steps(spot, n, 6, max_steps)
@@ -122,7 +124,7 @@ def test_first_steps_moments_match_oracle(pm, tables, e_mev, max_steps):
         assert abs(g[:, col].mean() - r[:, col].mean()) < 5 * so * se, name
         assert abs(sg / so - 1) < 0.02, name                               # widths (Highland x 1.07, hinge)
     # angle-displacement covariance of the hinge (Fermi-Eyges)
-    cg, co = np.mean((g[:, 0] - 5) * g[:, 3]), np.mean((r[:, 0] - 5) * r[:, 3])
+    cg, co = np.mean((g[:, 0] - 5.1) * g[:, 3]), np.mean((r[:, 0] - 5.1) * r[:, 3])
     assert abs(cg / co - 1) < 0.05
     # depth, energy and path length after max_steps
     for col, name in [(2, "z"), (6, "E"), (7, "path")]:
@@ -176,7 +178,9 @@ def test_nonelastic_c2_yields_spectra_angles(pm, oracle_c1, tables, Z, A, ie, e_
     assert np.all(np.abs(z) < 3.0 + 0.5), (z, yg.mean(axis=0), yo.mean(axis=0))   # 48 comparisons: 3 sigma + look-elsewhere
     assert np.all(np.abs(yg.mean(axis=0) - yo.mean(axis=0)) <= 0.01 * yo.mean(axis=0) + 3.5 * err)
     # INC attempts per event (L75 restart rule)
-    assert abs(cg["n_inc_tries"] / n - oracle_c1.counters()["n_inc_tries"] / n) < 0.02
+    # (the number of tries is geometric: variance m(m-1) per event; 5 sigma of the difference of the two means)
+    mt = oracle_c1.counters()["n_inc_tries"] / n
+    assert abs(cg["n_inc_tries"] / n - mt) < 5 * np.sqrt(2 * mt * max(mt - 1, 0.01) / n)
     # spectra (5 MeV bins) and angles (20 bins), per species and origin
     for (zz, aa) in [(0, 1), (1, 1), (2, 4)]:
         for origin in (0, 1):
@@ -328,7 +332,9 @@ def test_c4_head_and_neck_full_size_against_oracle_subsample(pm, tables):
         a, b = cg[k] / n_g, co[k] / n_o
         assert abs(a - b) < 5 * np.sqrt(b / n_o + a / n_g) + 5e-3 * b, (k, a, b)
     # voxel z-scores: the GPU dose is nearly noise-free at 1e7, the oracle's sigma dominates
-    frac, zmean, zrms, nv = parity.zscore_pass(dg, sg, do, so)
+    # (tissue voxels only: in the air bin, rho = 0.0012, one stopping proton is a 1000x dose spike that would set the
+    # "maximum" of a 4e5-history map)
+    frac, zmean, zrms, nv = parity.zscore_pass(dg, sg, do, so, region=w["hu"] >= -950)
     assert nv > 1000 and frac >= 0.985 and abs(zmean) < 0.15 and zrms < 1.4, (frac, zmean, zrms, nv)
     # the three 1-D projections of deposited energy
     for ax in range(3):
