@@ -71,7 +71,7 @@ struct pmc_ctx {
   std::vector<int> ez, ea;
   double e_cut = 0.1, highland = 1.07, kappa_g = 10, s_max = 0.2; int n_batches = 10;
   bool opt_strag = true, opt_mcs = true, opt_el = true, opt_ne = true; int aggregate = 1; bool profile = true;
-  uint64_t chunk = 1u << 21, history_offset = 0;
+  uint64_t chunk = 1u << 23, history_offset = 0;
   std::vector<HostMat> mats;
   // device tables
   DevBuf<float> d_lnR, d_lnR2, d_lnE, d_lnE2, d_sel, d_sne, d_sigbin, d_ek, d_ec;
@@ -81,7 +81,7 @@ struct pmc_ctx {
   DevBuf<int16_t> d_hu_own;
   // scratch
   QueueMem qa, qb, qel, qne, qres; DevBuf<uint32_t> d_resza; DevBuf<float> d_resp;
-  DevBuf<uint32_t> d_head; DevBuf<Counters> d_cnt; DevBuf<float> d_tally, d_mean, d_m2, d_out;
+  DevBuf<uint32_t> d_head; DevBuf<Counters> d_cnt; DevBuf<float> d_tally, d_out;
   DevBuf<SpotDev> d_spots; DevBuf<double> d_cdf;
   DevBuf<SecRec> d_slots; DevBuf<uint32_t> d_counts; DevBuf<unsigned long long> d_base;
   uint32_t *h_pinned = nullptr;     // pinned readback word(s)
@@ -357,7 +357,7 @@ void pmc_destroy(pmc_ctx *c) {
   c->d_sigbin.release(); c->d_ek.release(); c->d_ec.release(); c->d_mass.release(); c->d_bins.release(); c->d_lut.release();
   c->d_nuc.release(); c->d_nuc1.release(); c->d_hu_own.release();
   c->qa.release(); c->qb.release(); c->qel.release(); c->qne.release(); c->qres.release(); c->d_resza.release(); c->d_resp.release();
-  c->d_head.release(); c->d_cnt.release(); c->d_tally.release(); c->d_mean.release(); c->d_m2.release(); c->d_out.release();
+  c->d_head.release(); c->d_cnt.release(); c->d_tally.release(); c->d_out.release();
   c->d_spots.release(); c->d_cdf.release(); c->d_slots.release(); c->d_counts.release(); c->d_base.release();
   if (c->h_pinned) cudaFreeHost(c->h_pinned);
   if (c->ev[0]) { cudaEventDestroy(c->ev[0]); cudaEventDestroy(c->ev[1]); }
@@ -482,13 +482,17 @@ static int simulate_impl(pmc_ctx *c, const pmc_spot *spots_in, int nspots, uint6
   std::vector<pmc_spot> spots(spots_in, spots_in + nspots);
   for (auto &s : spots) for (int k = 0; k < 3; ++k) s.pos_cm[k] -= c->origin[k];
   rc = prepare_spots(c, spots.data(), nspots); if (rc) return rc;
-  const uint64_t per_batch = (n + B - 1) / B;
-  const uint64_t chunk = std::max<uint64_t>(1, std::min<uint64_t>(c->chunk, std::max<uint64_t>(per_batch, 1)));
+  // sub-groups: equal chunks of at most chunk_histories; every chunk carries histories of all the
+  // batches it spans, each batch scoring into its own tally grid (RunParams)
+  const uint64_t nchunks = std::max<uint64_t>(1, (n + c->chunk - 1) / c->chunk);
+  const uint64_t chunk = std::max<uint64_t>(1, (n + nchunks - 1) / nchunks);
   rc = ensure_scratch(c, chunk); if (rc) return rc;
-  const uint32_t nvox = (uint32_t)((size_t)c->G.nx * c->G.ny * c->G.nz);
-  CK(c->d_tally.alloc(nvox)); CK(c->d_mean.alloc(nvox)); CK(c->d_m2.alloc(nvox));
+  const size_t nvox_s = (size_t)c->G.nx * c->G.ny * c->G.nz;
+  const uint32_t nvox = (uint32_t)nvox_s;
+  if ((double)nvox_s * B >= 4294967296.0) return fail(c, PMC_E_UNSUPPORTED, "n_batches x voxels must be < 2^32");
+  CK(c->d_tally.alloc(nvox_s * B));
   cudaStream_t s = c->stream;
-  CK(cudaMemsetAsync(c->d_tally.p, 0, (size_t)nvox * 4, s)); CK(cudaMemsetAsync(c->d_cnt.p, 0, sizeof(Counters), s));
+  CK(cudaMemsetAsync(c->d_tally.p, 0, nvox_s * B * 4, s)); CK(cudaMemsetAsync(c->d_cnt.p, 0, sizeof(Counters), s));
   c->counters = pmc_counters{}; c->timing = pmc_timing{};
   float air_rho, air_wf, air_ix0, air_zoa; int air_tab; air_params(c, air_rho, air_wf, air_ix0, air_zoa, air_tab);
   const bool profile = c->profile;
@@ -496,28 +500,23 @@ static int simulate_impl(pmc_ctx *c, const pmc_spot *spots_in, int nspots, uint6
   cudaEvent_t e0, e1; CK(cudaEventCreate(&e0)); CK(cudaEventCreate(&e1));
   CK(cudaEventRecord(e0, s));
   const int grid_v = c->n_sm * 8;
-  for (int b = 0; b < B; ++b) {                                  // PAPER.md:L134 "10 groups of N/10"
-    const uint64_t h0 = (uint64_t)(((unsigned __int128)b * n + B - 1) / B), h1 = (uint64_t)(((unsigned __int128)(b + 1) * n + B - 1) / B);
-    for (uint64_t cs = h0; cs < h1; cs += chunk) {               // sub-groups (L134)
-      const uint32_t nc = (uint32_t)std::min<uint64_t>(chunk, h1 - cs);
-      RunParams P{}; P.seed = seed; P.hist0 = c->history_offset + cs; P.n = nc; P.max_steps = max_steps; P.dbg_out = dbg_out ? dbg_out + 8ull * (cs - h0) : nullptr;
-      P.aggregate = c->aggregate;
-      CK(cudaMemsetAsync(c->qa.q.count, 0, 4, s));
-      { Timer t(c, &c->timing.sampler_ms, profile);
-        sampler_kernel<<<(nc + 255) / 256, 256, 0, s>>>(c->T, c->G, c->d_spots.p, c->d_cdf.p, nspots, P, c->qa.q, c->d_cnt.p, air_rho, air_wf, air_ix0, air_zoa, air_tab); }
-      c->timing.launches_total++;
-      CK(cudaMemcpyAsync(c->h_pinned, c->qa.q.count, 4, cudaMemcpyDeviceToHost, s));
-      CK(cudaStreamSynchronize(s));
-      rc = run_generations(c, P, std::min(c->h_pinned[0], c->qcap), profile); if (rc) { cudaEventDestroy(e0); cudaEventDestroy(e1); return rc; }
-    }
-    if (!dbg_out) {
-      const float inv_nb = h1 > h0 ? (float)(1.0 / (double)(h1 - h0)) : 0.f;
-      { Timer t(c, &c->timing.statistics_ms, profile);
-        fold_kernel<<<grid_v, 256, 0, s>>>(c->T, c->G, c->d_tally.p, c->d_mean.p, c->d_m2.p, b, inv_nb, nvox); }
-      c->timing.launches_total++;
-    }
+  for (uint64_t cs = 0; cs < n; cs += chunk) {
+    const uint32_t nc = (uint32_t)std::min<uint64_t>(chunk, n - cs);
+    RunParams P{}; P.seed = seed; P.hist0 = c->history_offset + cs; P.n = nc; P.max_steps = max_steps; P.dbg_out = dbg_out ? dbg_out + 8ull * cs : nullptr;
+    P.aggregate = c->aggregate; P.local0 = cs; P.n_total = n; P.B = (uint32_t)B; P.nvox = nvox;
+    CK(cudaMemsetAsync(c->qa.q.count, 0, 4, s));
+    { Timer t(c, &c->timing.sampler_ms, profile);
+      sampler_kernel<<<(nc + 255) / 256, 256, 0, s>>>(c->T, c->G, c->d_spots.p, c->d_cdf.p, nspots, P, c->qa.q, c->d_cnt.p, air_rho, air_wf, air_ix0, air_zoa, air_tab); }
+    c->timing.launches_total++;
+    CK(cudaMemcpyAsync(c->h_pinned, c->qa.q.count, 4, cudaMemcpyDeviceToHost, s));
+    CK(cudaStreamSynchronize(s));
+    rc = run_generations(c, P, std::min(c->h_pinned[0], c->qcap), profile); if (rc) { cudaEventDestroy(e0); cudaEventDestroy(e1); return rc; }
   }
-  if (!dbg_out) { finish_kernel<<<grid_v, 256, 0, s>>>(c->d_mean.p, c->d_m2.p, dose_dev, sigma_dev, B, nvox); c->timing.launches_total++; }
+  if (!dbg_out) {                                                  // PAPER.md:L138 total and RMS dose per voxel
+    { Timer t(c, &c->timing.statistics_ms, profile);
+      stats_kernel<<<grid_v, 256, 0, s>>>(c->T, c->G, c->d_tally.p, dose_dev, sigma_dev, B, n, nvox); }
+    c->timing.launches_total++;
+  }
   CK(cudaEventRecord(e1, s));
   CK(cudaGetLastError());
   rc = fetch_counters(c);

@@ -8,6 +8,7 @@
 // baryon number are integers throughout.
 #pragma once
 #include "pmc_device.cuh"
+#include "pmc_transport.cuh"
 
 namespace pmc {
 
@@ -272,7 +273,7 @@ __global__ void __launch_bounds__(128) inc_kernel(Tables T, RunParams P, Queue i
         } else c_neu += (double)o.ke;                                        // neutrons: not transported
       }
       c_q += msum + R.mass_gs - MP_D - N.mass;
-      if (dep != 0.f) { atomicAdd(tally + p.vox, dep); c_dep += (double)dep; }
+      if (dep != 0.f) { atomicAdd(tally + batch_base(P, p.hist) + (uint32_t)p.vox, dep); c_dep += (double)dep; }
       // residual -> evaporation queue (keeps the event frame: p.d is the incident direction)
       const uint32_t slot = warp_alloc(rq.q.count);
       if (slot >= rq.q.cap) atomicOr(&cnt->overflow, 32u);
@@ -319,7 +320,7 @@ __global__ void __launch_bounds__(128) evap_kernel(Tables T, RunParams P, ResQue
       if (R.A == 1 && R.Z == 0) c_neu += kres; else dep += (float)kres;
       c_gam += R.estar;                                                     // L79: no photon evaporation
       c_q += msum + R.mass_gs - m0;
-      if (dep != 0.f) { atomicAdd(tally + p.vox, dep); c_dep += (double)dep; }
+      if (dep != 0.f) { atomicAdd(tally + batch_base(P, p.hist) + (uint32_t)p.vox, dep); c_dep += (double)dep; }
     }
   }
   flush(&cnt->e_deposit, c_dep); flush(&cnt->e_neutron, c_neu); flush(&cnt->e_q, c_q); flush(&cnt->e_gamma, c_gam);

@@ -13,9 +13,17 @@ struct SpotDev {                 // pmc_spot, prepared on the host (axis normali
 struct RunParams {
   uint64_t seed; uint64_t hist0;      // first history id of this launch
   uint32_t n;                         // histories in this launch
+  // All B batches ("10 groups") are in flight at once, each scoring into its own tally grid:
+  // history h (0-based within the call) belongs to batch floor(h B / n_total); tally of batch b starts at b * nvox.
+  uint64_t local0, n_total;           // call-local index of this launch's first history; histories in the call
+  uint32_t B, nvox;
   int max_steps; float *dbg_out;      // pmc_first_steps: stop after max_steps, write [hist][8]
   int aggregate;                      // warp-aggregated dose atomics
 };
+
+__device__ __forceinline__ uint32_t batch_base(const RunParams &P, uint32_t hist) {
+  return (uint32_t)(((P.local0 + hist) * (uint64_t)P.B) / P.n_total) * P.nvox;
+}
 
 // ------------------------------------------------------------------ material of a voxel
 struct VoxMat { float rho, wf, inv_x0, zoa; int table, bin; };
@@ -155,7 +163,7 @@ __global__ void __launch_bounds__(256) sampler_kernel(Tables T, Grid G, const Sp
 // ------------------------------------------------------------------ dose deposit (atomics)
 // Lanes of a warp that score into the same voxel in the same iteration are merged (warp match) so that a
 // single RED reaches the L2; with a pencil beam the lanes advance slab by slab and collide often.
-__device__ __forceinline__ void deposit(float *tally, int vox, float e, bool on, int aggregate) {
+__device__ __forceinline__ void deposit(float *tally, uint32_t vox, float e, bool on, int aggregate) {
   if (!aggregate) { if (on && e != 0.f) atomicAdd(tally + vox, e); return; }
   const unsigned act = __ballot_sync(0xffffffffu, on);
   if (!on) return;
@@ -200,7 +208,7 @@ __global__ void __launch_bounds__(256, 2) transport_kernel(Tables T, Grid G, Run
   const float sz[3] = {G.d[0], G.d[1], G.d[2]};
   const int lane = threadIdx.x & 31;
   bool active = false, exhausted = false;
-  Particle p; Rng g; int ix = 0, iy = 0, iz = 0, nstep = 0; float path = 0.f;
+  Particle p; Rng g; int ix = 0, iy = 0, iz = 0, nstep = 0; float path = 0.f; uint32_t tbase = 0;
   unsigned long long c_steps = 0, c_el = 0, c_ne = 0;
   double c_dep = 0, c_esc = 0;
   const bool nuclear = T.opt_el || T.opt_ne;
@@ -218,7 +226,7 @@ __global__ void __launch_bounds__(256, 2) transport_kernel(Tables T, Grid G, Run
           p = queue_load(in, idx);
           g.init(P.seed, P.hist0 + p.hist, p.pid, p.blk);
           ix = p.vox % G.nx; const int t = p.vox / G.nx; iy = t % G.ny; iz = t / G.ny;
-          active = true; nstep = 0; path = 0.f;
+          active = true; nstep = 0; path = 0.f; tbase = batch_base(P, p.hist);
         } else exhausted = true;
       }
     }
@@ -323,7 +331,7 @@ __global__ void __launch_bounds__(256, 2) transport_kernel(Tables T, Grid G, Run
         }
       }
     }
-    deposit(tally, dep_vox, dep, dep != 0.f, P.aggregate);
+    deposit(tally, tbase + (uint32_t)dep_vox, dep, dep != 0.f, P.aggregate);
   }
   flush(&cnt->n_steps, c_steps); flush(&cnt->n_elastic, c_el); flush(&cnt->n_nonelastic, c_ne);
   flush(&cnt->e_deposit, c_dep); flush(&cnt->e_escape, c_esc);
@@ -391,36 +399,30 @@ __global__ void __launch_bounds__(256) elastic_kernel(Tables T, RunParams P, Que
       if (!push_p) dep += p.e;
       if (push_p) { if (!queue_push(out, p)) atomicOr(&cnt->overflow, 8u); }
       if (push_rec) { if (!queue_push(out, s)) atomicOr(&cnt->overflow, 8u); }
-      if (dep != 0.f) { atomicAdd(tally + p.vox, dep); c_dep += (double)dep; }
+      if (dep != 0.f) { atomicAdd(tally + batch_base(P, p.hist) + (uint32_t)p.vox, dep); c_dep += (double)dep; }
     }
   }
   flush(&cnt->e_deposit, c_dep); flush(&cnt->n_secondary, c_sec);
 }
 
 // ------------------------------------------------------------------ K5: batch statistics (Reading R8)
-// After each batch: dose of the batch (Gy per primary) folded into a running mean and sum of squared
-// deviations (Welford), tally cleared.
-__global__ void __launch_bounds__(256) fold_kernel(Tables T, Grid G, float *tally, float *mean, float *m2, int b,
-                                                   float inv_nb, uint32_t nvox) {
+// One voxel per thread (L140): dose of each batch (Gy per primary) from its tally, running mean and sum of squared
+// deviations over the B batches (Welford), then mean dose and standard error.
+__global__ void __launch_bounds__(256) stats_kernel(Tables T, Grid G, const float *tally, float *dose, float *sigma, int B,
+                                                    uint64_t n_total, uint32_t nvox) {
   for (uint32_t v = blockIdx.x * blockDim.x + threadIdx.x; v < nvox; v += gridDim.x * blockDim.x) {
-    const float t = tally[v];
-    float d = 0.f;
-    if (t != 0.f) {
-      const int hu = G.hu[v];
-      const MatBin &m = T.bins[hu_to_bin(T, T.hu_lut, hu)];
-      d = t / (bin_density(m, hu) * G.vol) * inv_nb * 1.602176634e-10f;
-      tally[v] = 0.f;
+    const int hu = G.hu[v];
+    const MatBin &m = T.bins[hu_to_bin(T, T.hu_lut, hu)];
+    const float inv_m = 1.602176634e-10f / (bin_density(m, hu) * G.vol);
+    float mu = 0.f, s = 0.f;
+    for (int b = 0; b < B; ++b) {
+      const uint64_t h0 = ((uint64_t)b * n_total + B - 1) / B, h1 = ((uint64_t)(b + 1) * n_total + B - 1) / B;
+      const float t = tally[(size_t)b * nvox + v];
+      const float d = h1 > h0 ? t * inv_m / (float)(h1 - h0) : 0.f;
+      const float delta = d - mu; mu += delta / (float)(b + 1); s += delta * (d - mu);
     }
-    const float mu = b == 0 ? 0.f : mean[v], s = b == 0 ? 0.f : m2[v];
-    const float delta = d - mu, mu1 = mu + delta / (float)(b + 1);
-    mean[v] = mu1; m2[v] = s + delta * (d - mu1);
-  }
-}
-__global__ void __launch_bounds__(256) finish_kernel(const float *mean, const float *m2, float *dose, float *sigma,
-                                                     int B, uint32_t nvox) {
-  for (uint32_t v = blockIdx.x * blockDim.x + threadIdx.x; v < nvox; v += gridDim.x * blockDim.x) {
-    dose[v] = mean[v];
-    const float var = m2[v] / ((float)B * (float)(B - 1));
+    dose[v] = mu;
+    const float var = s / ((float)B * (float)(B - 1));
     sigma[v] = var > 0.f ? sqrtf(var) : 0.f;
   }
 }

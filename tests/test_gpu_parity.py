@@ -116,8 +116,14 @@ def test_first_steps_moments_match_oracle(pm, tables, e_mev, max_steps):
     # one-step x distribution is one-sided, with the side set by how 5.0/0.2 rounds in fp32 vs fp64
     spot = inputs.plan_single_spot((5.1, 5.1, 0.0), e_mev, 0.0)
     n = 200_000
-    g = pm.first_steps(spot, n, 5, max_steps).astype(np.float64)
-    r = o.first_steps(spot, n, 6, max_steps)
+    # s_max incommensurate with the 2 mm voxel: with the default (0.2 cm = the voxel) every deflected step is a
+    # near-tie between s_max and the face, and the depth after k steps depends on fp32-vs-fp64 rounding
+    pm.set_option("s_max_wet_cm", 0.07); o.set_option("s_max_wet_cm", 0.07)
+    try:
+        g = pm.first_steps(spot, n, 5, max_steps).astype(np.float64)
+        r = o.first_steps(spot, n, 6, max_steps)
+    finally:
+        pm.set_option("s_max_wet_cm", 0.2)
     se = np.sqrt(2.0 / n)
     for col, name in [(0, "x"), (1, "y"), (3, "u"), (4, "v")]:
         sg, so = g[:, col].std(), r[:, col].std()
@@ -275,7 +281,13 @@ def test_c1_water_phantom_as_configured(pm, tables):
 def test_c1_water_phantom_high_statistics(pm, tables):
     w = inputs.workload("c1")
     o = _setup(pm, tables, w["materials"], w["hu"], w["vox"])
-    dg, sg, do, so, cg, co = _dose_parity(pm, o, w["hu"], w["vox"], w["materials"], w["spots"], 400_000, 11)
+    # 40 batches: with 10-batch sigmas on both sides the z statistic is t-like and only 99.25 % of voxels fall within
+    # 3 under perfect parity; B is a run-time option on both sides
+    pm.set_option("n_batches", 40.0); o.set_option("n_batches", 40.0)
+    try:
+        dg, sg, do, so, cg, co = _dose_parity(pm, o, w["hu"], w["vox"], w["materials"], w["spots"], 400_000, 11)
+    finally:
+        pm.set_option("n_batches", 10.0)
     # lateral profile at the Bragg peak: MCS + nuclear halo
     k = int(np.argmax(do.sum(axis=(1, 2))))
     pg, po = dg[k - 5:k + 1].sum(axis=(0, 1)), do[k - 5:k + 1].sum(axis=(0, 1))
@@ -340,9 +352,12 @@ def test_c4_head_and_neck_full_size_against_oracle_subsample(pm, tables):
     for ax in range(3):
         pg, po = parity.depth_dose(dg * rho, ax), parity.depth_dose(do * rho, ax)
         m = po > 0.05 * po.max()
-        assert np.max(np.abs(pg[m] / po[m] - 1)) < 0.03, ax
+        # noise of the 4e5-history oracle projection scales as 1/sqrt(dose in the slab): ~1 % at the peak slab
+        tol = 0.01 + 0.012 * np.sqrt(po.max() / po[m])
+        assert np.all(np.abs(pg[m] / po[m] - 1) < tol), (ax, np.max(np.abs(pg[m] / po[m] - 1) / tol))
     # sigma scales as 1/sqrt(N): median relative error in the high-dose region
-    hi = do > 0.5 * do.max()
+    tissue = w["hu"] >= -950
+    hi = tissue & (do > 0.5 * do[tissue].max())
     ratio = np.median(sg[hi] / np.maximum(dg[hi], 1e-30)) / np.median(so[hi] / np.maximum(do[hi], 1e-30))
     assert abs(ratio * np.sqrt(n_g / n_o) - 1) < 0.25
 
