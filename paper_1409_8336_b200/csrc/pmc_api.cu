@@ -83,7 +83,7 @@ struct pmc_ctx {
   QueueMem qa, qb, qel, qne, qres; DevBuf<uint32_t> d_resza; DevBuf<float> d_resp;
   DevBuf<uint32_t> d_head; DevBuf<Counters> d_cnt; DevBuf<float> d_tally, d_out;
   DevBuf<SpotDev> d_spots; DevBuf<double> d_cdf;
-  DevBuf<SecRec> d_slots; DevBuf<uint32_t> d_counts; DevBuf<unsigned long long> d_base;
+  DevBuf<SecRec> d_slots; DevBuf<uint32_t> d_counts; DevBuf<unsigned long long> d_base; DevBuf<ResRec> d_res;
   uint32_t *h_pinned = nullptr;     // pinned readback word(s)
   uint32_t qcap = 0;
   int n_sm = 148; size_t smem_transport = 0;
@@ -208,7 +208,7 @@ int ensure_scratch(pmc_ctx *c, uint64_t chunk) {
     CK(c->d_resza.alloc(cap)); CK(c->d_resp.alloc((size_t)cap * 3));
     c->qcap = cap;
   }
-  CK(c->d_head.alloc(1)); CK(c->d_cnt.alloc(1));
+  CK(c->d_head.alloc(4)); CK(c->d_cnt.alloc(1));
   if (!c->h_pinned) CK(cudaMallocHost(&c->h_pinned, 64));
   if (!c->ev[0]) { CK(cudaEventCreate(&c->ev[0])); CK(cudaEventCreate(&c->ev[1])); }
   return PMC_OK;
@@ -276,7 +276,7 @@ int run_generations(pmc_ctx *c, RunParams P, uint32_t n0, bool profile) {
   ResQueue rq = res_queue(c);
   while (n_in > 0) {
     c->counters.n_generations++;
-    CK(cudaMemsetAsync(c->d_head.p, 0, 4, s)); CK(cudaMemsetAsync(nxt->q.count, 0, 4, s));
+    CK(cudaMemsetAsync(c->d_head.p, 0, 16, s)); CK(cudaMemsetAsync(nxt->q.count, 0, 4, s));
     CK(cudaMemsetAsync(c->qel.q.count, 0, 4, s)); CK(cudaMemsetAsync(c->qne.q.count, 0, 4, s)); CK(cudaMemsetAsync(c->qres.q.count, 0, 4, s));
     { Timer t(c, &c->timing.transport_ms, profile);
       transport_kernel<<<grid_t, 256, c->smem_transport, s>>>(c->T, c->G, P, cur->q, n_in, c->d_head.p, c->qel.q, c->qne.q, c->d_tally.p, c->d_cnt.p); }
@@ -285,9 +285,9 @@ int run_generations(pmc_ctx *c, RunParams P, uint32_t n0, bool profile) {
     { Timer t(c, &c->timing.elastic_ms, profile);
       elastic_kernel<<<grid_e, 256, 0, s>>>(c->T, P, c->qel.q, nxt->q, c->d_tally.p, c->d_cnt.p); }
     { Timer t(c, &c->timing.inc_ms, profile);
-      inc_kernel<<<c->n_sm * 8, 128, 0, s>>>(c->T, P, c->qne.q, nxt->q, rq, c->d_tally.p, c->d_cnt.p); }
+      inc_kernel<<<c->n_sm * 6, 128, 0, s>>>(c->T, P, c->qne.q, c->d_head.p + 1, nxt->q, rq, c->d_tally.p, c->d_cnt.p); }
     { Timer t(c, &c->timing.evaporation_ms, profile);
-      evap_kernel<<<c->n_sm * 8, 128, 0, s>>>(c->T, P, rq, nxt->q, c->d_tally.p, c->d_cnt.p); }
+      evap_kernel<<<c->n_sm * 8, 128, 0, s>>>(c->T, P, rq, c->d_head.p + 2, nxt->q, c->d_tally.p, c->d_cnt.p); }
     c->timing.launches_total += 3;
     CK(cudaMemcpyAsync(c->h_pinned, nxt->q.count, 4, cudaMemcpyDeviceToHost, s));
     CK(cudaStreamSynchronize(s));
@@ -358,7 +358,7 @@ void pmc_destroy(pmc_ctx *c) {
   c->d_nuc.release(); c->d_nuc1.release(); c->d_hu_own.release();
   c->qa.release(); c->qb.release(); c->qel.release(); c->qne.release(); c->qres.release(); c->d_resza.release(); c->d_resp.release();
   c->d_head.release(); c->d_cnt.release(); c->d_tally.release(); c->d_out.release();
-  c->d_spots.release(); c->d_cdf.release(); c->d_slots.release(); c->d_counts.release(); c->d_base.release();
+  c->d_spots.release(); c->d_cdf.release(); c->d_res.release(); c->d_slots.release(); c->d_counts.release(); c->d_base.release();
   if (c->h_pinned) cudaFreeHost(c->h_pinned);
   if (c->ev[0]) { cudaEventDestroy(c->ev[0]); cudaEventDestroy(c->ev[1]); }
   for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
@@ -563,11 +563,15 @@ int pmc_nonelastic(pmc_ctx *c, int Z, int A, double e_mev, uint64_t n, uint64_t 
   CK(c->d_nuc1.upload(hn, s));
   const uint32_t CH = 1u << 17;
   CK(c->d_slots.alloc((size_t)CH * MAX_SEC)); CK(c->d_counts.alloc(CH)); CK(c->d_base.alloc(1)); CK(c->d_cnt.alloc(1));
+  CK(c->d_res.alloc(CH)); CK(c->d_head.alloc(4));
   CK(cudaMemsetAsync(c->d_cnt.p, 0, sizeof(Counters), s)); CK(cudaMemsetAsync(c->d_base.p, 0, 8, s));
   c->counters = pmc_counters{};
   for (uint64_t ev0 = 0; ev0 < n; ev0 += CH) {
     const uint32_t nc = (uint32_t)std::min<uint64_t>(CH, n - ev0);
-    nonelastic_kernel<<<(nc + 127) / 128, 128, 0, s>>>(c->T, c->d_nuc1.p, (float)e_mev, seed, ev0, nc, c->d_slots.p, c->d_counts.p, c->d_cnt.p);
+    CK(cudaMemsetAsync(c->d_head.p, 0, 16, s));
+    const int gb = (int)std::min<uint32_t>((nc + 127) / 128, (uint32_t)c->n_sm * 8);
+    nonelastic_inc_kernel<<<gb, 128, 0, s>>>(c->T, c->d_nuc1.p, (float)e_mev, seed, ev0, nc, c->d_head.p + 1, c->d_slots.p, c->d_counts.p, c->d_res.p, c->d_cnt.p);
+    nonelastic_evap_kernel<<<gb, 128, 0, s>>>(c->T, c->d_nuc1.p, seed, ev0, nc, c->d_head.p + 2, c->d_slots.p, c->d_counts.p, c->d_res.p, c->d_cnt.p);
     scan_kernel<<<1, 1024, 0, s>>>(c->d_counts.p, nc, off_dev + ev0, c->d_base.p);
     compact_kernel<<<(nc + 255) / 256, 256, 0, s>>>(c->d_slots.p, c->d_counts.p, off_dev + ev0, nc, reinterpret_cast<SecRec *>(out_dev), capacity);
   }

@@ -20,7 +20,7 @@ constexpr int NQ = 64;              // quadrature bins of the evaporation spectr
 struct SecRec { int16_t Z, A; uint8_t origin, pad[3]; float ke; float dir[3]; };   // == pmc_secondary (24 B)
 static_assert(sizeof(SecRec) == 24, "pmc_secondary layout");
 
-struct OutNuc { int type; float ke; V3 dir; double p[3]; };                      // type 0 proton, 1 neutron
+struct OutNuc { int type; float ke; V3 dir; };                                   // type 0 proton, 1 neutron
 struct Residual { int Z, A; double estar; double P[3]; double mass_gs; };
 struct CascNucleon { V3 r, p; int type, shell; };
 
@@ -29,131 +29,176 @@ __device__ __forceinline__ double nmass(const Tables &T, int z, int a) {
   return (z < 0 || a < 1 || z >= T.zdim || a >= T.adim || z > a) ? 0.0 : T.mass[z * T.adim + a];
 }
 
-// one cascade attempt; false if no Pauli-allowed collision happened or the outcome is invalid (L75)
-__device__ bool inc_attempt(const Tables &T, const Nucleus &N, float t_in, Rng &g, OutNuc *out, int &n_out_ret,
-                            Residual &res) {
+// Per-lane state of one cascade attempt.  The cascade is written as a state machine (begin / step / finalize) so
+// that the 32 lanes of a warp execute the same step of 32 different cascades together: a thread-per-event loop nest
+// with early exits leaves the lanes serialised (measured: 1.4 active lanes per instruction).
+struct IncLane {
+  CascNucleon stack[CASC_STACK]; OutNuc out[MAX_INC_OUT];
+  CascNucleon c;
+  int sp, ncoll, n_out, np_out, guard; bool alive, failed;
+  double e_out_sum, pxs, pys, pzs;
+};
+
+// entry: uniform over the disc of radius rmax, travelling along +z (L75 "random point of entry"); refraction into
+// the outermost shell: gains V, tangential momentum conserved
+__device__ __forceinline__ void inc_begin(const Nucleus &N, float t_in, Rng &g, IncLane &L) {
   const int ns = N.nshell;
-  CascNucleon stack[CASC_STACK]; int sp = 0;
-  int ncoll = 0, n_out = 0, np_out = 0;
-  double e_out_sum = 0, pxs = 0, pys = 0, pzs = 0;
-  {
-    // entry: uniform over the disc of radius rmax, travelling along +z (L75 "random point of entry");
-    // refraction into the outermost shell: gains V, tangential momentum conserved
-    const uint4 r = g.next4();
-    const float b = N.rmax * sqrtf(u01(r.x)); float sph, cph; sincospif(2.0f * u01(r.y), &sph, &cph);
-    const V3 r0{b * cph, b * sph, -sqrtf(fmaxf(0.f, N.rmax * N.rmax - b * b))};
-    const float Tn = t_in + N.V[0][ns - 1], p0 = sqrtf(t_in * (t_in + 2.0f * MP)), p1 = sqrtf(Tn * (Tn + 2.0f * MP));
-    const V3 nh = unit(r0), pv{0.f, 0.f, p0};
-    const float pr = dot(pv, nh); const V3 pt = pv - pr * nh;
-    const float pr2 = p1 * p1 - dot(pt, pt);
-    stack[sp++] = {r0, pt + (-sqrtf(fmaxf(pr2, 0.f))) * nh, 0, ns - 1};
-  }
-  int guard = 0;
-  while (sp > 0) {
-    CascNucleon c = stack[--sp];
-    bool alive = true;
-    while (alive) {
-      if (++guard > 20000) return false;
-      const int k = c.shell, ty = c.type;
-      const float m = nucleon_mass(ty), p2 = dot(c.p, c.p), E = sqrtf(p2 + m * m), Tk = p2 / (E + m);
-      const V3 d = rsqrtf(p2) * c.p;
-      // candidate collisions with a proton and with a neutron of the Fermi sea (Reading R6.3)
-      float dbest = BIG, plab_best = 0.f; int tbest = -1; V3 qbest{0.f, 0.f, 0.f};
+  L.sp = 0; L.ncoll = 0; L.n_out = 0; L.np_out = 0; L.guard = 0; L.failed = false;
+  L.e_out_sum = 0; L.pxs = 0; L.pys = 0; L.pzs = 0;
+  const uint4 r = g.next4();
+  const float b = N.rmax * sqrtf(u01(r.x)); float sph, cph; sincospif(2.0f * u01(r.y), &sph, &cph);
+  const V3 r0{b * cph, b * sph, -sqrtf(fmaxf(0.f, N.rmax * N.rmax - b * b))};
+  const float Tn = t_in + N.V[0][ns - 1], p0 = sqrtf(t_in * (t_in + 2.0f * MP)), p1 = sqrtf(Tn * (Tn + 2.0f * MP));
+  const V3 nh = unit(r0), pv{0.f, 0.f, p0};
+  const float pr = dot(pv, nh); const V3 pt = pv - pr * nh;
+  const float pr2 = p1 * p1 - dot(pt, pt);
+  L.c = {r0, pt + (-sqrtf(fmaxf(pr2, 0.f))) * nh, 0, ns - 1};
+  L.alive = true;
+}
+__device__ __forceinline__ void inc_fail(IncLane &L) { L.failed = true; L.alive = false; L.sp = 0; }
+
+// one step of the nucleon being tracked: candidate collisions vs shell boundary (Reading R6.3-R6.5)
+__device__ __forceinline__ void inc_step(const Nucleus &N, Rng &g, IncLane &L) {
+  CascNucleon &c = L.c;
+  const int ns = N.nshell;
+  if (++L.guard > 20000) { inc_fail(L); return; }
+  const int k = c.shell, ty = c.type;
+  const float m = nucleon_mass(ty), p2 = dot(c.p, c.p), E = sqrtf(p2 + m * m), Tk = p2 / (E + m);
+  const V3 d = rsqrtf(p2) * c.p;
+  // candidate collisions with a proton and with a neutron of the Fermi sea (Reading R6.3)
+  float dbest = BIG, plab_best = 0.f; int tbest = -1; V3 qbest{0.f, 0.f, 0.f};
 #pragma unroll
-      for (int tp = 0; tp < 2; ++tp) {
-        if (N.rho[tp][k] <= 0.f) continue;
-        const uint4 r = g.next4();
-        const float mq = nucleon_mass(tp), qmag = N.pF[tp][k] * cbrtf(u01(r.x));
-        const V3 q = qmag * isotropic(r.y, r.z);
-        const float Eq = sqrtf(qmag * qmag + mq * mq);
-        const float e1 = (E * Eq - dot(c.p, q)) / mq;                       // projectile energy in the partner rest frame
-        const float plab = sqrtf(fmaxf(e1 * e1 - m * m, 0.f));
-        const float sig = N.const_sigma_mb >= 0.f ? N.const_sigma_mb
-                                                  : (tp == ty ? cug_sigma_pp(plab * 1e-3f) : cug_sigma_np(plab * 1e-3f));
-        const float dist = -__logf(u01(r.w)) / (N.rho[tp][k] * sig * 0.1f);  // 1 mb = 0.1 fm^2
-        if (dist < dbest) { dbest = dist; tbest = tp; qbest = q; plab_best = plab; }
-      }
-      // distance to the shell boundaries along d
-      const float rr = dot(c.r, c.r), bq = dot(c.r, d), r_out = N.rout[k], r_in = k > 0 ? N.rout[k - 1] : 0.f;
-      float dbound = -bq + sqrtf(fmaxf(bq * bq - (rr - r_out * r_out), 0.f)); bool inward = false;
-      if (k > 0 && bq < 0.f) {
-        const float disc = bq * bq - (rr - r_in * r_in);
-        if (disc > 0.f) { const float s_in = -bq - sqrtf(disc); if (s_in < dbound) { dbound = fmaxf(s_in, 0.f); inward = true; } }
-      }
-      if (dbest < dbound) {
-        // ---- collision attempt (Reading R6.4)
-        c.r = c.r + dbest * d;
-        const int tp = tbest; const float mq = nucleon_mass(tp);
-        const V3 q = qbest; const float Eq = sqrtf(dot(q, q) + mq * mq);
-        const V3 Pt = c.p + q; const float Et = E + Eq; const V3 beta = (1.0f / Et) * Pt;
-        const float s = Et * Et - dot(Pt, Pt);
-        const float pcm = sqrtf(fmaxf((s - (m + mq) * (m + mq)) * (s - (m - mq) * (m - mq)), 0.f) / (4.0f * s));
-        V3 p1 = c.p; float E1 = E; boost(-1.0f * beta, p1, E1);             // projectile in the CM
-        const V3 ax = unit(p1);
-        const uint4 r = g.next4();
-        const float ct = sample_nn_cos(tp == ty, plab_best * 1e-3f, pcm, r.x, r.y), st = sqrtf(fmaxf(0.f, 1.0f - ct * ct));
-        float sph, cph; sincospif(2.0f * u01(r.z), &sph, &cph);
-        V3 n1 = pcm * to_lab(ax, st * cph, st * sph, ct), n2 = -1.0f * n1;
-        float En1 = sqrtf(pcm * pcm + m * m), En2 = sqrtf(pcm * pcm + mq * mq);
-        boost(beta, n1, En1); boost(beta, n2, En2);
-        const float T1 = En1 - m, T2 = En2 - mq;
-        const bool ok = !N.pauli || (T1 > N.EF[ty][k] && T2 > N.EF[tp][k]);  // L77 Pauli blocking
-        if (!ok) continue;                                                   // blocked: go on unchanged
-        ncoll++;
-        // trapping (Reading R6.4): outside energy eps = T - V <= B_C stays in the nucleus
-        const float bc2 = tp == 0 ? N.coulomb : 0.f, bc1 = ty == 0 ? N.coulomb : 0.f;
-        if (T2 - N.V[tp][k] > bc2) { if (sp >= CASC_STACK) return false; stack[sp++] = {c.r, n2, tp, k}; }
-        if (T1 - N.V[ty][k] > bc1) c.p = n1; else alive = false;
-        continue;
-      }
-      // ---- shell boundary (L77 "reflection and refraction"; Reading R6.5)
-      c.r = c.r + dbound * d;
-      const float rb = inward ? r_in : r_out;
-      c.r = (rb * rsqrtf(dot(c.r, c.r))) * c.r;
-      const V3 nh = (1.0f / rb) * c.r;
-      const float pr = dot(c.p, nh); const V3 pt = c.p - pr * nh;
-      const int k2 = inward ? k - 1 : k + 1;
-      const float Vnew = k2 >= ns ? 0.f : N.V[ty][k2], T2 = Tk + (Vnew - N.V[ty][k]);
-      const float pn2 = T2 > 0.f ? T2 * (T2 + 2.0f * m) : -1.0f, pr2 = pn2 - dot(pt, pt);
-      if (pn2 <= 0.f || pr2 <= 0.f) { c.p = pt - pr * nh; continue; }         // specular reflection
-      const V3 pnew = pt + ((pr > 0.f ? 1.0f : -1.0f) * sqrtf(pr2)) * nh;
-      if (k2 >= ns) {                                                       // leaves the nucleus with KE = eps
-        if (n_out >= MAX_INC_OUT) return false;
-        OutNuc &o = out[n_out++];
-        o.type = ty; o.ke = T2; o.dir = unit(pnew); o.p[0] = pnew.x; o.p[1] = pnew.y; o.p[2] = pnew.z;
-        e_out_sum += (double)T2 + (ty == 0 ? MP_D : MN_D); pxs += pnew.x; pys += pnew.y; pzs += pnew.z;
-        if (ty == 0) np_out++;
-        alive = false;
-      } else { c.p = pnew; c.shell = k2; }
-    }
+  for (int tp = 0; tp < 2; ++tp) {
+    if (N.rho[tp][k] <= 0.f) continue;
+    const uint4 r = g.next4();
+    const float mq = nucleon_mass(tp), qmag = N.pF[tp][k] * cbrtf(u01(r.x));
+    const V3 q = qmag * isotropic(r.y, r.z);
+    const float Eq = sqrtf(qmag * qmag + mq * mq);
+    const float e1 = (E * Eq - dot(c.p, q)) / mq;                       // projectile energy in the partner rest frame
+    const float plab = sqrtf(fmaxf(e1 * e1 - m * m, 0.f));
+    const float sig = N.const_sigma_mb >= 0.f ? N.const_sigma_mb
+                                              : (tp == ty ? cug_sigma_pp(plab * 1e-3f) : cug_sigma_np(plab * 1e-3f));
+    const float dist = -__logf(u01(r.w)) / (N.rho[tp][k] * sig * 0.1f);  // 1 mb = 0.1 fm^2
+    if (dist < dbest) { dbest = dist; tbest = tp; qbest = q; plab_best = plab; }
   }
-  if (ncoll == 0) return false;                                             // L75: need >= 1 allowed collision
-  // ---- residual nucleus (Reading R6.7): exact integers, relativistic invariant mass, fp64
-  const int Ar = N.A + 1 - n_out, Zr = N.Z + 1 - np_out;
+  // distance to the shell boundaries along d
+  const float rr = dot(c.r, c.r), bq = dot(c.r, d), r_out = N.rout[k], r_in = k > 0 ? N.rout[k - 1] : 0.f;
+  float dbound = -bq + sqrtf(fmaxf(bq * bq - (rr - r_out * r_out), 0.f)); bool inward = false;
+  if (k > 0 && bq < 0.f) {
+    const float disc = bq * bq - (rr - r_in * r_in);
+    if (disc > 0.f) { const float s_in = -bq - sqrtf(disc); if (s_in < dbound) { dbound = fmaxf(s_in, 0.f); inward = true; } }
+  }
+  if (dbest < dbound) {
+    // ---- collision attempt (Reading R6.4)
+    c.r = c.r + dbest * d;
+    const int tp = tbest; const float mq = nucleon_mass(tp);
+    const V3 q = qbest; const float Eq = sqrtf(dot(q, q) + mq * mq);
+    const V3 Pt = c.p + q; const float Et = E + Eq; const V3 beta = (1.0f / Et) * Pt;
+    const float s = Et * Et - dot(Pt, Pt);
+    const float pcm = sqrtf(fmaxf((s - (m + mq) * (m + mq)) * (s - (m - mq) * (m - mq)), 0.f) / (4.0f * s));
+    V3 p1 = c.p; float E1 = E; boost(-1.0f * beta, p1, E1);             // projectile in the CM
+    const V3 ax = unit(p1);
+    const uint4 r = g.next4();
+    const float ct = sample_nn_cos(tp == ty, plab_best * 1e-3f, pcm, r.x, r.y), st = sqrtf(fmaxf(0.f, 1.0f - ct * ct));
+    float sph, cph; sincospif(2.0f * u01(r.z), &sph, &cph);
+    V3 n1 = pcm * to_lab(ax, st * cph, st * sph, ct), n2 = -1.0f * n1;
+    float En1 = sqrtf(pcm * pcm + m * m), En2 = sqrtf(pcm * pcm + mq * mq);
+    boost(beta, n1, En1); boost(beta, n2, En2);
+    const float T1 = En1 - m, T2 = En2 - mq;
+    const bool ok = !N.pauli || (T1 > N.EF[ty][k] && T2 > N.EF[tp][k]);  // L77 Pauli blocking
+    if (!ok) return;                                                     // blocked: go on unchanged
+    L.ncoll++;
+    // trapping (Reading R6.4): outside energy eps = T - V <= B_C stays in the nucleus
+    const float bc2 = tp == 0 ? N.coulomb : 0.f, bc1 = ty == 0 ? N.coulomb : 0.f;
+    if (T2 - N.V[tp][k] > bc2) {
+      if (L.sp >= CASC_STACK) { inc_fail(L); return; }
+      L.stack[L.sp++] = {c.r, n2, tp, k};
+    }
+    if (T1 - N.V[ty][k] > bc1) c.p = n1; else L.alive = false;
+    return;
+  }
+  // ---- shell boundary (L77 "reflection and refraction"; Reading R6.5)
+  c.r = c.r + dbound * d;
+  const float rb = inward ? r_in : r_out;
+  c.r = (rb * rsqrtf(dot(c.r, c.r))) * c.r;
+  const V3 nh = (1.0f / rb) * c.r;
+  const float pr = dot(c.p, nh); const V3 pt = c.p - pr * nh;
+  const int k2 = inward ? k - 1 : k + 1;
+  const float Vnew = k2 >= ns ? 0.f : N.V[ty][k2], T2 = Tk + (Vnew - N.V[ty][k]);
+  const float pn2 = T2 > 0.f ? T2 * (T2 + 2.0f * m) : -1.0f, pr2 = pn2 - dot(pt, pt);
+  if (pn2 <= 0.f || pr2 <= 0.f) { c.p = pt - pr * nh; return; }           // specular reflection
+  const V3 pnew = pt + ((pr > 0.f ? 1.0f : -1.0f) * sqrtf(pr2)) * nh;
+  if (k2 >= ns) {                                                       // leaves the nucleus with KE = eps
+    if (L.n_out >= MAX_INC_OUT) { inc_fail(L); return; }
+    OutNuc &o = L.out[L.n_out++];
+    o.type = ty; o.ke = T2; o.dir = unit(pnew);
+    L.e_out_sum += (double)T2 + (ty == 0 ? MP_D : MN_D); L.pxs += pnew.x; L.pys += pnew.y; L.pzs += pnew.z;
+    if (ty == 0) L.np_out++;
+    L.alive = false;
+  } else { c.p = pnew; c.shell = k2; }
+}
+
+// end of an attempt: false if no Pauli-allowed collision happened or the outcome is invalid (L75); else the
+// residual nucleus (Reading R6.7): exact integers, relativistic invariant mass, fp64
+__device__ __forceinline__ bool inc_finalize(const Tables &T, const Nucleus &N, float t_in, const IncLane &L, Residual &res) {
+  if (L.failed || L.ncoll == 0) return false;                               // L75: need >= 1 allowed collision
+  const int Ar = N.A + 1 - L.n_out, Zr = N.Z + 1 - L.np_out;
   const double Mgs = nmass(T, Zr, Ar);
   if (Ar < 1 || Zr < 0 || Zr > Ar || Mgs <= 0) return false;
   const double tin = (double)t_in, pin = sqrt(tin * (tin + 2 * MP_D));
-  const double Eres = (tin + MP_D + N.mass) - e_out_sum, Px = -pxs, Py = -pys, Pz = pin - pzs;
+  const double Eres = (tin + MP_D + N.mass) - L.e_out_sum, Px = -L.pxs, Py = -L.pys, Pz = pin - L.pzs;
   const double M2 = Eres * Eres - (Px * Px + Py * Py + Pz * Pz);
   if (Eres <= 0 || M2 <= 0) return false;
   const double estar = sqrt(M2) - Mgs;
   if (estar < 0) return false;
   if (Ar == 1 && estar > 1e-4) return false;                                // a lone nucleon cannot be excited
   res.Z = Zr; res.A = Ar; res.estar = estar; res.P[0] = Px; res.P[1] = Py; res.P[2] = Pz; res.mass_gs = Mgs;
-  n_out_ret = n_out;
   return true;
 }
-
-__device__ void inc_event(const Tables &T, const Nucleus &N, float t_in, Rng &g, OutNuc *out, int &n_out, Residual &res,
-                          unsigned long long &tries) {
-  for (int it = 0; it < 100000; ++it) {                 // L75 "This is repeated until ..."
-    tries++;
-    if (inc_attempt(T, N, t_in, g, out, n_out, res)) return;
-  }
-  // Reading R6.8 (never reached in the configs): form the compound nucleus (Z+1, A+1)
-  n_out = 0;
+// Reading R6.8 (never reached in the configs): after 1e5 failed attempts form the compound nucleus (Z+1, A+1)
+__device__ __forceinline__ void inc_compound(const Tables &T, const Nucleus &N, float t_in, Residual &res) {
   const double tin = (double)t_in, pin = sqrt(tin * (tin + 2 * MP_D)), Et = tin + MP_D + N.mass, Mgs = nmass(T, N.Z + 1, N.A + 1);
   res.Z = N.Z + 1; res.A = N.A + 1; res.estar = sqrt(Et * Et - pin * pin) - Mgs; res.P[0] = 0; res.P[1] = 0; res.P[2] = pin; res.mass_gs = Mgs;
+}
+
+// Warp-synchronous cascade engine: every lane owns one event at a time and all 32 lanes take one cascade step per
+// trip of the loop; a lane whose event is done fetches the next one from the shared counter `head` (warp-aggregated).
+// load(i, N, t_in, g) sets up event i; store(i, g, out, n_out, R) consumes its result.  L75: the attempt is repeated
+// (fresh draws of the same stream) until it has at least one Pauli-allowed collision and a valid residual.
+// All 32 lanes of every warp must call.
+template <class Load, class Store>
+__device__ __forceinline__ void inc_machine(const Tables &T, uint32_t n, uint32_t *head, unsigned long long &tries,
+                                            Load load, Store store) {
+  IncLane L; L.alive = false; L.sp = 0; L.failed = false;
+  const Nucleus *N = nullptr; float t_in = 0.f; Rng g; uint32_t ev = 0; int ntry = 0;
+  bool busy = false, exhausted = false;
+  const int lane = threadIdx.x & 31;
+  while (true) {
+    const unsigned need = __ballot_sync(0xffffffffu, !busy && !exhausted);
+    if (need) {
+      const int leader = __ffs(need) - 1;
+      uint32_t base = 0;
+      if (lane == leader) base = atomicAdd(head, (uint32_t)__popc(need));
+      base = __shfl_sync(0xffffffffu, base, leader);
+      if (!busy && !exhausted) {
+        ev = base + (uint32_t)__popc(need & ((1u << lane) - 1u));
+        if (ev < n) { load(ev, N, t_in, g); busy = true; ntry = 1; tries++; inc_begin(*N, t_in, g, L); }
+        else exhausted = true;
+      }
+    }
+    if (!__any_sync(0xffffffffu, busy)) break;
+    if (busy && !L.alive) {
+      if (L.sp > 0) { L.c = L.stack[--L.sp]; L.alive = true; }
+      else {
+        Residual R;
+        if (inc_finalize(T, *N, t_in, L, R)) { store(ev, g, L.out, L.n_out, R); busy = false; }
+        else if (ntry >= 100000) { inc_compound(T, *N, t_in, R); store(ev, g, L.out, 0, R); busy = false; }
+        else { ++ntry; tries++; inc_begin(*N, t_in, g, L); }
+      }
+    }
+    __syncwarp();
+    if (busy && L.alive) inc_step(*N, g, L);
+  }
 }
 
 // ------------------------------------------------------------------ evaporation (Reading R7)
@@ -244,124 +289,172 @@ __device__ __forceinline__ double residual_ke(const Residual &R) {
   return p2 / (sqrt(p2 + Mres * Mres) + Mres);
 }
 
+// Warp-synchronous evaporation engine (same scheme as inc_machine): one emission per lane per trip of the loop.
+// load(i, R, g) sets up residual i; emit(i, g, em) consumes one emitted particle; done(i, g, R) the final residual.
+template <class Load, class Emit, class Done>
+__device__ __forceinline__ void evap_machine(const Tables &T, uint32_t n, uint32_t *head, Load load, Emit emit, Done done) {
+  Residual R; Rng g; uint32_t ev = 0; int nem = 0;
+  bool busy = false, exhausted = false;
+  const int lane = threadIdx.x & 31;
+  while (true) {
+    const unsigned need = __ballot_sync(0xffffffffu, !busy && !exhausted);
+    if (need) {
+      const int leader = __ffs(need) - 1;
+      uint32_t base = 0;
+      if (lane == leader) base = atomicAdd(head, (uint32_t)__popc(need));
+      base = __shfl_sync(0xffffffffu, base, leader);
+      if (!busy && !exhausted) {
+        ev = base + (uint32_t)__popc(need & ((1u << lane) - 1u));
+        if (ev < n) { load(ev, R, g); busy = true; nem = 0; }
+        else exhausted = true;
+      }
+    }
+    if (!__any_sync(0xffffffffu, busy)) break;
+    Emission em; bool ok = false;
+    if (busy) ok = nem < 200 && evap_emit(T, R, g, 0x3Fu, em, nullptr, nullptr);
+    __syncwarp();
+    if (busy) {
+      if (ok) { ++nem; emit(ev, g, em); }
+      else { done(ev, g, R); busy = false; }
+    }
+  }
+}
+
 // ------------------------------------------------------------------ event-queue kernels of the transport scheduler
 struct ResQueue { Queue q; uint32_t *za; float *px, *py, *pz; };   // q.e = E*, q.aux = next product index
 
-// K3: one cascade per thread over the non-elastic queue (PAPER.md:L128(3), L136)
-__global__ void __launch_bounds__(128) inc_kernel(Tables T, RunParams P, Queue in, Queue out, ResQueue rq, float *tally,
-                                                  Counters *cnt) {
+// K3: intranuclear cascades over the non-elastic queue (PAPER.md:L128(3), L136), one event per lane at a time
+__global__ void __launch_bounds__(128) inc_kernel(Tables T, RunParams P, Queue in, uint32_t *head, Queue out, ResQueue rq,
+                                                  float *tally, Counters *cnt) {
   const uint32_t n = min(*in.count, in.cap);
   double c_dep = 0, c_neu = 0, c_q = 0; unsigned long long c_sec = 0, c_tries = 0;
-  for (uint32_t i0 = blockIdx.x * blockDim.x; i0 < n; i0 += gridDim.x * blockDim.x) {
-    const uint32_t i = i0 + threadIdx.x;
-    if (i < n) {
-      Particle p = queue_load(in, i);
-      Rng g; g.init(P.seed, P.hist0 + p.hist, p.pid, p.blk);
-      const Nucleus &N = T.nuc[p.aux];
-      OutNuc outn[MAX_INC_OUT]; int n_out = 0; Residual R;
-      inc_event(T, N, p.e, g, outn, n_out, R, c_tries);
-      float dep = 0.f; uint32_t kchild = 0; double msum = 0;
-      for (int k = 0; k < n_out; ++k) {
-        const OutNuc &o = outn[k];
-        msum += o.type == 0 ? MP_D : MN_D;
-        if (o.type == 0) {                                                   // L79: only protons are followed
-          if (o.ke > T.e_cut) {
-            Particle s = p; s.d = unit(to_lab(p.d, o.dir.x, o.dir.y, o.dir.z)); s.e = o.ke;
-            s.pid = g.child_id(kchild++); s.blk = 0u; s.aux = 0u; c_sec++;
-            if (!queue_push(out, s)) atomicOr(&cnt->overflow, 16u);
-          } else dep += o.ke;
-        } else c_neu += (double)o.ke;                                        // neutrons: not transported
-      }
-      c_q += msum + R.mass_gs - MP_D - N.mass;
-      if (dep != 0.f) { atomicAdd(tally + batch_base(P, p.hist) + (uint32_t)p.vox, dep); c_dep += (double)dep; }
-      // residual -> evaporation queue (keeps the event frame: p.d is the incident direction)
-      const uint32_t slot = warp_alloc(rq.q.count);
-      if (slot >= rq.q.cap) atomicOr(&cnt->overflow, 32u);
-      else {
-        const Queue &q = rq.q;
-        q.x[slot] = p.r.x; q.y[slot] = p.r.y; q.z[slot] = p.r.z; q.u[slot] = p.d.x; q.v[slot] = p.d.y; q.w[slot] = p.d.z;
-        q.e[slot] = (float)R.estar; q.vox[slot] = p.vox; q.hist[slot] = p.hist; q.pid[slot] = p.pid; q.blk[slot] = g.blk;
-        q.aux[slot] = kchild; rq.za[slot] = ((uint32_t)R.Z << 16) | (uint32_t)R.A;
-        rq.px[slot] = (float)R.P[0]; rq.py[slot] = (float)R.P[1]; rq.pz[slot] = (float)R.P[2];
-      }
+  Particle p;
+  auto load = [&](uint32_t i, const Nucleus *&N, float &t_in, Rng &g) {
+    p = queue_load(in, i);
+    g.init(P.seed, P.hist0 + p.hist, p.pid, p.blk);
+    N = &T.nuc[p.aux]; t_in = p.e;
+  };
+  auto store = [&](uint32_t, Rng &g, const OutNuc *outn, int n_out, const Residual &R) {
+    const Nucleus &N = T.nuc[p.aux];
+    float dep = 0.f; uint32_t kchild = 0; double msum = 0;
+    for (int k = 0; k < n_out; ++k) {
+      const OutNuc &o = outn[k];
+      msum += o.type == 0 ? MP_D : MN_D;
+      if (o.type == 0) {                                                   // L79: only protons are followed
+        if (o.ke > T.e_cut) {
+          Particle s = p; s.d = unit(to_lab(p.d, o.dir.x, o.dir.y, o.dir.z)); s.e = o.ke;
+          s.pid = g.child_id(kchild++); s.blk = 0u; s.aux = 0u; c_sec++;
+          if (!queue_push(out, s)) atomicOr(&cnt->overflow, 16u);
+        } else dep += o.ke;
+      } else c_neu += (double)o.ke;                                        // neutrons: not transported
     }
-  }
+    c_q += msum + R.mass_gs - MP_D - N.mass;
+    if (dep != 0.f) { atomicAdd(tally + batch_base(P, p.hist) + (uint32_t)p.vox, dep); c_dep += (double)dep; }
+    // residual -> evaporation queue (keeps the event frame: p.d is the incident direction)
+    const uint32_t slot = warp_alloc(rq.q.count);
+    if (slot >= rq.q.cap) atomicOr(&cnt->overflow, 32u);
+    else {
+      const Queue &q = rq.q;
+      q.x[slot] = p.r.x; q.y[slot] = p.r.y; q.z[slot] = p.r.z; q.u[slot] = p.d.x; q.v[slot] = p.d.y; q.w[slot] = p.d.z;
+      q.e[slot] = (float)R.estar; q.vox[slot] = p.vox; q.hist[slot] = p.hist; q.pid[slot] = p.pid; q.blk[slot] = g.blk;
+      q.aux[slot] = kchild; rq.za[slot] = ((uint32_t)R.Z << 16) | (uint32_t)R.A;
+      rq.px[slot] = (float)R.P[0]; rq.py[slot] = (float)R.P[1]; rq.pz[slot] = (float)R.P[2];
+    }
+  };
+  inc_machine(T, n, head, c_tries, load, store);
   flush(&cnt->e_deposit, c_dep); flush(&cnt->e_neutron, c_neu); flush(&cnt->e_q, c_q);
   flush(&cnt->n_secondary, c_sec); flush(&cnt->n_inc_tries, c_tries);
 }
 
-// K4: one nuclear de-excitation per thread over the residual queue (PAPER.md:L128(4), L136)
-__global__ void __launch_bounds__(128) evap_kernel(Tables T, RunParams P, ResQueue rq, Queue out, float *tally, Counters *cnt) {
+// K4: nuclear de-excitations over the residual queue (PAPER.md:L128(4), L136), one residual per lane at a time
+__global__ void __launch_bounds__(128) evap_kernel(Tables T, RunParams P, ResQueue rq, uint32_t *head, Queue out, float *tally,
+                                                   Counters *cnt) {
   const uint32_t n = min(*rq.q.count, rq.q.cap);
   double c_dep = 0, c_neu = 0, c_q = 0, c_gam = 0; unsigned long long c_sec = 0;
-  for (uint32_t i0 = blockIdx.x * blockDim.x; i0 < n; i0 += gridDim.x * blockDim.x) {
-    const uint32_t i = i0 + threadIdx.x;
-    if (i < n) {
-      Particle p = queue_load(rq.q, i);
-      Rng g; g.init(P.seed, P.hist0 + p.hist, p.pid, p.blk);
-      Residual R; R.Z = (int)(rq.za[i] >> 16); R.A = (int)(rq.za[i] & 0xffffu); R.estar = (double)p.e;
-      R.P[0] = rq.px[i]; R.P[1] = rq.py[i]; R.P[2] = rq.pz[i]; R.mass_gs = nmass(T, R.Z, R.A);
-      const double m0 = R.mass_gs; double msum = 0;
-      uint32_t kchild = p.aux; float dep = 0.f;
-      for (int it = 0; it < 200; ++it) {
-        Emission em;
-        if (!evap_emit(T, R, g, 0x3Fu, em, nullptr, nullptr)) break;
-        msum += nmass(T, EJ_Z[em.j], EJ_A[em.j]);
-        if (em.j == 1) {
-          if (em.ke > T.e_cut) {
-            Particle s = p; s.d = unit(to_lab(p.d, em.dir.x, em.dir.y, em.dir.z)); s.e = em.ke;
-            s.pid = g.child_id(kchild++); s.blk = 0u; s.aux = 0u; c_sec++;
-            if (!queue_push(out, s)) atomicOr(&cnt->overflow, 64u);
-          } else dep += em.ke;
-        } else if (em.j == 0) c_neu += (double)em.ke;
-        else dep += em.ke;                                                   // d, t, 3He, alpha: local (L79)
-      }
-      const double kres = residual_ke(R);
-      if (R.A == 1 && R.Z == 0) c_neu += kres; else dep += (float)kres;
-      c_gam += R.estar;                                                     // L79: no photon evaporation
-      c_q += msum + R.mass_gs - m0;
-      if (dep != 0.f) { atomicAdd(tally + batch_base(P, p.hist) + (uint32_t)p.vox, dep); c_dep += (double)dep; }
-    }
-  }
+  Particle p; double m0 = 0, msum = 0; uint32_t kchild = 0; float dep = 0.f;
+  auto load = [&](uint32_t i, Residual &R, Rng &g) {
+    p = queue_load(rq.q, i);
+    g.init(P.seed, P.hist0 + p.hist, p.pid, p.blk);
+    R.Z = (int)(rq.za[i] >> 16); R.A = (int)(rq.za[i] & 0xffffu); R.estar = (double)p.e;
+    R.P[0] = rq.px[i]; R.P[1] = rq.py[i]; R.P[2] = rq.pz[i]; R.mass_gs = nmass(T, R.Z, R.A);
+    m0 = R.mass_gs; msum = 0; kchild = p.aux; dep = 0.f;
+  };
+  auto emit = [&](uint32_t, Rng &g, const Emission &em) {
+    msum += nmass(T, EJ_Z[em.j], EJ_A[em.j]);
+    if (em.j == 1) {
+      if (em.ke > T.e_cut) {
+        Particle s = p; s.d = unit(to_lab(p.d, em.dir.x, em.dir.y, em.dir.z)); s.e = em.ke;
+        s.pid = g.child_id(kchild++); s.blk = 0u; s.aux = 0u; c_sec++;
+        if (!queue_push(out, s)) atomicOr(&cnt->overflow, 64u);
+      } else dep += em.ke;
+    } else if (em.j == 0) c_neu += (double)em.ke;
+    else dep += em.ke;                                                     // d, t, 3He, alpha: local (L79)
+  };
+  auto done = [&](uint32_t, Rng &, const Residual &R) {
+    const double kres = residual_ke(R);
+    if (R.A == 1 && R.Z == 0) c_neu += kres; else dep += (float)kres;
+    c_gam += R.estar;                                                       // L79: no photon evaporation
+    c_q += msum + R.mass_gs - m0;
+    if (dep != 0.f) { atomicAdd(tally + batch_base(P, p.hist) + (uint32_t)p.vox, dep); c_dep += (double)dep; }
+  };
+  evap_machine(T, n, head, load, emit, done);
   flush(&cnt->e_deposit, c_dep); flush(&cnt->e_neutron, c_neu); flush(&cnt->e_q, c_q); flush(&cnt->e_gamma, c_gam);
   flush(&cnt->n_secondary, c_sec);
 }
 
 // ------------------------------------------------------------------ standalone non-elastic events (pmc_nonelastic; Table I)
-__global__ void __launch_bounds__(128) nonelastic_kernel(Tables T, const Nucleus *nuc, float t_in, uint64_t seed, uint64_t ev0,
-                                                         uint32_t n, SecRec *slots, uint32_t *counts, Counters *cnt) {
-  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
-  unsigned long long c_tries = 0, c_bad = 0; double c_gam = 0;
-  if (i < n) {
-    const Nucleus &N = *nuc;
-    Rng g; g.init(seed, ev0 + i, 0u, 0u);
-    OutNuc outn[MAX_INC_OUT]; int n_out = 0; Residual R;
-    inc_event(T, N, t_in, g, outn, n_out, R, c_tries);
-    SecRec *s = slots + (size_t)i * MAX_SEC; int ns = 0, zs = 0, as = 0;
+// Two kernels like the scheduler's (cascade, then de-excitation); event i of the call uses the stream (seed, ev0 + i).
+struct ResRec { int Z, A; double estar; double P[3]; uint32_t blk; int zs, as; };
+
+__global__ void __launch_bounds__(128) nonelastic_inc_kernel(Tables T, const Nucleus *nuc, float t_in0, uint64_t seed, uint64_t ev0,
+                                                             uint32_t n, uint32_t *head, SecRec *slots, uint32_t *counts,
+                                                             ResRec *res, Counters *cnt) {
+  unsigned long long c_tries = 0;
+  auto load = [&](uint32_t i, const Nucleus *&N, float &t_in, Rng &g) { g.init(seed, ev0 + i, 0u, 0u); N = nuc; t_in = t_in0; };
+  auto store = [&](uint32_t i, Rng &g, const OutNuc *outn, int n_out, const Residual &R) {
+    SecRec *s = slots + (size_t)i * MAX_SEC; int zs = 0;
     for (int k = 0; k < n_out; ++k) {
       SecRec rec{}; rec.Z = outn[k].type == 0 ? 1 : 0; rec.A = 1; rec.origin = 0; rec.ke = outn[k].ke;
       rec.dir[0] = outn[k].dir.x; rec.dir[1] = outn[k].dir.y; rec.dir[2] = outn[k].dir.z;
-      zs += rec.Z; as += 1; s[ns++] = rec;
+      zs += rec.Z; s[k] = rec;
     }
-    for (int it = 0; it < 200; ++it) {
-      Emission em;
-      if (!evap_emit(T, R, g, 0x3Fu, em, nullptr, nullptr)) break;
-      SecRec rec{}; rec.Z = (int16_t)EJ_Z[em.j]; rec.A = (int16_t)EJ_A[em.j]; rec.origin = 1; rec.ke = em.ke;
-      rec.dir[0] = em.dir.x; rec.dir[1] = em.dir.y; rec.dir[2] = em.dir.z;
-      zs += rec.Z; as += rec.A;
-      if (ns < MAX_SEC - 1) s[ns++] = rec; else atomicOr(&cnt->overflow, 128u);
-    }
-    {
-      const double pn = sqrt(R.P[0] * R.P[0] + R.P[1] * R.P[1] + R.P[2] * R.P[2]);
-      SecRec rec{}; rec.Z = (int16_t)R.Z; rec.A = (int16_t)R.A; rec.origin = 2; rec.ke = (float)residual_ke(R);
-      if (pn > 0) { rec.dir[0] = (float)(R.P[0] / pn); rec.dir[1] = (float)(R.P[1] / pn); rec.dir[2] = (float)(R.P[2] / pn); }
-      else { rec.dir[2] = 1.f; }
-      zs += R.Z; as += R.A; s[ns++] = rec;
-    }
-    if (zs != N.Z + 1 || as != N.A + 1) c_bad++;
-    counts[i] = (uint32_t)ns; c_gam = R.estar;
-  }
-  flush(&cnt->n_inc_tries, c_tries); flush(&cnt->n_zab_bad, c_bad); flush(&cnt->e_gamma, c_gam);
+    counts[i] = (uint32_t)n_out;
+    ResRec rr; rr.Z = R.Z; rr.A = R.A; rr.estar = R.estar; rr.P[0] = R.P[0]; rr.P[1] = R.P[1]; rr.P[2] = R.P[2];
+    rr.blk = g.blk; rr.zs = zs; rr.as = n_out;
+    res[i] = rr;
+  };
+  inc_machine(T, n, head, c_tries, load, store);
+  flush(&cnt->n_inc_tries, c_tries);
+}
+
+__global__ void __launch_bounds__(128) nonelastic_evap_kernel(Tables T, const Nucleus *nuc, uint64_t seed, uint64_t ev0, uint32_t n,
+                                                              uint32_t *head, SecRec *slots, uint32_t *counts, const ResRec *res,
+                                                              Counters *cnt) {
+  unsigned long long c_bad = 0; double c_gam = 0;
+  int ns = 0, zs = 0, as = 0;
+  auto load = [&](uint32_t i, Residual &R, Rng &g) {
+    const ResRec rr = res[i];
+    g.init(seed, ev0 + i, 0u, rr.blk);
+    R.Z = rr.Z; R.A = rr.A; R.estar = rr.estar; R.P[0] = rr.P[0]; R.P[1] = rr.P[1]; R.P[2] = rr.P[2]; R.mass_gs = nmass(T, rr.Z, rr.A);
+    ns = (int)counts[i]; zs = rr.zs; as = rr.as;
+  };
+  auto emit = [&](uint32_t i, Rng &, const Emission &em) {
+    SecRec rec{}; rec.Z = (int16_t)EJ_Z[em.j]; rec.A = (int16_t)EJ_A[em.j]; rec.origin = 1; rec.ke = em.ke;
+    rec.dir[0] = em.dir.x; rec.dir[1] = em.dir.y; rec.dir[2] = em.dir.z;
+    zs += rec.Z; as += rec.A;
+    if (ns < MAX_SEC - 1) slots[(size_t)i * MAX_SEC + ns++] = rec; else atomicOr(&cnt->overflow, 128u);
+  };
+  auto done = [&](uint32_t i, Rng &, const Residual &R) {
+    const double pn = sqrt(R.P[0] * R.P[0] + R.P[1] * R.P[1] + R.P[2] * R.P[2]);
+    SecRec rec{}; rec.Z = (int16_t)R.Z; rec.A = (int16_t)R.A; rec.origin = 2; rec.ke = (float)residual_ke(R);
+    if (pn > 0) { rec.dir[0] = (float)(R.P[0] / pn); rec.dir[1] = (float)(R.P[1] / pn); rec.dir[2] = (float)(R.P[2] / pn); }
+    else { rec.dir[2] = 1.f; }
+    zs += R.Z; as += R.A; slots[(size_t)i * MAX_SEC + ns++] = rec;
+    if (zs != nuc->Z + 1 || as != nuc->A + 1) c_bad++;
+    counts[i] = (uint32_t)ns; c_gam += R.estar;
+  };
+  evap_machine(T, n, head, load, emit, done);
+  flush(&cnt->n_zab_bad, c_bad); flush(&cnt->e_gamma, c_gam);
 }
 
 // exclusive scan of counts[n] -> off[n+1] shifted by base (single block; n <= a few 1e5)
