@@ -248,7 +248,7 @@ bool inc_attempt(const Tables &T, const Nucleus &N, double t_in, Rng &g, std::ve
     CascNucleon c = stack.back(); stack.pop_back();
     bool alive = true;
     while (alive) {
-      if (++guard > 20000) return false;
+      if (++guard > 1024) return false;      // Reading R6.8: a nucleon on a bound orbit in a dilute shell never ends the attempt
       int k = c.shell, ty = c.type;
       double m = nucleon_mass(ty), p2 = dot(c.p, c.p), E = std::sqrt(p2 + m * m), Tk = E - m;
       V3 d = (1.0 / std::sqrt(p2)) * c.p;

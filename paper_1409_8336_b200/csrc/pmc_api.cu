@@ -272,14 +272,14 @@ int run_generations(pmc_ctx *c, RunParams P, uint32_t n0, bool profile) {
   cudaStream_t s = c->stream;
   QueueMem *cur = &c->qa, *nxt = &c->qb;
   uint32_t n_in = n0;
-  const int grid_t = c->n_sm * 2, grid_e = c->n_sm * 4;
+  const int grid_t = c->n_sm * TRANSPORT_BLOCKS_PER_SM, grid_e = c->n_sm * 4;
   ResQueue rq = res_queue(c);
   while (n_in > 0) {
     c->counters.n_generations++;
     CK(cudaMemsetAsync(c->d_head.p, 0, 16, s)); CK(cudaMemsetAsync(nxt->q.count, 0, 4, s));
     CK(cudaMemsetAsync(c->qel.q.count, 0, 4, s)); CK(cudaMemsetAsync(c->qne.q.count, 0, 4, s)); CK(cudaMemsetAsync(c->qres.q.count, 0, 4, s));
     { Timer t(c, &c->timing.transport_ms, profile);
-      transport_kernel<<<grid_t, 256, c->smem_transport, s>>>(c->T, c->G, P, cur->q, n_in, c->d_head.p, c->qel.q, c->qne.q, c->d_tally.p, c->d_cnt.p); }
+      transport_kernel<<<grid_t, TRANSPORT_THREADS, c->smem_transport, s>>>(c->T, c->G, P, cur->q, n_in, c->d_head.p, c->qel.q, c->qne.q, c->d_tally.p, c->d_cnt.p); }
     c->timing.launches_total++; c->timing.launches_transport++;
     if (P.dbg_out) break;
     { Timer t(c, &c->timing.elastic_ms, profile);
@@ -561,7 +561,7 @@ int pmc_nonelastic(pmc_ctx *c, int Z, int A, double e_mev, uint64_t n, uint64_t 
   cudaStream_t s = c->stream;
   std::vector<Nucleus> hn(1, build_nucleus(c, Z, A));
   CK(c->d_nuc1.upload(hn, s));
-  const uint32_t CH = 1u << 17;
+  const uint32_t CH = 1u << 19;
   CK(c->d_slots.alloc((size_t)CH * MAX_SEC)); CK(c->d_counts.alloc(CH)); CK(c->d_base.alloc(1)); CK(c->d_cnt.alloc(1));
   CK(c->d_res.alloc(CH)); CK(c->d_head.alloc(4));
   CK(cudaMemsetAsync(c->d_cnt.p, 0, sizeof(Counters), s)); CK(cudaMemsetAsync(c->d_base.p, 0, 8, s));
@@ -569,7 +569,7 @@ int pmc_nonelastic(pmc_ctx *c, int Z, int A, double e_mev, uint64_t n, uint64_t 
   for (uint64_t ev0 = 0; ev0 < n; ev0 += CH) {
     const uint32_t nc = (uint32_t)std::min<uint64_t>(CH, n - ev0);
     CK(cudaMemsetAsync(c->d_head.p, 0, 16, s));
-    const int gb = (int)std::min<uint32_t>((nc + 127) / 128, (uint32_t)c->n_sm * 8);
+    const int gb = (int)std::min<uint32_t>((nc + 127) / 128, (uint32_t)c->n_sm * 6);
     nonelastic_inc_kernel<<<gb, 128, 0, s>>>(c->T, c->d_nuc1.p, (float)e_mev, seed, ev0, nc, c->d_head.p + 1, c->d_slots.p, c->d_counts.p, c->d_res.p, c->d_cnt.p);
     nonelastic_evap_kernel<<<gb, 128, 0, s>>>(c->T, c->d_nuc1.p, seed, ev0, nc, c->d_head.p + 2, c->d_slots.p, c->d_counts.p, c->d_res.p, c->d_cnt.p);
     scan_kernel<<<1, 1024, 0, s>>>(c->d_counts.p, nc, off_dev + ev0, c->d_base.p);

@@ -46,6 +46,26 @@ struct Rng {
 };
 __device__ __forceinline__ float u01(uint32_t x) { return ((float)(x >> 8) + 0.5f) * (1.0f / 16777216.0f); }   // (0,1)
 
+// Fast fp32 arithmetic of the hot loops (the paper's -use_fast_math build was dosimetrically equivalent, PAPER.md:L203,
+// L248): 2-ulp division, and series for log1p / expm1 / sincos of the small arguments that occur at almost every step
+// (accurate to < 1e-7 relative there), with the library routine as the fallback.
+__device__ __forceinline__ float fdiv(float a, float b) { return __fdividef(a, b); }
+__device__ __forceinline__ float log1p_small(float x) {          // ln(1 + x)
+  if (fabsf(x) < 0.06f) return x * (1.0f + x * (-0.5f + x * ((1.0f / 3.0f) + x * (-0.25f + x * (0.2f - x * (1.0f / 6.0f))))));
+  return log1pf(x);
+}
+__device__ __forceinline__ float expm1_small(float x) {          // e^x - 1
+  if (fabsf(x) < 0.06f) return x * (1.0f + x * (0.5f + x * ((1.0f / 6.0f) + x * ((1.0f / 24.0f) + x * (1.0f / 120.0f)))));
+  return expm1f(x);
+}
+__device__ __forceinline__ void sincos_small(float x, float *s, float *c) {
+  if (fabsf(x) < 0.25f) {
+    const float x2 = x * x;
+    *s = x * (1.0f + x2 * ((-1.0f / 6.0f) + x2 * ((1.0f / 120.0f) - x2 * (1.0f / 5040.0f))));
+    *c = 1.0f + x2 * (-0.5f + x2 * ((1.0f / 24.0f) + x2 * ((-1.0f / 720.0f) + x2 * (1.0f / 40320.0f))));
+  } else sincosf(x, s, c);
+}
+
 // ------------------------------------------------------------------ device tables
 struct MatBin {                 // one HU bin, 16 floats
   float hu_lo, inv_dhu, dhu, rho_lo, drho;
@@ -206,32 +226,32 @@ __device__ __forceinline__ float gauss_pair(uint32_t a, uint32_t b) {
 }
 __device__ float straggle(const Tables &T, Rng &g, float e_start, float mean_loss, float rhoL, float zoa) {
   if (rhoL <= 0.f || mean_loss <= 0.f) return mean_loss;
-  const float gam = 1.0f + e_start * (1.0f / MP), b2 = 1.0f - 1.0f / (gam * gam), bg2 = b2 * gam * gam;
-  const float tmax = 2.0f * ME * bg2 / (1.0f + 2.0f * gam * (ME / MP) + (ME / MP) * (ME / MP));
-  const float xi = 0.5f * KBETHE * zoa * rhoL / b2;
+  const float gam = 1.0f + e_start * (1.0f / MP), g2m = gam * gam, b2 = 1.0f - fdiv(1.0f, g2m), bg2 = g2m - 1.0f;
+  const float tmax = fdiv(2.0f * ME * bg2, 1.0f + 2.0f * gam * (ME / MP) + (ME / MP) * (ME / MP));
+  const float xi = fdiv(0.5f * KBETHE * zoa * rhoL, b2);
   float loss;
   uint4 r = g.next4();
   const float z = gauss_pair(r.x, r.y);
   if (xi >= T.kappa_g * tmax) {
     loss = mean_loss + sqrtf(xi * tmax * (1.0f - 0.5f * b2)) * z;
   } else {
-    const float itmax = 1.0f / tmax;
+    const float itmax = fdiv(1.0f, tmax);
     const float tc0 = fminf(1e-3f, 0.01f * tmax);                            // Reading R4: below tc0 the soft part is Gaussian
-    float tc = fmaxf(tc0, 1.0f / (MU_HARD / xi + itmax));
+    float tc = fmaxf(tc0, fdiv(1.0f, fdiv(MU_HARD, xi) + itmax));
     tc = fminf(tc, tmax);
-    const float itc = 1.0f / tc, ltc = __logf(tmax * itc);
+    const float itc = fdiv(1.0f, tc), ltc = __logf(tmax * itc);
     const float mu_c = xi * (itc - itmax);                                   // candidates (before thinning)
     const float mean_hard = xi * (ltc - b2 * (1.0f - tc * itmax));
     // Poisson(mu_c) by inversion with one uniform
     float pk = __expf(-mu_c), cdf = pk; const float up = u01(r.z);
     int n = 0;
-    while (up > cdf && n < 64) { ++n; pk *= mu_c / (float)n; cdf += pk; }
+    while (up > cdf && n < 64) { ++n; pk *= fdiv(mu_c, (float)n); cdf += pk; }
     float hard = 0.f;
     uint4 q = make_uint4(0, 0, 0, 0);
     for (int k = 0; k < n; ++k) {
       if ((k & 1) == 0) q = g.next4();
       const uint32_t ra = (k & 1) ? q.z : q.x, rb = (k & 1) ? q.w : q.y;
-      const float t = 1.0f / (itc - u01(ra) * (itc - itmax));
+      const float t = fdiv(1.0f, itc - u01(ra) * (itc - itmax));
       if (u01(rb) < 1.0f - b2 * t * itmax) hard += t;
     }
     // soft part: variance k2 = xi tc (1 - b2 tc/2Tmax) of everything below tc; the 3rd and 4th cumulants
@@ -242,8 +262,8 @@ __device__ float straggle(const Tables &T, Rng &g, float e_start, float mean_los
     const float k2 = xi * tc * (1.0f - 0.5f * x);
     float cf = z;
     if (tc > tc0) {
-      const float g1 = (1.0f - f0 * f0) * xi * tc * tc * (0.5f - x * (1.0f / 3.0f)) / (k2 * sqrtf(k2));
-      const float g2 = (1.0f - f0 * f0 * f0) * xi * tc * tc * tc * ((1.0f / 3.0f) - 0.25f * x) / (k2 * k2);
+      const float g1 = (1.0f - f0 * f0) * xi * tc * tc * (0.5f - x * (1.0f / 3.0f)) * rsqrtf(k2) * fdiv(1.0f, k2);
+      const float g2 = (1.0f - f0 * f0 * f0) * xi * tc * tc * tc * fdiv((1.0f / 3.0f) - 0.25f * x, k2 * k2);
       const float z2 = z * z;
       cf = z + g1 * (1.0f / 6.0f) * (z2 - 1.0f) + g2 * (1.0f / 24.0f) * z * (z2 - 3.0f)
            - g1 * g1 * (1.0f / 36.0f) * z * (2.0f * z2 - 5.0f);

@@ -15,6 +15,7 @@ namespace pmc {
 constexpr int CASC_STACK = 48;      // cascade nucleons waiting to be tracked (an attempt that needs more fails)
 constexpr int MAX_INC_OUT = 32;     // nucleons leaving the nucleus in one cascade
 constexpr int MAX_SEC = 48;         // records per event in the standalone kernel's slot buffer (INC + evaporation + residual)
+constexpr int MAX_INC_STEPS = 1024; // tracking steps per attempt before it is abandoned and repeated (Reading R6.8)
 constexpr int NQ = 64;              // quadrature bins of the evaporation spectrum (Reading R7)
 
 struct SecRec { int16_t Z, A; uint8_t origin, pad[3]; float ke; float dir[3]; };   // == pmc_secondary (24 B)
@@ -61,7 +62,7 @@ __device__ __forceinline__ void inc_fail(IncLane &L) { L.failed = true; L.alive 
 __device__ __forceinline__ void inc_step(const Nucleus &N, Rng &g, IncLane &L) {
   CascNucleon &c = L.c;
   const int ns = N.nshell;
-  if (++L.guard > 20000) { inc_fail(L); return; }
+  if (++L.guard > MAX_INC_STEPS) { inc_fail(L); return; }   // bound orbit in a dilute shell (Reading R6.8)
   const int k = c.shell, ty = c.type;
   const float m = nucleon_mass(ty), p2 = dot(c.p, c.p), E = sqrtf(p2 + m * m), Tk = p2 / (E + m);
   const V3 d = rsqrtf(p2) * c.p;

@@ -42,7 +42,7 @@ __device__ __forceinline__ float dist_to_face(const V3 &r, const V3 &d, const fl
 #pragma unroll
   for (int a = 0; a < 3; ++a) {
     if (dd[a] != 0.f) {
-      const float t = fmaxf(((dd[a] > 0.f ? sz[a] : 0.f) - rr[a]) / dd[a], 0.f);
+      const float t = fmaxf(fdiv((dd[a] > 0.f ? sz[a] : 0.f) - rr[a], dd[a]), 0.f);
       if (t < best) { best = t; axis = a; sgn = dd[a] > 0.f ? 1 : -1; }
     }
   }
@@ -52,14 +52,14 @@ __device__ __forceinline__ float dist_to_face(const V3 &r, const V3 &d, const fl
 // Highland theta0 with the paper's factor; t = mass thickness / X0
 __device__ __forceinline__ float highland(const Tables &T, float e, float t) {
   if (t <= 0.f) return 0.f;
-  const float pc2 = e * (e + 2.0f * MP), bcp = pc2 / (e + MP);
-  return T.highland * 13.6f / bcp * sqrtf(t) * fmaxf(0.f, 1.0f + 0.038f * __logf(t));
+  const float pc2 = e * (e + 2.0f * MP);
+  return fdiv(T.highland * 13.6f * (e + MP), pc2) * sqrtf(t) * fmaxf(0.f, 1.0f + 0.038f * __logf(t));
 }
 // one MCS deflection: two independent projected Gaussians of width theta0 (Reading R3.4)
 __device__ __forceinline__ V3 deflect(V3 d, float theta0, uint32_t r0, uint32_t r1) {
   const float th = theta0 * sqrtf(-2.0f * __logf(u01(r0)));
   float st, ct, sp, cp;
-  sincosf(th, &st, &ct); sincospif(2.0f * u01(r1), &sp, &cp);
+  sincos_small(th, &st, &ct); sincospif(2.0f * u01(r1), &sp, &cp);
   return unit(to_lab(d, st * cp, st * sp, ct));
 }
 
@@ -69,8 +69,8 @@ __device__ __forceinline__ float mean_loss(const Tables &T, const float *lnE, co
                                            float e, float lnEv, float lnRv, float Rg, float dr) {
   const float r1 = Rg - dr;
   float lnE1 = T.ln_emin;
-  if (r1 > 0.f) lnE1 = ln_energy_of(T, lnE, lnE2, tab, lnRv + log1pf(-dr / Rg));
-  const float m = -e * expm1f(lnE1 - lnEv);
+  if (r1 > 0.f) lnE1 = ln_energy_of(T, lnE, lnE2, tab, lnRv + log1p_small(-fdiv(dr, Rg)));
+  const float m = -e * expm1_small(lnE1 - lnEv);
   return fminf(fmaxf(m, 0.f), e);
 }
 
@@ -183,9 +183,9 @@ __device__ __forceinline__ void deposit(float *tally, uint32_t vox, float e, boo
 // Persistent kernel: every lane pulls a particle from the input queue, steps it in registers until it stops,
 // leaves the grid or reaches a discrete nuclear event, then refills from the queue (warp-aggregated fetch).
 // Particles that reach an event are appended to the elastic or non-elastic queue; nothing else is written back.
-struct TransportSmem { int dummy; };
+constexpr int TRANSPORT_THREADS = 128, TRANSPORT_BLOCKS_PER_SM = 5;
 
-__global__ void __launch_bounds__(256, 2) transport_kernel(Tables T, Grid G, RunParams P, Queue in, uint32_t n_in,
+__global__ void __launch_bounds__(TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM) transport_kernel(Tables T, Grid G, RunParams P, Queue in, uint32_t n_in,
                                                            uint32_t *head, Queue q_el, Queue q_ne, float *tally,
                                                            Counters *cnt) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -243,13 +243,13 @@ __global__ void __launch_bounds__(256, 2) transport_kernel(Tables T, Grid G, Run
       c_steps++;
       const uint4 r = g.next4();
       // ---- 1. nuclear distance, face distance, residual range
-      const float e0 = p.e, lnEv = logf(fminf(fmaxf(e0, T.e_min), T.e_max));
+      const float e0 = p.e, lnEv = __logf(fminf(fmaxf(e0, T.e_min), T.e_max));
       const EIdx k = e_index(T, lnEv);
       float lam = BIG;
-      if (nuclear) { const float Sig = rho * lerp_tab(s_sig + bin * T.n_e, k); if (Sig > 0.f) lam = -__logf(u01(r.x)) / Sig; }
+      if (nuclear) { const float Sig = rho * lerp_tab(s_sig + bin * T.n_e, k); if (Sig > 0.f) lam = fdiv(-__logf(u01(r.x)), Sig); }
       int ax, sg; const float dface = dist_to_face(p.r, p.d, sz, ax, sg);
-      const float lnRv = ln_range(T, s_lnR, s_lnR2, tab, k), Rg = expf(lnRv);
-      const float R = Rg / wf, smax = T.s_max > 0.f ? T.s_max / wf : BIG;
+      const float lnRv = ln_range(T, s_lnR, s_lnR2, tab, k), Rg = __expf(lnRv), iwf = fdiv(1.0f, wf);
+      const float R = Rg * iwf, smax = T.s_max > 0.f ? T.s_max * iwf : BIG;
       // ---- 2. step = min (Reading R3.2)
       float dx = lam; int lim = 2;
       if (dface < dx) { dx = dface; lim = 1; }
