@@ -215,12 +215,15 @@ __device__ __forceinline__ void flush(unsigned long long *dst, unsigned long lon
 
 // ------------------------------------------------------------------ straggling (Reading R4)
 // Vavilov(kappa, beta^2) as its defining compound-Poisson process, shifted to the CSDA mean loss.  The collision
-// spectrum xi/T^2 (1 - beta^2 T/Tmax) is split at T_c: collisions above T_c are sampled one by one (Poisson
-// number by inversion, thinning for the (1 - beta^2 T/Tmax) factor); the many soft ones below T_c are replaced
-// by a Cornish-Fisher-corrected normal deviate carrying their exact 2nd, 3rd and 4th cumulants.  T_c is chosen
-// so that about MU_HARD hard collisions are expected (never below the oracle's own cut).  kappa >= kappa_G:
-// plain Gaussian of variance xi Tmax (1 - beta^2/2).
-constexpr float MU_HARD = 4.0f;
+// spectrum xi/T^2 (1 - beta^2 T/Tmax) is split at T_c: collisions above T_c are sampled one by one (Poisson number by
+// inversion, thinning for the (1 - beta^2 T/Tmax) factor).  Below T_c: the part under the oracle's own cut T_c0 is
+// Gaussian (Reading R4); the collisions in [T_c0, T_c] add skewness, and the sum of both is drawn as a shifted gamma
+// variate with the exact variance and third cumulant (its fourth cumulant, 3 k3^2 / 2 k2, is within 12 % of the
+// exact xi T_c^3 / 3), through the Wilson-Hilferty cube of one normal deviate - monotone, and the plain Gaussian in
+// the limit T_c -> T_c0.  T_c is chosen so that about MU_HARD hard collisions are expected, which keeps the lanes of
+// a warp in step (the shape parameter of the gamma is then >= 16).  kappa >= kappa_G: Gaussian, variance
+// xi Tmax (1 - beta^2/2).
+constexpr float MU_HARD = 1.0f;
 __device__ __forceinline__ float gauss_pair(uint32_t a, uint32_t b) {
   return sqrtf(-2.0f * __logf(u01(a))) * cospif(2.0f * u01(b));
 }
@@ -236,7 +239,7 @@ __device__ float straggle(const Tables &T, Rng &g, float e_start, float mean_los
     loss = mean_loss + sqrtf(xi * tmax * (1.0f - 0.5f * b2)) * z;
   } else {
     const float itmax = fdiv(1.0f, tmax);
-    const float tc0 = fminf(1e-3f, 0.01f * tmax);                            // Reading R4: below tc0 the soft part is Gaussian
+    const float tc0 = fminf(1e-3f, 0.01f * tmax);                            // Reading R4: Gaussian below tc0
     float tc = fmaxf(tc0, fdiv(1.0f, fdiv(MU_HARD, xi) + itmax));
     tc = fminf(tc, tmax);
     const float itc = fdiv(1.0f, tc), ltc = __logf(tmax * itc);
@@ -254,21 +257,17 @@ __device__ float straggle(const Tables &T, Rng &g, float e_start, float mean_los
       const float t = fdiv(1.0f, itc - u01(ra) * (itc - itmax));
       if (u01(rb) < 1.0f - b2 * t * itmax) hard += t;
     }
-    // soft part: variance k2 = xi tc (1 - b2 tc/2Tmax) of everything below tc; the 3rd and 4th cumulants
-    // k3 = xi (tc^2 - tc0^2)(1/2 - ..), k4 = xi (tc^3 - tc0^3)(1/3 - ..) only of the collisions in [tc0, tc] that were
-    // moved from the hard to the soft part, so that at tc = tc0 the sampler is the Gaussian of Reading R4 and the
-    // skewness never exceeds 1/4 (tc <= xi/MU_HARD), where the Cornish-Fisher expansion is monotone.
-    const float x = b2 * tc * itmax, f0 = tc0 * itc;
-    const float k2 = xi * tc * (1.0f - 0.5f * x);
-    float cf = z;
-    if (tc > tc0) {
-      const float g1 = (1.0f - f0 * f0) * xi * tc * tc * (0.5f - x * (1.0f / 3.0f)) * rsqrtf(k2) * fdiv(1.0f, k2);
-      const float g2 = (1.0f - f0 * f0 * f0) * xi * tc * tc * tc * fdiv((1.0f / 3.0f) - 0.25f * x, k2 * k2);
-      const float z2 = z * z;
-      cf = z + g1 * (1.0f / 6.0f) * (z2 - 1.0f) + g2 * (1.0f / 24.0f) * z * (z2 - 3.0f)
-           - g1 * g1 * (1.0f / 36.0f) * z * (2.0f * z2 - 5.0f);
+    // soft part: k2 = xi tc (1 - b2 tc/2Tmax) of everything below tc; k3 = xi [t^2 (1/2 - b2 t/3Tmax)] from tc0 to tc
+    const float x = b2 * tc * itmax, x0 = b2 * tc0 * itmax;
+    const float k2 = xi * tc * (1.0f - 0.5f * x), sd = sqrtf(k2);
+    const float k3 = xi * (tc * tc * (0.5f - x * (1.0f / 3.0f)) - tc0 * tc0 * (0.5f - x0 * (1.0f / 3.0f)));
+    float soft = sd * z;
+    if (tc > tc0 && k3 > 0.f) {
+      const float sa = fdiv(2.0f * k2 * sd, k3), isa = fdiv(1.0f, sa), c9 = isa * isa * (1.0f / 9.0f);   // sa = sqrt(shape)
+      const float e = fmaxf(z * isa * (1.0f / 3.0f) - c9, -1.0f);
+      soft = sd * sa * (e * (3.0f + e * (3.0f + e)) + c9 * c9 * c9);          // sqrt(k2 a) [(1 + e)^3 - E(1 + e)^3]
     }
-    loss = mean_loss + (hard - mean_hard) + sqrtf(k2) * cf;
+    loss = mean_loss + (hard - mean_hard) + soft;
   }
   return fminf(fmaxf(loss, 0.f), e_start);
 }
