@@ -49,14 +49,16 @@ __device__ __forceinline__ float u01(uint32_t x) { return ((float)(x >> 8) + 0.5
 // Fast fp32 arithmetic of the hot loops (the paper's -use_fast_math build was dosimetrically equivalent, PAPER.md:L203,
 // L248): 2-ulp division, and series for log1p / expm1 / sincos of the small arguments that occur at almost every step
 // (accurate to < 1e-7 relative there), with the library routine as the fallback.
-__device__ __forceinline__ float fdiv(float a, float b) { return __fdividef(a, b); }
+__device__ __forceinline__ float fdiv(float a, float b) {      // MUFU.RCP + FMUL
+  float q; asm("div.approx.ftz.f32 %0, %1, %2;" : "=f"(q) : "f"(a), "f"(b)); return q;
+}
 __device__ __forceinline__ float log1p_small(float x) {          // ln(1 + x)
   if (fabsf(x) < 0.06f) return x * (1.0f + x * (-0.5f + x * ((1.0f / 3.0f) + x * (-0.25f + x * (0.2f - x * (1.0f / 6.0f))))));
-  return log1pf(x);
+  return __logf(1.0f + x);                                      // |x| >= 0.06: relative error < 3e-6
 }
 __device__ __forceinline__ float expm1_small(float x) {          // e^x - 1
   if (fabsf(x) < 0.06f) return x * (1.0f + x * (0.5f + x * ((1.0f / 6.0f) + x * ((1.0f / 24.0f) + x * (1.0f / 120.0f)))));
-  return expm1f(x);
+  return __expf(x) - 1.0f;
 }
 __device__ __forceinline__ void sincos_small(float x, float *s, float *c) {
   if (fabsf(x) < 0.25f) {
