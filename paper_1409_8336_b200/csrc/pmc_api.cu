@@ -71,7 +71,7 @@ struct pmc_ctx {
   std::vector<int> ez, ea;
   double e_cut = 0.1, highland = 1.07, kappa_g = 10, s_max = 0.2; int n_batches = 10;
   bool opt_strag = true, opt_mcs = true, opt_el = true, opt_ne = true; int aggregate = 1; bool profile = true;
-  uint64_t chunk = 1u << 23, history_offset = 0;
+  uint64_t chunk = 1u << 24, history_offset = 0;
   std::vector<HostMat> mats;
   // device tables
   DevBuf<float> d_lnR, d_lnR2, d_lnE, d_lnE2, d_sel, d_sne, d_sigbin, d_ek, d_ec;

@@ -218,7 +218,7 @@ __device__ __forceinline__ void flush(unsigned long long *dst, unsigned long lon
 // ------------------------------------------------------------------ straggling (Reading R4)
 // Vavilov(kappa, beta^2) as its defining compound-Poisson process, shifted to the CSDA mean loss.  The collision
 // spectrum xi/T^2 (1 - beta^2 T/Tmax) is split at T_c: collisions above T_c are sampled one by one (Poisson number by
-// inversion, thinning for the (1 - beta^2 T/Tmax) factor).  Below T_c: the part under the oracle's own cut T_c0 is
+// inversion, thinning for the (1 - beta^2 T/Tmax) factor; one random word per collision).  Below T_c: the part under the oracle's own cut T_c0 is
 // Gaussian (Reading R4); the collisions in [T_c0, T_c] add skewness, and the sum of both is drawn as a shifted gamma
 // variate with the exact variance and third cumulant (its fourth cumulant, 3 k3^2 / 2 k2, is within 12 % of the
 // exact xi T_c^3 / 3), through the Wilson-Hilferty cube of one normal deviate - monotone, and the plain Gaussian in
@@ -251,13 +251,17 @@ __device__ float straggle(const Tables &T, Rng &g, float e_start, float mean_los
     float pk = __expf(-mu_c), cdf = pk; const float up = u01(r.z);
     int n = 0;
     while (up > cdf && n < 64) { ++n; pk *= fdiv(mu_c, (float)n); cdf += pk; }
+    // one 32-bit word per candidate: 20 bits place it on the 1/T^2 spectrum, the other 12 decide the thinning;
+    // candidate 0 uses the last word of r, the next four one more block
     float hard = 0.f;
     uint4 q = make_uint4(0, 0, 0, 0);
     for (int k = 0; k < n; ++k) {
-      if ((k & 1) == 0) q = g.next4();
-      const uint32_t ra = (k & 1) ? q.z : q.x, rb = (k & 1) ? q.w : q.y;
-      const float t = fdiv(1.0f, itc - u01(ra) * (itc - itmax));
-      if (u01(rb) < 1.0f - b2 * t * itmax) hard += t;
+      if (((k - 1) & 3) == 0) q = g.next4();
+      const int j = (k - 1) & 3;
+      const uint32_t w = k == 0 ? r.w : (j == 0 ? q.x : j == 1 ? q.y : j == 2 ? q.z : q.w);
+      const float ut = ((float)(w >> 12) + 0.5f) * (1.0f / 1048576.0f), ua = ((float)(w & 0xFFFu) + 0.5f) * (1.0f / 4096.0f);
+      const float t = fdiv(1.0f, itc - ut * (itc - itmax));
+      if (ua < 1.0f - b2 * t * itmax) hard += t;
     }
     // soft part: k2 = xi tc (1 - b2 tc/2Tmax) of everything below tc; k3 = xi [t^2 (1/2 - b2 t/3Tmax)] from tc0 to tc
     const float x = b2 * tc * itmax, x0 = b2 * tc0 * itmax;
