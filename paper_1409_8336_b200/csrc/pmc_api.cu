@@ -504,6 +504,7 @@ static int simulate_impl(pmc_ctx *c, const pmc_spot *spots_in, int nspots, uint6
     const uint32_t nc = (uint32_t)std::min<uint64_t>(chunk, n - cs);
     RunParams P{}; P.seed = seed; P.hist0 = c->history_offset + cs; P.n = nc; P.max_steps = max_steps; P.dbg_out = dbg_out ? dbg_out + 8ull * cs : nullptr;
     P.aggregate = c->aggregate; P.local0 = cs; P.n_total = n; P.B = (uint32_t)B; P.nvox = nvox;
+    P.b_over_n = (float)((double)B / (double)n); P.inv_nx = 1.0f / (float)c->G.nx; P.inv_ny = 1.0f / (float)c->G.ny;
     CK(cudaMemsetAsync(c->qa.q.count, 0, 4, s));
     { Timer t(c, &c->timing.sampler_ms, profile);
       sampler_kernel<<<(nc + 255) / 256, 256, 0, s>>>(c->T, c->G, c->d_spots.p, c->d_cdf.p, nspots, P, c->qa.q, c->d_cnt.p, air_rho, air_wf, air_ix0, air_zoa, air_tab); }

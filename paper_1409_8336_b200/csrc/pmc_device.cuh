@@ -52,6 +52,9 @@ __device__ __forceinline__ float u01(uint32_t x) { return ((float)(x >> 8) + 0.5
 __device__ __forceinline__ float fdiv(float a, float b) {      // MUFU.RCP + FMUL
   float q; asm("div.approx.ftz.f32 %0, %1, %2;" : "=f"(q) : "f"(a), "f"(b)); return q;
 }
+__device__ __forceinline__ float fsqrt(float a) { float q; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(q) : "f"(a)); return q; }
+// sin and cos of 2 pi u, u in (0,1): MUFU.SIN/COS (absolute error ~5e-7), for azimuths and Box-Muller
+__device__ __forceinline__ void sincos_2pi(float u, float *s, float *c) { const float x = TWO_PI * u - 3.14159265358979f; *s = -__sinf(x); *c = -__cosf(x); }
 __device__ __forceinline__ float log1p_small(float x) {          // ln(1 + x)
   if (fabsf(x) < 0.06f) return x * (1.0f + x * (-0.5f + x * ((1.0f / 3.0f) + x * (-0.25f + x * (0.2f - x * (1.0f / 6.0f))))));
   return __logf(1.0f + x);                                      // |x| >= 0.06: relative error < 3e-6
@@ -227,7 +230,7 @@ __device__ __forceinline__ void flush(unsigned long long *dst, unsigned long lon
 // xi Tmax (1 - beta^2/2).
 constexpr float MU_HARD = 1.0f;
 __device__ __forceinline__ float gauss_pair(uint32_t a, uint32_t b) {
-  return sqrtf(-2.0f * __logf(u01(a))) * cospif(2.0f * u01(b));
+  return fsqrt(-2.0f * __logf(u01(a))) * -__cosf(TWO_PI * u01(b) - 3.14159265358979f);
 }
 __device__ float straggle(const Tables &T, Rng &g, float e_start, float mean_loss, float rhoL, float zoa) {
   if (rhoL <= 0.f || mean_loss <= 0.f) return mean_loss;
@@ -238,7 +241,7 @@ __device__ float straggle(const Tables &T, Rng &g, float e_start, float mean_los
   uint4 r = g.next4();
   const float z = gauss_pair(r.x, r.y);
   if (xi >= T.kappa_g * tmax) {
-    loss = mean_loss + sqrtf(xi * tmax * (1.0f - 0.5f * b2)) * z;
+    loss = mean_loss + fsqrt(xi * tmax * (1.0f - 0.5f * b2)) * z;
   } else {
     const float itmax = fdiv(1.0f, tmax);
     const float tc0 = fminf(1e-3f, 0.01f * tmax);                            // Reading R4: Gaussian below tc0
@@ -247,25 +250,24 @@ __device__ float straggle(const Tables &T, Rng &g, float e_start, float mean_los
     const float itc = fdiv(1.0f, tc), ltc = __logf(tmax * itc);
     const float mu_c = xi * (itc - itmax);                                   // candidates (before thinning)
     const float mean_hard = xi * (ltc - b2 * (1.0f - tc * itmax));
-    // Poisson(mu_c) by inversion with one uniform
+    // Poisson(mu_c) number of candidates by inversion with one uniform, each candidate handled as soon as the
+    // inversion shows it exists.  One 32-bit word per candidate: 20 bits place it on the 1/T^2 spectrum, the other
+    // 12 decide the thinning; candidate 0 uses the last word of r, the next four one more block, ...
     float pk = __expf(-mu_c), cdf = pk; const float up = u01(r.z);
-    int n = 0;
-    while (up > cdf && n < 64) { ++n; pk *= fdiv(mu_c, (float)n); cdf += pk; }
-    // one 32-bit word per candidate: 20 bits place it on the 1/T^2 spectrum, the other 12 decide the thinning;
-    // candidate 0 uses the last word of r, the next four one more block
     float hard = 0.f;
-    uint4 q = make_uint4(0, 0, 0, 0);
-    for (int k = 0; k < n; ++k) {
-      if (((k - 1) & 3) == 0) q = g.next4();
-      const int j = (k - 1) & 3;
-      const uint32_t w = k == 0 ? r.w : (j == 0 ? q.x : j == 1 ? q.y : j == 2 ? q.z : q.w);
+    uint4 q = make_uint4(r.w, 0u, 0u, 0u);
+    int k = 0, avail = 1;
+    while (up > cdf && k < 64) {
+      if (avail == 0) { q = g.next4(); avail = 4; }
+      const uint32_t w = q.x; q.x = q.y; q.y = q.z; q.z = q.w; --avail;
       const float ut = ((float)(w >> 12) + 0.5f) * (1.0f / 1048576.0f), ua = ((float)(w & 0xFFFu) + 0.5f) * (1.0f / 4096.0f);
       const float t = fdiv(1.0f, itc - ut * (itc - itmax));
       if (ua < 1.0f - b2 * t * itmax) hard += t;
+      ++k; pk *= fdiv(mu_c, (float)k); cdf += pk;
     }
     // soft part: k2 = xi tc (1 - b2 tc/2Tmax) of everything below tc; k3 = xi [t^2 (1/2 - b2 t/3Tmax)] from tc0 to tc
     const float x = b2 * tc * itmax, x0 = b2 * tc0 * itmax;
-    const float k2 = xi * tc * (1.0f - 0.5f * x), sd = sqrtf(k2);
+    const float k2 = xi * tc * (1.0f - 0.5f * x), sd = fsqrt(k2);
     const float k3 = xi * (tc * tc * (0.5f - x * (1.0f / 3.0f)) - tc0 * tc0 * (0.5f - x0 * (1.0f / 3.0f)));
     float soft = sd * z;
     if (tc > tc0 && k3 > 0.f) {

@@ -17,12 +17,24 @@ struct RunParams {
   // history h (0-based within the call) belongs to batch floor(h B / n_total); tally of batch b starts at b * nvox.
   uint64_t local0, n_total;           // call-local index of this launch's first history; histories in the call
   uint32_t B, nvox;
+  float b_over_n, inv_nx, inv_ny;     // B / n_total, 1 / nx, 1 / ny
   int max_steps; float *dbg_out;      // pmc_first_steps: stop after max_steps, write [hist][8]
   int aggregate;                      // warp-aggregated dose atomics
 };
 
+// floor(h B / n_total) * nvox without a 64-bit division: float estimate, exact correction
 __device__ __forceinline__ uint32_t batch_base(const RunParams &P, uint32_t hist) {
-  return (uint32_t)(((P.local0 + hist) * (uint64_t)P.B) / P.n_total) * P.nvox;
+  const uint64_t h = P.local0 + hist, hb = h * (uint64_t)P.B;
+  uint32_t b = min((uint32_t)((float)h * P.b_over_n), P.B - 1u);
+  while ((uint64_t)b * P.n_total > hb) --b;
+  while ((uint64_t)(b + 1u) * P.n_total <= hb) ++b;
+  return b * P.nvox;
+}
+// q = a / d, r = a % d for 0 <= a < 2^31, d >= 1 (float estimate, exact correction)
+__device__ __forceinline__ void divmod(int a, int d, float inv_d, int &q, int &r) {
+  q = (int)((float)a * inv_d); r = a - q * d;
+  while (r < 0) { --q; r += d; }
+  while (r >= d) { ++q; r -= d; }
 }
 
 // ------------------------------------------------------------------ material of a voxel
@@ -53,13 +65,13 @@ __device__ __forceinline__ float dist_to_face(const V3 &r, const V3 &d, const fl
 __device__ __forceinline__ float highland(const Tables &T, float e, float t) {
   if (t <= 0.f) return 0.f;
   const float pc2 = e * (e + 2.0f * MP);
-  return fdiv(T.highland * 13.6f * (e + MP), pc2) * sqrtf(t) * fmaxf(0.f, 1.0f + 0.038f * __logf(t));
+  return fdiv(T.highland * 13.6f * (e + MP), pc2) * fsqrt(t) * fmaxf(0.f, 1.0f + 0.038f * __logf(t));
 }
 // one MCS deflection: two independent projected Gaussians of width theta0 (Reading R3.4)
 __device__ __forceinline__ V3 deflect(V3 d, float theta0, uint32_t r0, uint32_t r1) {
-  const float th = theta0 * sqrtf(-2.0f * __logf(u01(r0)));
+  const float th = theta0 * fsqrt(-2.0f * __logf(u01(r0)));
   float st, ct, sp, cp;
-  sincos_small(th, &st, &ct); sincospif(2.0f * u01(r1), &sp, &cp);
+  sincos_small(th, &st, &ct); sincos_2pi(u01(r1), &sp, &cp);
   return unit(to_lab(d, st * cp, st * sp, ct));
 }
 
@@ -225,7 +237,7 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM) tr
         if (idx < n_in) {
           p = queue_load(in, idx);
           g.init(P.seed, P.hist0 + p.hist, p.pid, p.blk);
-          ix = p.vox % G.nx; const int t = p.vox / G.nx; iy = t % G.ny; iz = t / G.ny;
+          int t; divmod(p.vox, G.nx, P.inv_nx, t, ix); divmod(t, G.ny, P.inv_ny, iz, iy);
           active = true; nstep = 0; path = 0.f; tbase = batch_base(P, p.hist);
         } else exhausted = true;
       }
