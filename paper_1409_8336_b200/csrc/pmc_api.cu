@@ -80,7 +80,7 @@ struct pmc_ctx {
   Tables T{}; Grid G{}; double origin[3] = {0, 0, 0};
   DevBuf<int16_t> d_hu_own;
   // scratch
-  QueueMem qa, qb, qel, qne, qres; DevBuf<uint32_t> d_resza; DevBuf<float> d_resp;
+  QueueMem qa, qb, qev, qel, qne, qres; DevBuf<uint32_t> d_resza; DevBuf<float> d_resp;
   DevBuf<uint32_t> d_head; DevBuf<Counters> d_cnt; DevBuf<float> d_tally, d_out;
   DevBuf<SpotDev> d_spots; DevBuf<double> d_cdf;
   DevBuf<SecRec> d_slots; DevBuf<uint32_t> d_counts; DevBuf<unsigned long long> d_base; DevBuf<ResRec> d_res;
@@ -204,7 +204,7 @@ int sync_tables(pmc_ctx *c) {
 int ensure_scratch(pmc_ctx *c, uint64_t chunk) {
   const uint32_t cap = (uint32_t)std::max<uint64_t>(chunk + chunk / 4 + 4096, 8192);
   if (cap > c->qcap) {
-    CK(c->qa.alloc(cap)); CK(c->qb.alloc(cap)); CK(c->qel.alloc(cap)); CK(c->qne.alloc(cap)); CK(c->qres.alloc(cap));
+    CK(c->qa.alloc(cap)); CK(c->qb.alloc(cap)); CK(c->qev.alloc(cap)); CK(c->qel.alloc(cap)); CK(c->qne.alloc(cap)); CK(c->qres.alloc(cap));
     CK(c->d_resza.alloc(cap)); CK(c->d_resp.alloc((size_t)cap * 3));
     c->qcap = cap;
   }
@@ -278,17 +278,19 @@ int run_generations(pmc_ctx *c, RunParams P, uint32_t n0, bool profile) {
     c->counters.n_generations++;
     CK(cudaMemsetAsync(c->d_head.p, 0, 16, s)); CK(cudaMemsetAsync(nxt->q.count, 0, 4, s));
     CK(cudaMemsetAsync(c->qel.q.count, 0, 4, s)); CK(cudaMemsetAsync(c->qne.q.count, 0, 4, s)); CK(cudaMemsetAsync(c->qres.q.count, 0, 4, s));
+    CK(cudaMemsetAsync(c->qev.q.count, 0, 4, s));
     { Timer t(c, &c->timing.transport_ms, profile);
-      transport_kernel<<<grid_t, TRANSPORT_THREADS, c->smem_transport, s>>>(c->T, c->G, P, cur->q, n_in, c->d_head.p, c->qel.q, c->qne.q, c->d_tally.p, c->d_cnt.p); }
+      transport_kernel<<<grid_t, TRANSPORT_THREADS, c->smem_transport, s>>>(c->T, c->G, P, cur->q, n_in, c->d_head.p, c->qev.q, c->d_tally.p, c->d_cnt.p); }
     c->timing.launches_total++; c->timing.launches_transport++;
     if (P.dbg_out) break;
     { Timer t(c, &c->timing.elastic_ms, profile);
+      event_kernel<<<grid_e, 256, 0, s>>>(c->T, c->G, P, c->qev.q, c->qel.q, c->qne.q, nxt->q, c->d_cnt.p);
       elastic_kernel<<<grid_e, 256, 0, s>>>(c->T, P, c->qel.q, nxt->q, c->d_tally.p, c->d_cnt.p); }
     { Timer t(c, &c->timing.inc_ms, profile);
       inc_kernel<<<c->n_sm * 6, 128, 0, s>>>(c->T, P, c->qne.q, c->d_head.p + 1, nxt->q, rq, c->d_tally.p, c->d_cnt.p); }
     { Timer t(c, &c->timing.evaporation_ms, profile);
       evap_kernel<<<c->n_sm * 8, 128, 0, s>>>(c->T, P, rq, c->d_head.p + 2, nxt->q, c->d_tally.p, c->d_cnt.p); }
-    c->timing.launches_total += 3;
+    c->timing.launches_total += 4;
     CK(cudaMemcpyAsync(c->h_pinned, nxt->q.count, 4, cudaMemcpyDeviceToHost, s));
     CK(cudaStreamSynchronize(s));
     n_in = c->h_pinned[0];
@@ -356,7 +358,7 @@ void pmc_destroy(pmc_ctx *c) {
   c->d_lnR.release(); c->d_lnR2.release(); c->d_lnE.release(); c->d_lnE2.release(); c->d_sel.release(); c->d_sne.release();
   c->d_sigbin.release(); c->d_ek.release(); c->d_ec.release(); c->d_mass.release(); c->d_bins.release(); c->d_lut.release();
   c->d_nuc.release(); c->d_nuc1.release(); c->d_hu_own.release();
-  c->qa.release(); c->qb.release(); c->qel.release(); c->qne.release(); c->qres.release(); c->d_resza.release(); c->d_resp.release();
+  c->qa.release(); c->qb.release(); c->qev.release(); c->qel.release(); c->qne.release(); c->qres.release(); c->d_resza.release(); c->d_resp.release();
   c->d_head.release(); c->d_cnt.release(); c->d_tally.release(); c->d_out.release();
   c->d_spots.release(); c->d_cdf.release(); c->d_res.release(); c->d_slots.release(); c->d_counts.release(); c->d_base.release();
   if (c->h_pinned) cudaFreeHost(c->h_pinned);

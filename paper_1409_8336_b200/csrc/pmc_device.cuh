@@ -151,8 +151,8 @@ __device__ __forceinline__ V3 to_lab(V3 d, float a, float b, float c) {
   return {a * d.x * d.z * is - b * d.y * is + c * d.x, a * d.y * d.z * is + b * d.x * is + c * d.y, -a * s + c * d.z};
 }
 __device__ __forceinline__ V3 isotropic(uint32_t r0, uint32_t r1) {
-  const float c = 2.0f * u01(r0) - 1.0f, s = sqrtf(fmaxf(0.f, 1.0f - c * c));
-  float sp, cp; sincospif(2.0f * u01(r1), &sp, &cp);
+  const float c = 2.0f * u01(r0) - 1.0f, s = fsqrt(fmaxf(0.f, 1.0f - c * c));
+  float sp, cp; sincos_2pi(u01(r1), &sp, &cp);
   return {s * cp, s * sp, c};
 }
 // Lorentz transformation of (p,E) from a frame moving with velocity beta

@@ -64,7 +64,7 @@ __device__ __forceinline__ void inc_step(const Nucleus &N, Rng &g, IncLane &L) {
   const int ns = N.nshell;
   if (++L.guard > MAX_INC_STEPS) { inc_fail(L); return; }   // bound orbit in a dilute shell (Reading R6.8)
   const int k = c.shell, ty = c.type;
-  const float m = nucleon_mass(ty), p2 = dot(c.p, c.p), E = sqrtf(p2 + m * m), Tk = p2 / (E + m);
+  const float m = nucleon_mass(ty), p2 = dot(c.p, c.p), E = fsqrt(p2 + m * m), Tk = fdiv(p2, E + m);
   const V3 d = rsqrtf(p2) * c.p;
   // candidate collisions with a proton and with a neutron of the Fermi sea (Reading R6.3)
   float dbest = BIG, plab_best = 0.f; int tbest = -1; V3 qbest{0.f, 0.f, 0.f};
@@ -72,38 +72,38 @@ __device__ __forceinline__ void inc_step(const Nucleus &N, Rng &g, IncLane &L) {
   for (int tp = 0; tp < 2; ++tp) {
     if (N.rho[tp][k] <= 0.f) continue;
     const uint4 r = g.next4();
-    const float mq = nucleon_mass(tp), qmag = N.pF[tp][k] * cbrtf(u01(r.x));
+    const float mq = nucleon_mass(tp), qmag = N.pF[tp][k] * __powf(u01(r.x), 1.0f / 3.0f);
     const V3 q = qmag * isotropic(r.y, r.z);
-    const float Eq = sqrtf(qmag * qmag + mq * mq);
-    const float e1 = (E * Eq - dot(c.p, q)) / mq;                       // projectile energy in the partner rest frame
-    const float plab = sqrtf(fmaxf(e1 * e1 - m * m, 0.f));
+    const float Eq = fsqrt(qmag * qmag + mq * mq);
+    const float e1 = (E * Eq - dot(c.p, q)) * (tp == 0 ? 1.0f / MP : 1.0f / MN);                       // projectile energy in the partner rest frame
+    const float plab = fsqrt(fmaxf(e1 * e1 - m * m, 0.f));
     const float sig = N.const_sigma_mb >= 0.f ? N.const_sigma_mb
                                               : (tp == ty ? cug_sigma_pp(plab * 1e-3f) : cug_sigma_np(plab * 1e-3f));
-    const float dist = -__logf(u01(r.w)) / (N.rho[tp][k] * sig * 0.1f);  // 1 mb = 0.1 fm^2
+    const float dist = fdiv(-__logf(u01(r.w)), N.rho[tp][k] * sig * 0.1f);  // 1 mb = 0.1 fm^2
     if (dist < dbest) { dbest = dist; tbest = tp; qbest = q; plab_best = plab; }
   }
   // distance to the shell boundaries along d
   const float rr = dot(c.r, c.r), bq = dot(c.r, d), r_out = N.rout[k], r_in = k > 0 ? N.rout[k - 1] : 0.f;
-  float dbound = -bq + sqrtf(fmaxf(bq * bq - (rr - r_out * r_out), 0.f)); bool inward = false;
+  float dbound = -bq + fsqrt(fmaxf(bq * bq - (rr - r_out * r_out), 0.f)); bool inward = false;
   if (k > 0 && bq < 0.f) {
     const float disc = bq * bq - (rr - r_in * r_in);
-    if (disc > 0.f) { const float s_in = -bq - sqrtf(disc); if (s_in < dbound) { dbound = fmaxf(s_in, 0.f); inward = true; } }
+    if (disc > 0.f) { const float s_in = -bq - fsqrt(disc); if (s_in < dbound) { dbound = fmaxf(s_in, 0.f); inward = true; } }
   }
   if (dbest < dbound) {
     // ---- collision attempt (Reading R6.4)
     c.r = c.r + dbest * d;
     const int tp = tbest; const float mq = nucleon_mass(tp);
-    const V3 q = qbest; const float Eq = sqrtf(dot(q, q) + mq * mq);
-    const V3 Pt = c.p + q; const float Et = E + Eq; const V3 beta = (1.0f / Et) * Pt;
+    const V3 q = qbest; const float Eq = fsqrt(dot(q, q) + mq * mq);
+    const V3 Pt = c.p + q; const float Et = E + Eq; const V3 beta = fdiv(1.0f, Et) * Pt;
     const float s = Et * Et - dot(Pt, Pt);
-    const float pcm = sqrtf(fmaxf((s - (m + mq) * (m + mq)) * (s - (m - mq) * (m - mq)), 0.f) / (4.0f * s));
+    const float pcm = fsqrt(fmaxf((s - (m + mq) * (m + mq)) * (s - (m - mq) * (m - mq)), 0.f) * fdiv(0.25f, s));
     V3 p1 = c.p; float E1 = E; boost(-1.0f * beta, p1, E1);             // projectile in the CM
     const V3 ax = unit(p1);
     const uint4 r = g.next4();
-    const float ct = sample_nn_cos(tp == ty, plab_best * 1e-3f, pcm, r.x, r.y), st = sqrtf(fmaxf(0.f, 1.0f - ct * ct));
-    float sph, cph; sincospif(2.0f * u01(r.z), &sph, &cph);
+    const float ct = sample_nn_cos(tp == ty, plab_best * 1e-3f, pcm, r.x, r.y), st = fsqrt(fmaxf(0.f, 1.0f - ct * ct));
+    float sph, cph; sincos_2pi(u01(r.z), &sph, &cph);
     V3 n1 = pcm * to_lab(ax, st * cph, st * sph, ct), n2 = -1.0f * n1;
-    float En1 = sqrtf(pcm * pcm + m * m), En2 = sqrtf(pcm * pcm + mq * mq);
+    float En1 = fsqrt(pcm * pcm + m * m), En2 = fsqrt(pcm * pcm + mq * mq);
     boost(beta, n1, En1); boost(beta, n2, En2);
     const float T1 = En1 - m, T2 = En2 - mq;
     const bool ok = !N.pauli || (T1 > N.EF[ty][k] && T2 > N.EF[tp][k]);  // L77 Pauli blocking
@@ -122,13 +122,13 @@ __device__ __forceinline__ void inc_step(const Nucleus &N, Rng &g, IncLane &L) {
   c.r = c.r + dbound * d;
   const float rb = inward ? r_in : r_out;
   c.r = (rb * rsqrtf(dot(c.r, c.r))) * c.r;
-  const V3 nh = (1.0f / rb) * c.r;
+  const V3 nh = fdiv(1.0f, rb) * c.r;
   const float pr = dot(c.p, nh); const V3 pt = c.p - pr * nh;
   const int k2 = inward ? k - 1 : k + 1;
   const float Vnew = k2 >= ns ? 0.f : N.V[ty][k2], T2 = Tk + (Vnew - N.V[ty][k]);
   const float pn2 = T2 > 0.f ? T2 * (T2 + 2.0f * m) : -1.0f, pr2 = pn2 - dot(pt, pt);
   if (pn2 <= 0.f || pr2 <= 0.f) { c.p = pt - pr * nh; return; }           // specular reflection
-  const V3 pnew = pt + ((pr > 0.f ? 1.0f : -1.0f) * sqrtf(pr2)) * nh;
+  const V3 pnew = pt + ((pr > 0.f ? 1.0f : -1.0f) * fsqrt(pr2)) * nh;
   if (k2 >= ns) {                                                       // leaves the nucleus with KE = eps
     if (L.n_out >= MAX_INC_OUT) { inc_fail(L); return; }
     OutNuc &o = L.out[L.n_out++];
@@ -170,35 +170,49 @@ __device__ __forceinline__ void inc_compound(const Tables &T, const Nucleus &N, 
 template <class Load, class Store>
 __device__ __forceinline__ void inc_machine(const Tables &T, uint32_t n, uint32_t *head, unsigned long long &tries,
                                             Load load, Store store) {
+  // Lane states.  STEP: tracking a nucleon.  WAIT: attempt finished (needs finalize, then store + next event, or a
+  // fresh attempt) or no event yet.  DONE: queue exhausted.  The turnover work of WAIT lanes is divergent and long
+  // compared with one step, so it is batched: it runs when TURNOVER lanes are waiting (or nobody can step), not
+  // every time a single lane finishes.
+  enum { STEP = 0, WAIT = 1, DONE = 2 };
+  constexpr int TURNOVER = 8;
   IncLane L; L.alive = false; L.sp = 0; L.failed = false;
   const Nucleus *N = nullptr; float t_in = 0.f; Rng g; uint32_t ev = 0; int ntry = 0;
-  bool busy = false, exhausted = false;
+  bool busy = false; int state = WAIT;
   const int lane = threadIdx.x & 31;
   while (true) {
-    const unsigned need = __ballot_sync(0xffffffffu, !busy && !exhausted);
-    if (need) {
-      const int leader = __ffs(need) - 1;
-      uint32_t base = 0;
-      if (lane == leader) base = atomicAdd(head, (uint32_t)__popc(need));
-      base = __shfl_sync(0xffffffffu, base, leader);
-      if (!busy && !exhausted) {
-        ev = base + (uint32_t)__popc(need & ((1u << lane) - 1u));
-        if (ev < n) { load(ev, N, t_in, g); busy = true; ntry = 1; tries++; inc_begin(*N, t_in, g, L); }
-        else exhausted = true;
-      }
-    }
-    if (!__any_sync(0xffffffffu, busy)) break;
-    if (busy && !L.alive) {
-      if (L.sp > 0) { L.c = L.stack[--L.sp]; L.alive = true; }
-      else {
+    const unsigned waiting = __ballot_sync(0xffffffffu, state == WAIT), stepping = __ballot_sync(0xffffffffu, state == STEP);
+    if (!waiting && !stepping) break;
+    if (waiting && (__popc(waiting) >= TURNOVER || !stepping)) {
+      if (state == WAIT && busy) {                       // end of an attempt
         Residual R;
         if (inc_finalize(T, *N, t_in, L, R)) { store(ev, g, L.out, L.n_out, R); busy = false; }
         else if (ntry >= 100000) { inc_compound(T, *N, t_in, R); store(ev, g, L.out, 0, R); busy = false; }
-        else { ++ntry; tries++; inc_begin(*N, t_in, g, L); }
+        else { ++ntry; tries++; inc_begin(*N, t_in, g, L); state = STEP; }
+      }
+      __syncwarp();
+      const unsigned need = __ballot_sync(0xffffffffu, state == WAIT && !busy);
+      if (need) {                                        // next events, warp-aggregated fetch
+        const int leader = __ffs(need) - 1;
+        uint32_t base = 0;
+        if (lane == leader) base = atomicAdd(head, (uint32_t)__popc(need));
+        base = __shfl_sync(0xffffffffu, base, leader);
+        if (state == WAIT && !busy) {
+          ev = base + (uint32_t)__popc(need & ((1u << lane) - 1u));
+          if (ev < n) { load(ev, N, t_in, g); busy = true; ntry = 1; tries++; inc_begin(*N, t_in, g, L); state = STEP; }
+          else state = DONE;
+        }
+      }
+      __syncwarp();
+    }
+    if (state == STEP) {
+      inc_step(*N, g, L);
+      if (!L.alive) {
+        if (L.sp > 0) { L.c = L.stack[--L.sp]; L.alive = true; }
+        else state = WAIT;
       }
     }
     __syncwarp();
-    if (busy && L.alive) inc_step(*N, g, L);
   }
 }
 

@@ -198,8 +198,7 @@ __device__ __forceinline__ void deposit(float *tally, uint32_t vox, float e, boo
 constexpr int TRANSPORT_THREADS = 256, TRANSPORT_BLOCKS_PER_SM = 3;
 
 __global__ void __launch_bounds__(TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM) transport_kernel(Tables T, Grid G, RunParams P, Queue in, uint32_t n_in,
-                                                           uint32_t *head, Queue q_el, Queue q_ne, float *tally,
-                                                           Counters *cnt) {
+                                                           uint32_t *head, Queue q_ev, float *tally, Counters *cnt) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   // shared-memory staging of the stopping-power/range and cross-section tables (PAPER.md:L144 used textures)
   float *s_lnR = reinterpret_cast<float *>(smem_raw);
@@ -221,7 +220,7 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM) tr
   const int lane = threadIdx.x & 31;
   bool active = false, exhausted = false;
   Particle p; Rng g; int ix = 0, iy = 0, iz = 0, nstep = 0; float path = 0.f; uint32_t tbase = 0;
-  unsigned long long c_steps = 0, c_el = 0, c_ne = 0;
+  unsigned long long c_steps = 0, c_ev = 0;
   double c_dep = 0, c_esc = 0;
   const bool nuclear = T.opt_el || T.opt_ne;
 
@@ -302,36 +301,12 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM) tr
         else p.vox = (iz * G.ny + iy) * G.nx + ix;
       }
       ++nstep;
-      if (alive && cls == 2) {
-        // ---- 8. discrete nuclear event at the end point (L71, L75; Reading R5): class, then target element
-        const float lnE1 = logf(fminf(fmaxf(p.e, T.e_min), T.e_max));
-        const EIdx k1 = e_index(T, lnE1);
-        float pel[MAX_ELEM], pne[MAX_ELEM], sel = 0.f, sne = 0.f;
-#pragma unroll
-        for (int i = 0; i < MAX_ELEM; ++i) {
-          pel[i] = 0.f; pne[i] = 0.f;
-          if (i < T.n_elem && m.nfac[i] > 0.f) {
-            if (T.opt_el) pel[i] = m.nfac[i] * lerp_tab(T.sig_el + i * T.n_e, k1);
-            if (T.opt_ne) pne[i] = m.nfac[i] * lerp_tab(T.sig_ne + i * T.n_e, k1);
-          }
-          sel += pel[i]; sne += pne[i];
-        }
-        if (sel + sne > 0.f) {
-          const uint4 q = g.next4();
-          const bool is_el = u01(q.x) * (sel + sne) < sel;
-          float u = u01(q.y) * (is_el ? sel : sne); int el = -1;
-#pragma unroll
-          for (int i = 0; i < MAX_ELEM; ++i) {
-            const float w = is_el ? pel[i] : pne[i];
-            if (w > 0.f && (el < 0 || u >= 0.f)) { el = i; u -= w; }
-          }
-          p.aux = (uint32_t)el; p.blk = g.blk; p.vox = dep_vox;
-          if (P.dbg_out == nullptr) {
-            if (is_el) { c_el++; if (!queue_push(q_el, p)) atomicOr(&cnt->overflow, 2u); }
-            else { c_ne++; if (!queue_push(q_ne, p)) atomicOr(&cnt->overflow, 4u); }
-            alive = false;
-          }
-        }
+      if (alive && cls == 2 && P.dbg_out == nullptr) {
+        // ---- 8. discrete nuclear event at the end point (L71): handed to event_kernel, which picks the class and
+        // the target element with all lanes busy instead of one lane of this warp
+        p.blk = g.blk; p.vox = dep_vox; c_ev++;
+        if (!queue_push(q_ev, p)) atomicOr(&cnt->overflow, 2u);
+        alive = false;
       }
       if (alive && P.max_steps > 0 && nstep >= P.max_steps) alive = false;
       if (!alive) {
@@ -345,8 +320,52 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM) tr
     }
     deposit(tally, tbase + (uint32_t)dep_vox, dep, dep != 0.f, P.aggregate);
   }
-  flush(&cnt->n_steps, c_steps); flush(&cnt->n_elastic, c_el); flush(&cnt->n_nonelastic, c_ne);
+  flush(&cnt->n_steps, c_steps); (void)c_ev;
   flush(&cnt->e_deposit, c_dep); flush(&cnt->e_escape, c_esc);
+}
+
+// ------------------------------------------------------------------ event class and target element (Reading R5)
+// One event per thread over the event queue: elastic vs non-elastic in proportion to the macroscopic cross-sections at
+// the energy after the step, then the target element in proportion to n_i sigma_i within the class.  If both vanish at
+// that energy nothing happens and the proton goes on in the next generation.
+__global__ void __launch_bounds__(256) event_kernel(Tables T, Grid G, RunParams P, Queue in, Queue q_el, Queue q_ne, Queue next,
+                                                    Counters *cnt) {
+  const uint32_t n = min(*in.count, in.cap);
+  unsigned long long c_el = 0, c_ne = 0;
+  for (uint32_t i0 = blockIdx.x * blockDim.x; i0 < n; i0 += gridDim.x * blockDim.x) {
+    const uint32_t i = i0 + threadIdx.x;
+    if (i < n) {
+      Particle p = queue_load(in, i);
+      Rng g; g.init(P.seed, P.hist0 + p.hist, p.pid, p.blk);
+      const int hu = G.hu[p.vox];
+      const MatBin &m = T.bins[hu_to_bin(T, T.hu_lut, hu)];
+      const EIdx k1 = e_index(T, logf(fminf(fmaxf(p.e, T.e_min), T.e_max)));
+      float pel[MAX_ELEM], pne[MAX_ELEM], sel = 0.f, sne = 0.f;
+#pragma unroll
+      for (int e = 0; e < MAX_ELEM; ++e) {
+        pel[e] = 0.f; pne[e] = 0.f;
+        if (e < T.n_elem && m.nfac[e] > 0.f) {
+          if (T.opt_el) pel[e] = m.nfac[e] * lerp_tab(T.sig_el + e * T.n_e, k1);
+          if (T.opt_ne) pne[e] = m.nfac[e] * lerp_tab(T.sig_ne + e * T.n_e, k1);
+        }
+        sel += pel[e]; sne += pne[e];
+      }
+      if (sel + sne > 0.f) {
+        const uint4 q = g.next4();
+        const bool is_el = u01(q.x) * (sel + sne) < sel;
+        float u = u01(q.y) * (is_el ? sel : sne); int el = -1;
+#pragma unroll
+        for (int e = 0; e < MAX_ELEM; ++e) {
+          const float w = is_el ? pel[e] : pne[e];
+          if (w > 0.f && (el < 0 || u >= 0.f)) { el = e; u -= w; }
+        }
+        p.aux = (uint32_t)el; p.blk = g.blk;
+        if (is_el) { c_el++; if (!queue_push(q_el, p)) atomicOr(&cnt->overflow, 2u); }
+        else { c_ne++; if (!queue_push(q_ne, p)) atomicOr(&cnt->overflow, 4u); }
+      } else if (!queue_push(next, p)) atomicOr(&cnt->overflow, 8u);
+    }
+  }
+  flush(&cnt->n_elastic, c_el); flush(&cnt->n_nonelastic, c_ne);
 }
 
 // ------------------------------------------------------------------ nuclear elastic (Eq.3; Reading R5)

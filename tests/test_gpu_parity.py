@@ -342,7 +342,7 @@ def test_c4_head_and_neck_full_size_against_oracle_subsample(pm, tables):
     assert abs(eg - cg["e_deposit"] / n_g) < 3e-4 * eg
     for k in ("n_steps", "n_elastic", "n_nonelastic", "n_secondary_protons", "n_missed"):
         a, b = cg[k] / n_g, co[k] / n_o
-        assert abs(a - b) < 5 * np.sqrt(b / n_o + a / n_g) + 5e-3 * b, (k, a, b)
+        assert abs(a - b) <= 5 * np.sqrt(b / n_o + a / n_g) + 5e-3 * b, (k, a, b)
     # voxel z-scores: the GPU dose is nearly noise-free at 1e7, the oracle's sigma dominates
     # (tissue voxels only: in the air bin, rho = 0.0012, one stopping proton is a 1000x dose spike that would set the
     # "maximum" of a 4e5-history map)
@@ -360,6 +360,41 @@ def test_c4_head_and_neck_full_size_against_oracle_subsample(pm, tables):
     hi = tissue & (do > 0.5 * do[tissue].max())
     ratio = np.median(sg[hi] / np.maximum(dg[hi], 1e-30)) / np.median(so[hi] / np.maximum(do[hi], 1e-30))
     assert abs(ratio * np.sqrt(n_g / n_o) - 1) < 0.25
+
+
+def test_c5_pelvis_full_size_against_oracle_subsample(pm, tables):
+    """C5 (512x512x200 pelvis with Ti implants, 11033 spots, 100-230 MeV) at BASELINE's full 1e8 histories on the GPU
+    (6 sub-groups of 2^24 histories, 2.1 GB of per-batch tallies); the oracle runs a 5e5-history subsample."""
+    w = inputs.workload("c5")
+    o = _setup(pm, tables, w["materials"], w["hu"], w["vox"])
+    n_g, n_o = w["n_histories"], 500_000
+    dg, sg = pm.simulate(w["spots"], n_g, w["seed"])
+    cg = pm.counters()
+    dg, sg = dg.cpu().numpy().astype(np.float64), sg.cpu().numpy().astype(np.float64)
+    do, so = o.simulate(w["spots"], n_o, w["seed"] + 1)
+    co = o.counters()
+    assert _ledger_closes(cg) and cg["n_zab_violations"] == 0 and np.all(np.isfinite(dg)) and np.all(sg >= 0)
+    rho = _density(w["hu"], w["materials"])
+    vol = np.prod(w["vox"])
+    eg, eo = (dg * rho).sum() * vol / parity.GY_PER_MEV_G, (do * rho).sum() * vol / parity.GY_PER_MEV_G
+    assert abs(eg / eo - 1) < 5e-3                                         # integrated dose 0.5 %
+    assert abs(eg - cg["e_deposit"] / n_g) < 3e-4 * eg
+    for k in ("n_steps", "n_elastic", "n_nonelastic", "n_secondary_protons", "n_missed"):
+        a, b = cg[k] / n_g, co[k] / n_o
+        assert abs(a - b) <= 5 * np.sqrt(b / n_o + a / n_g) + 5e-3 * b, (k, a, b)
+    # energy deposited in the titanium implants (own stopping-power table, HU clamp 3071 -> 4.5 g/cm3, L49)
+    ti = w["hu"] >= 3060
+    a, b = (dg * rho)[ti].sum(), (do * rho)[ti].sum()
+    assert b > 0 and abs(a / b - 1) < 0.03, (a, b)
+    # voxel z-scores in tissue and bone (not air, see C4); few oracle histories per voxel: the 10-batch sigma of a
+    # skewed voxel dose correlates with the dose itself, which pushes the mean z up and fattens the tails
+    frac, zmean, zrms, nv = parity.zscore_pass(dg, sg, do, so, region=w["hu"] >= -950)
+    assert nv > 100_000 and frac >= 0.975 and abs(zmean) < 0.2 and zrms < 1.3, (frac, zmean, zrms, nv)
+    for ax in range(3):
+        pg, po = parity.depth_dose(dg * rho, ax), parity.depth_dose(do * rho, ax)
+        m = po > 0.05 * po.max()
+        tol = 0.01 + 0.012 * np.sqrt(po.max() / po[m])
+        assert np.all(np.abs(pg[m] / po[m] - 1) < tol), (ax, np.max(np.abs(pg[m] / po[m] - 1) / tol))
 
 
 # ------------------------------------------------------------------ edge and degenerate cases
