@@ -226,9 +226,9 @@ __device__ __forceinline__ void flush(unsigned long long *dst, unsigned long lon
 // variate with the exact variance and third cumulant (its fourth cumulant, 3 k3^2 / 2 k2, is within 12 % of the
 // exact xi T_c^3 / 3), through the Wilson-Hilferty cube of one normal deviate - monotone, and the plain Gaussian in
 // the limit T_c -> T_c0.  T_c is chosen so that about MU_HARD hard collisions are expected, which keeps the lanes of
-// a warp in step (the shape parameter of the gamma is then >= 16).  kappa >= kappa_G: Gaussian, variance
+// a warp in step (MU_HARD = 1/2: the shape parameter of the gamma is then >= 8, its skewness <= 0.71).  kappa >= kappa_G: Gaussian, variance
 // xi Tmax (1 - beta^2/2).
-constexpr float MU_HARD = 1.0f;
+constexpr float MU_HARD = 0.5f;
 __device__ __forceinline__ float gauss_pair(uint32_t a, uint32_t b) {
   return fsqrt(-2.0f * __logf(u01(a))) * -__cosf(TWO_PI * u01(b) - 3.14159265358979f);
 }

@@ -195,7 +195,7 @@ __device__ __forceinline__ void deposit(float *tally, uint32_t vox, float e, boo
 // Persistent kernel: every lane pulls a particle from the input queue, steps it in registers until it stops,
 // leaves the grid or reaches a discrete nuclear event, then refills from the queue (warp-aggregated fetch).
 // Particles that reach an event are appended to the elastic or non-elastic queue; nothing else is written back.
-constexpr int TRANSPORT_THREADS = 256, TRANSPORT_BLOCKS_PER_SM = 3;
+constexpr int TRANSPORT_THREADS = 256, TRANSPORT_BLOCKS_PER_SM = 4;
 
 __global__ void __launch_bounds__(TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM) transport_kernel(Tables T, Grid G, RunParams P, Queue in, uint32_t n_in,
                                                            uint32_t *head, Queue q_ev, float *tally, Counters *cnt) {
