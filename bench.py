@@ -28,6 +28,9 @@ METRIC = "proton histories/sec (full physics, dose on CT grid)"
 UNIT = "histories/s"
 # algorithmic thread-instructions of one condensed-history step of the transport kernel
 ALGO_INST_PER_STEP = 520.0
+# dram__bytes_read.sum + dram__bytes_write.sum of the first-generation transport launch of a 1e7-history C4 step, per
+# history (one `ncu --set full` capture, profiles/r01_transport_full.md): 546.2 MB + 117.7 MB
+NCU_DRAM_BYTES_PER_HISTORY_C4 = 66.4
 ISSUE_LANES_PER_SM_PER_CLK = 128.0     # 4 schedulers x 32 lanes
 N_SM = 148
 
@@ -262,7 +265,10 @@ def main():
         peak = N_SM * ISSUE_LANES_PER_SM_PER_CLK * sm_mhz * 1e6 / 1e9            # G thread-inst/s at the clock seen
         achieved = ALGO_INST_PER_STEP * steps_total / (t_transport * 1e-3) / 1e9 if t_transport > 0 else 0.0
         roofline = {"bound": "alu", "kernel": "transport_kernel", "achieved": achieved, "peak": peak,
-                    "unit": "Gthread-inst/s", "frac": achieved / peak if peak else None, "traffic": None,
+                    "unit": "Gthread-inst/s", "frac": achieved / peak if peak else None,
+                    "traffic": NCU_DRAM_BYTES_PER_HISTORY_C4 * n_hist if w["name"] == "c4" else None,
+                    "traffic_note": "DRAM bytes of the first-generation launch (ncu capture in profiles/); the kernel is "
+                                    "issue-bound, HBM carries < 1 % of its peak",
                     "peak_source": "148 SMs x 4 schedulers x 32 lanes x median SM clock under load (derived, DESIGN.md)",
                     "avg_launch_ms": t_transport / max(1, n_transport), "launches": n_transport,
                     "algorithmic_inst_per_condensed_step": ALGO_INST_PER_STEP,

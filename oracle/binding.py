@@ -154,6 +154,12 @@ class Oracle:
                                          C.c_uint64(n_histories), C.c_uint64(seed), _dp(dose), _dp(sigma)))
         return dose.reshape(self.shape), sigma.reshape(self.shape)
 
+    def letd(self):
+        """LET_d map (keV/um) of the last simulate() made with set_option("score_letd", 1)."""
+        out = np.zeros(self.shape, dtype=np.float64)
+        self._chk(self.lib.opmc_get_letd(self.ctx, _dp(out)))
+        return out
+
     def nonelastic(self, Z, A, e_mev, n, seed, capacity=None):
         capacity = capacity or 24 * n + 64
         out = np.zeros(capacity, dtype=SECONDARY_DTYPE)

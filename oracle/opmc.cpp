@@ -495,6 +495,7 @@ struct opmc_ctx {
   std::vector<Nucleus> nuc;                   // per element (A > 1)
   std::vector<int16_t> hu; int nx = 0, ny = 0, nz = 0; double d[3] = {0, 0, 0}, org[3] = {0, 0, 0};
   bool opt_strag = true, opt_mcs = true, opt_el = true, opt_ne = true; int threads = 0;
+  bool score_let = false; std::vector<double> let_num, let_den;   // LET_d tallies (Reading R9)
   opmc_counters cnt{};
   std::string err;
 };
@@ -595,12 +596,13 @@ bool transport_step(opmc_ctx *c, Particle &p, Rng &g, double *tally, Ledger &led
   p.d = dnew;
   if (pathlen) *pathlen += L;
   // 6. energy loss from the range table (L61-63, Eq.2) + straggling
-  double loss;
+  double loss, let_mean = 0;
   if (cls == 3) loss = e0;                         // 7. range-out: everything stays here (L71)
   else {
     double r1 = T.range_gcm2(m.table_id, e0) - L * wf;
     double mean = e0 - (r1 > 0 ? T.energy_of_range(m.table_id, r1) : 0.0);
     mean = std::min(std::max(mean, 0.0), e0);
+    let_mean = mean;
     loss = c->opt_strag ? straggle(T, g, e0, mean, L * rho, m.zoa) : mean;
   }
   p.E = e0 - loss;
@@ -610,6 +612,17 @@ bool transport_step(opmc_ctx *c, Particle &p, Rng &g, double *tally, Ledger &led
   #pragma omp atomic
   tally[vox] += dep;
   led.dep += dep;
+  if (c->score_let && dep > 0 && L > 0) {
+    // dose-averaged LET (Reading R9): every proton step weighs its LET, the table's mean energy loss
+    // over the step divided by the step length (keV/um = 0.1 MeV/cm; a proton that ranges out: its energy over its
+    // residual range), with the energy the step deposits; heavy recoils and fragments do not enter (L282)
+    const double mean_step = cls == 3 ? e0 : let_mean;
+    const double let_kev_um = 0.1 * mean_step / L;
+    #pragma omp atomic
+    c->let_num[vox] += dep * let_kev_um;
+    #pragma omp atomic
+    c->let_den[vox] += dep;
+  }
   if (!alive) return false;
   if (cls == 1) {                                                          // boundary: next voxel
     p.idx[ax2] += sg2;
@@ -852,7 +865,8 @@ int opmc_set_option(opmc_ctx *c, const char *key, double v) {
   if (k == "straggling") c->opt_strag = v != 0; else if (k == "mcs") c->opt_mcs = v != 0;
   else if (k == "elastic") c->opt_el = v != 0; else if (k == "nonelastic") c->opt_ne = v != 0;
   else if (k == "s_max_wet_cm") c->T.s_max = v; else if (k == "n_batches") c->T.n_batches = (int)v;
-  else if (k == "threads") c->threads = (int)v; else return fail(c, "unknown option");
+  else if (k == "threads") c->threads = (int)v; else if (k == "score_letd") c->score_let = v != 0;
+  else return fail(c, "unknown option");
   return 0;
 }
 
@@ -863,6 +877,7 @@ int opmc_simulate(opmc_ctx *c, const opmc_spot *spots, int nspots, uint64_t n, u
   if (B < 2) return fail(c, "need >= 2 batches");
   std::vector<double> cdf = spot_cdf(spots, nspots), tally(nv), s1(nv, 0.0), s2(nv, 0.0);
   c->cnt = opmc_counters{};
+  if (c->score_let) { c->let_num.assign(nv, 0.0); c->let_den.assign(nv, 0.0); }
 #ifdef _OPENMP
   if (c->threads > 0) omp_set_num_threads(c->threads);
 #endif
@@ -922,6 +937,13 @@ int opmc_nonelastic(opmc_ctx *c, int Z, int A, double e, uint64_t n, uint64_t se
   return 0;
 }
 
+// LET_d map of the last opmc_simulate run with "score_letd" on: keV/um, 0 where no proton step deposited energy
+int opmc_get_letd(opmc_ctx *c, double *out) {
+  if (!c || !out) return -1;
+  if (!c->score_let || c->let_num.size() != c->hu.size() || c->let_num.empty()) return fail(c, "no LET_d tally: set score_letd and simulate");
+  for (size_t v = 0; v < c->let_num.size(); ++v) out[v] = c->let_den[v] > 0 ? c->let_num[v] / c->let_den[v] : 0.0;
+  return 0;
+}
 int opmc_get_counters(opmc_ctx *c, opmc_counters *o) { if (!c || !o) return -1; *o = c->cnt; return 0; }
 
 // ---------------------------------------------------------------- test hooks

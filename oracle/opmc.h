@@ -87,6 +87,9 @@ int  opmc_simulate(opmc_ctx *, const opmc_spot *spots, int nspots, uint64_t n_hi
 int  opmc_nonelastic(opmc_ctx *, int Z, int A, double e_mev, uint64_t n, uint64_t seed,
                      opmc_secondary *out, uint64_t capacity, uint32_t *event_offsets, uint64_t *n_out);
 int  opmc_get_counters(opmc_ctx *, opmc_counters *);
+/* PAPER.md:L282 (Reading R9): dose-averaged LET of the last opmc_simulate call made with option "score_letd" = 1;
+ * out: nx*ny*nz doubles, keV/um, 0 where no proton step deposited energy. */
+int  opmc_get_letd(opmc_ctx *, double *out);
 const char *opmc_last_error(opmc_ctx *);
 
 /* ---- hooks used only by the pin tests ---- */

@@ -516,3 +516,72 @@ def test_air_gap_step(tables):
     assert c["e_air"] / 10 == pytest.approx(want, rel=1e-9)
     assert 0.25 < want < 0.40                                   # ~6.4 MeV cm2/g * 0.048 g/cm2 of air
     assert c["max_ledger_residual"] < 1e-9
+
+
+# ------------------------------------------------------------------ LET_d scoring (Reading R9)
+def _water_column(tables, nz=100, dz=0.2, **opts):
+    o = Oracle(tables, inputs.make_materials_c1())
+    o.load_ct(np.zeros((nz, 1, 1), dtype=np.int16), (50.0, 50.0, dz))
+    for k, v in opts.items():
+        o.set_option(k, v)
+    return o
+
+
+@pytest.mark.parametrize("s_max", [0.0, 0.05])
+def test_letd_csda_closed_form(tables, s_max):
+    """Fluctuations off, 150 MeV along a water column: every step in slab k has the same LET, so LET_d of the slab is
+    the stopping power averaged over it, 0.1 (E_in - E_out)/dz keV/um.  Expected values by direct integration of
+    dE/dz = -S(E) with the Bethe stopping power (scipy), not by the oracle's tables.  A dropped 0.1, a step length in
+    place of the water-equivalent length, or energy/length weights swapped would all fail this."""
+    dz, nz = 0.2, 100
+    o = _water_column(tables, nz, dz, straggling=0, mcs=0, elastic=0, nonelastic=0, s_max_wet_cm=s_max, score_letd=1)
+    o.simulate(inputs.plan_single_spot((25.0, 25.0, 0.0), 150.0, 0.0), 20, 3)
+    let = o.letd()[:, 0, 0]
+    zoa_w, i_w = 0.555087, 75.0
+    sol = integrate.solve_ivp(lambda z, e: -bethe_mass_stopping(np.maximum(e, 1e-3), zoa_w, i_w), (0.0, 14.0), [150.0],
+                              t_eval=np.arange(0, 71) * dz, rtol=1e-10, atol=1e-10)
+    e_face = sol.y[0]
+    expect = 0.1 * (e_face[:-1] - e_face[1:]) / dz
+    assert np.max(np.abs(let[:70] / expect - 1)) < 5e-3
+    # textbook entrance value: S(150 MeV, water) = 5.445 MeV cm2/g  ->  0.5445 keV/um (SURVEY 8(c).1)
+    assert abs(let[0] / 0.5445 - 1) < 5e-3
+    # rises monotonically to the end of range (15.77 cm) and is zero beyond it
+    k_end = int(15.77 / dz)
+    assert np.all(np.diff(let[:k_end]) > 0) and np.all(let[k_end + 1:] == 0) and let[k_end] > 5 * let[0]
+
+
+def test_letd_invariants_full_physics(oracle_c1):
+    """LET_d is a ratio of totals: independent of the batch split and (statistically) of the number of histories;
+    never below the minimum stopping power on the path; secondary protons raise it at the entrance (L280, ref [36])."""
+    hu, vox = inputs.phantom_c1()
+    o = oracle_c1
+    o.load_ct(hu, vox)
+    spots = inputs.plan_single_spot((5.1, 5.1, 0.0), 150.0, 0.3)
+    for k in ("straggling", "mcs", "elastic", "nonelastic", "score_letd"):
+        o.set_option(k, 1)
+    try:
+        d1, _ = o.simulate(spots, 20000, 5); l1 = o.letd()
+        o.set_option("n_batches", 20)
+        d2, _ = o.simulate(spots, 20000, 5); l2 = o.letd()
+        o.set_option("n_batches", 10)
+        assert np.allclose(l1, l2, rtol=1e-9, atol=1e-12)                 # same histories, other batch split
+        hi = d1 > 0.1 * d1.max()
+        assert np.all(l1[hi] > 0.5445 * 0.98)                            # S_min on the path is S(150 MeV)
+        # dose-weighted LET_d per slab: secondaries lift the entrance value above the primary's stopping power
+        num = (l1 * d1).sum(axis=(1, 2)); den = d1.sum(axis=(1, 2))
+        prof = num / np.maximum(den, 1e-300)
+        assert 1.01 < prof[0] / 0.5445 < 1.6
+        assert prof[70] > 2 * prof[0] and prof[78] > 1.5 * prof[70]           # towards the Bragg peak (R = 15.8 cm)
+        o.set_option("nonelastic", 0); o.set_option("elastic", 0)
+        d3, _ = o.simulate(spots, 20000, 5); l3 = o.letd()
+        prof3 = (l3 * d3).sum(axis=(1, 2)) / np.maximum(d3.sum(axis=(1, 2)), 1e-300)
+        assert abs(prof3[0] / 0.5445 - 1) < 0.01 and prof[0] > prof3[0]
+        # without score_letd there is no tally to read
+        o.set_option("score_letd", 0)
+        o.simulate(spots, 100, 5)
+        with pytest.raises(Exception):
+            o.letd()
+    finally:
+        for k in ("straggling", "mcs", "elastic", "nonelastic"):
+            o.set_option(k, 1)
+        o.set_option("score_letd", 0)
