@@ -129,7 +129,7 @@ int  pmc_load_ct_host(pmc_ctx *ctx, const int16_t *hu_host, int nx, int ny, int 
 
 /* Options: "straggling" "mcs" "elastic" "nonelastic" (0/1), "s_max_wet_cm", "n_batches",
  * "chunk_histories" (histories per sub-group), "history_offset" (first history id, for sharding
- * a run over several GPUs), "dose_aggregate" (0/1 warp-aggregated dose atomics),
+ * a run over several GPUs), "dose_aggregate" (0/1 warp-aggregated dose atomics), "score_letd" (0/1, see pmc_get_letd),
  * "profile" (0/1, default 1: a CUDA-event pair is recorded on the context's stream around every kernel launch and
  * resolved into pmc_timing at the end of the call; no extra synchronisation). */
 int  pmc_set_option(pmc_ctx *ctx, const char *key, double value);
@@ -153,6 +153,14 @@ int  pmc_simulate_host(pmc_ctx *ctx, const pmc_spot *spots_host, int nspots, uin
  * PMC_E_UNSUPPORTED if (Z,A) or its neighbours are not in the mass table. */
 int  pmc_nonelastic(pmc_ctx *ctx, int Z, int A, double e_mev, uint64_t n, uint64_t seed,
                     pmc_secondary *out_dev, uint64_t capacity, uint32_t *event_offsets_dev, uint64_t *n_out_host);
+
+/* PAPER.md:L282 (Fig 9; Reading R9): dose-averaged LET scored "simultaneously" with the dose.  With option
+ * "score_letd" = 1, pmc_simulate also tallies, for every step of every proton (primaries and secondaries; heavy
+ * recoils and fragments do not enter, L282), e x LET and e per voxel, where e is the energy the step deposits and LET
+ * the range table's mean energy loss over the step divided by the step length.  pmc_get_letd writes
+ * sum(e x LET) / sum(e) in keV/um (0 where no proton step deposited energy) into letd_dev: DEVICE array of nx*ny*nz
+ * float, caller-owned.  Errors: PMC_E_STATE if the last pmc_simulate did not score LET_d. */
+int  pmc_get_letd(pmc_ctx *ctx, float *letd_dev);
 
 int  pmc_get_counters(pmc_ctx *ctx, pmc_counters *out_host);
 int  pmc_get_timing(pmc_ctx *ctx, pmc_timing *out_host);

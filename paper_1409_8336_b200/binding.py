@@ -19,7 +19,7 @@ _I = C.POINTER(C.c_int32)
 
 EXPORTS = ["pmc_create", "pmc_destroy", "pmc_load_physics_tables", "pmc_set_hu_materials", "pmc_load_ct",
            "pmc_load_ct_host", "pmc_set_option", "pmc_simulate", "pmc_simulate_host", "pmc_nonelastic",
-           "pmc_get_counters", "pmc_get_timing", "pmc_last_error", "pmc_philox4x32_10", "pmc_range_of_energy",
+           "pmc_get_counters", "pmc_get_timing", "pmc_get_letd", "pmc_last_error", "pmc_philox4x32_10", "pmc_range_of_energy",
            "pmc_energy_of_range", "pmc_straggle", "pmc_elastic", "pmc_first_steps"]
 
 
@@ -179,6 +179,13 @@ class Pmc:
         self._chk(self.lib.pmc_simulate_host(self.ctx, spots.ctypes.data_as(C.c_void_p), C.c_int(spots.shape[0]),
                                              C.c_uint64(n_histories), C.c_uint64(seed),
                                              dose_host.ctypes.data_as(C.c_void_p), sigma_host.ctypes.data_as(C.c_void_p)))
+
+    def letd(self, out=None):
+        """-> LET_d map (keV/um), CUDA float32 tensor (nz, ny, nx), of the last simulate() with score_letd = 1."""
+        if out is None:
+            out = self.torch.empty(self.shape, dtype=self.torch.float32, device=self.device)
+        self._chk(self.lib.pmc_get_letd(self.ctx, _ptr(out)))
+        return out
 
     def nonelastic(self, Z, A, e_mev, n, seed, capacity=None):
         """-> (records: numpy structured array, offsets: numpy uint32 [n+1])."""

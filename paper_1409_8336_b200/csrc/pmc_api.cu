@@ -81,7 +81,8 @@ struct pmc_ctx {
   DevBuf<int16_t> d_hu_own;
   // scratch
   QueueMem qa, qb, qev, qel, qne, qres; DevBuf<uint32_t> d_resza; DevBuf<float> d_resp;
-  DevBuf<uint32_t> d_head; DevBuf<Counters> d_cnt; DevBuf<float> d_tally, d_out;
+  DevBuf<uint32_t> d_head; DevBuf<Counters> d_cnt; DevBuf<float> d_tally, d_out, d_let;
+  bool score_let = false, have_let = false;
   DevBuf<SpotDev> d_spots; DevBuf<double> d_cdf;
   DevBuf<SecRec> d_slots; DevBuf<uint32_t> d_counts; DevBuf<unsigned long long> d_base; DevBuf<ResRec> d_res;
   uint32_t *h_pinned = nullptr;     // pinned readback word(s)
@@ -359,7 +360,7 @@ void pmc_destroy(pmc_ctx *c) {
   c->d_sigbin.release(); c->d_ek.release(); c->d_ec.release(); c->d_mass.release(); c->d_bins.release(); c->d_lut.release();
   c->d_nuc.release(); c->d_nuc1.release(); c->d_hu_own.release();
   c->qa.release(); c->qb.release(); c->qev.release(); c->qel.release(); c->qne.release(); c->qres.release(); c->d_resza.release(); c->d_resp.release();
-  c->d_head.release(); c->d_cnt.release(); c->d_tally.release(); c->d_out.release();
+  c->d_head.release(); c->d_cnt.release(); c->d_tally.release(); c->d_out.release(); c->d_let.release();
   c->d_spots.release(); c->d_cdf.release(); c->d_res.release(); c->d_slots.release(); c->d_counts.release(); c->d_base.release();
   if (c->h_pinned) cudaFreeHost(c->h_pinned);
   if (c->ev[0]) { cudaEventDestroy(c->ev[0]); cudaEventDestroy(c->ev[1]); }
@@ -466,6 +467,7 @@ int pmc_set_option(pmc_ctx *c, const char *key, double v) {
   else if (k == "history_offset") { if (v < 0) return fail(c, PMC_E_INVALID_ARG, "negative offset"); c->history_offset = (uint64_t)v; }
   else if (k == "dose_aggregate") c->aggregate = v != 0;
   else if (k == "profile") c->profile = v != 0;
+  else if (k == "score_letd") c->score_let = v != 0;
   else return fail(c, PMC_E_INVALID_ARG, "unknown option");
   c->tables_dirty = true;
   return PMC_OK;
@@ -495,6 +497,9 @@ static int simulate_impl(pmc_ctx *c, const pmc_spot *spots_in, int nspots, uint6
   CK(c->d_tally.alloc(nvox_s * B));
   cudaStream_t s = c->stream;
   CK(cudaMemsetAsync(c->d_tally.p, 0, nvox_s * B * 4, s)); CK(cudaMemsetAsync(c->d_cnt.p, 0, sizeof(Counters), s));
+  const bool let_on = c->score_let && !dbg_out;
+  c->have_let = false;
+  if (let_on) { CK(c->d_let.alloc(2 * nvox_s)); CK(cudaMemsetAsync(c->d_let.p, 0, 2 * nvox_s * 4, s)); }
   c->counters = pmc_counters{}; c->timing = pmc_timing{};
   float air_rho, air_wf, air_ix0, air_zoa; int air_tab; air_params(c, air_rho, air_wf, air_ix0, air_zoa, air_tab);
   const bool profile = c->profile;
@@ -506,6 +511,7 @@ static int simulate_impl(pmc_ctx *c, const pmc_spot *spots_in, int nspots, uint6
     const uint32_t nc = (uint32_t)std::min<uint64_t>(chunk, n - cs);
     RunParams P{}; P.seed = seed; P.hist0 = c->history_offset + cs; P.n = nc; P.max_steps = max_steps; P.dbg_out = dbg_out ? dbg_out + 8ull * cs : nullptr;
     P.aggregate = c->aggregate; P.local0 = cs; P.n_total = n; P.B = (uint32_t)B; P.nvox = nvox;
+    P.let_num = let_on ? c->d_let.p : nullptr; P.let_den = let_on ? c->d_let.p + nvox_s : nullptr;
     P.b_over_n = (float)((double)B / (double)n); P.inv_nx = 1.0f / (float)c->G.nx; P.inv_ny = 1.0f / (float)c->G.ny;
     CK(cudaMemsetAsync(c->qa.q.count, 0, 4, s));
     { Timer t(c, &c->timing.sampler_ms, profile);
@@ -523,6 +529,7 @@ static int simulate_impl(pmc_ctx *c, const pmc_spot *spots_in, int nspots, uint6
   CK(cudaEventRecord(e1, s));
   CK(cudaGetLastError());
   rc = fetch_counters(c);
+  c->have_let = let_on && rc == PMC_OK;
   resolve_timers(c);
   float ms = 0; cudaEventElapsedTime(&ms, e0, e1); c->timing.total_ms = ms;
   cudaEventDestroy(e0); cudaEventDestroy(e1);
@@ -590,6 +597,16 @@ int pmc_nonelastic(pmc_ctx *c, int Z, int A, double e_mev, uint64_t n, uint64_t 
   rc = fetch_counters(c); if (rc) return rc;
   c->counters.n_nonelastic = n;
   if (total > capacity) return fail(c, PMC_E_CAPACITY, "capacity too small");
+  return PMC_OK;
+}
+
+int pmc_get_letd(pmc_ctx *c, float *letd_dev) {
+  if (!c || !letd_dev) return fail(c, PMC_E_INVALID_ARG, "null argument");
+  if (!c->have_let) return fail(c, PMC_E_STATE, "no LET_d tally: set option score_letd = 1 and call pmc_simulate");
+  cudaSetDevice(c->device);
+  const size_t nvox = (size_t)c->G.nx * c->G.ny * c->G.nz;
+  letd_kernel<<<c->n_sm * 8, 256, 0, c->stream>>>(c->d_let.p, c->d_let.p + nvox, letd_dev, (uint32_t)nvox);
+  CK(cudaStreamSynchronize(c->stream)); CK(cudaGetLastError());
   return PMC_OK;
 }
 

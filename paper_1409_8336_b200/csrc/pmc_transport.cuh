@@ -18,6 +18,7 @@ struct RunParams {
   uint64_t local0, n_total;           // call-local index of this launch's first history; histories in the call
   uint32_t B, nvox;
   float b_over_n, inv_nx, inv_ny;     // B / n_total, 1 / nx, 1 / ny
+  float *let_num, *let_den;           // LET_d tallies [nvox] (Reading R9) or nullptr
   int max_steps; float *dbg_out;      // pmc_first_steps: stop after max_steps, write [hist][8]
   int aggregate;                      // warp-aggregated dose atomics
 };
@@ -175,20 +176,35 @@ __global__ void __launch_bounds__(256) sampler_kernel(Tables T, Grid G, const Sp
 // ------------------------------------------------------------------ dose deposit (atomics)
 // Lanes of a warp that score into the same voxel in the same iteration are merged (warp match) so that a
 // single RED reaches the L2; with a pencil beam the lanes advance slab by slab and collide often.
-__device__ __forceinline__ void deposit(float *tally, uint32_t vox, float e, bool on, int aggregate) {
-  if (!aggregate) { if (on && e != 0.f) atomicAdd(tally + vox, e); return; }
+// With LET_d scoring on, the same merge also carries the step's e x LET into the numerator grid and e into the
+// denominator grid (indexed by voxel, not by batch).
+__device__ __forceinline__ void deposit(float *tally, uint32_t tvox, float e, bool on, int aggregate,
+                                        float *let_num, float *let_den, uint32_t vox, float e_let, float let) {
+  const bool has_let = let_num != nullptr;
+  if (!aggregate) {
+    if (on && e != 0.f) atomicAdd(tally + tvox, e);
+    if (has_let && on && e_let > 0.f) { atomicAdd(let_num + vox, e_let * let); atomicAdd(let_den + vox, e_let); }
+    return;
+  }
   const unsigned act = __ballot_sync(0xffffffffu, on);
   if (!on) return;
-  const unsigned peers = __match_any_sync(act, vox);
+  const unsigned peers = __match_any_sync(act, tvox);
   const int lane = threadIdx.x & 31, leader = __ffs(peers) - 1;
-  float sum = e;
+  float sum = e, sn = e_let * let, sd = e_let;
   if (peers != (1u << lane)) {
     // segmented reduction over the peer set
-    sum = 0.f;
+    sum = 0.f; sn = 0.f; sd = 0.f;
     unsigned m = peers;
-    while (m) { const int src = __ffs(m) - 1; m &= m - 1; sum += __shfl_sync(peers, e, src); }
+    while (m) {
+      const int src = __ffs(m) - 1; m &= m - 1;
+      sum += __shfl_sync(peers, e, src);
+      if (has_let) { sn += __shfl_sync(peers, e_let * let, src); sd += __shfl_sync(peers, e_let, src); }
+    }
   }
-  if (lane == leader && sum != 0.f) atomicAdd(tally + vox, sum);
+  if (lane == leader) {
+    if (sum != 0.f) atomicAdd(tally + tvox, sum);
+    if (has_let && sd > 0.f) { atomicAdd(let_num + vox, sn); atomicAdd(let_den + vox, sd); }
+  }
 }
 
 // ------------------------------------------------------------------ K2: condensed-history step kernel (Reading R3)
@@ -243,7 +259,7 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM) tr
     }
     if (!__any_sync(0xffffffffu, active)) break;
 
-    float dep = 0.f; int dep_vox = p.vox;
+    float dep = 0.f, let = 0.f; int dep_vox = p.vox;
     if (active) {
       // ---- material of the current voxel
       const int hu = G.hu[p.vox];
@@ -282,10 +298,11 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM) tr
       p.d = dnew; path += L;
       // ---- 6. energy loss from the range table (Eq.2) + straggling (L61)
       float loss;
-      if (cls == 3) loss = e0;                                  // 7. range-out: everything stays here (L71)
+      if (cls == 3) { loss = e0; let = L > 0.f ? fdiv(0.1f * e0, L) : 0.f; }   // 7. range-out: everything stays here (L71)
       else if (L <= 0.f) loss = 0.f;
       else {
         loss = mean_loss(T, s_lnE, s_lnE2, tab, e0, lnEv, lnRv, Rg, L * wf);
+        let = fdiv(0.1f * loss, L);                              // keV/um of this step (Reading R9)
         if (T.opt_strag) loss = straggle(T, g, e0, loss, L * rho, m.zoa);
       }
       p.e = e0 - loss; dep = loss;
@@ -318,7 +335,7 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM) tr
         }
       }
     }
-    deposit(tally, tbase + (uint32_t)dep_vox, dep, dep != 0.f, P.aggregate);
+    deposit(tally, tbase + (uint32_t)dep_vox, dep, dep != 0.f, P.aggregate, P.let_num, P.let_den, (uint32_t)dep_vox, let > 0.f ? dep : 0.f, let);
   }
   flush(&cnt->n_steps, c_steps); (void)c_ev;
   flush(&cnt->e_deposit, c_dep); flush(&cnt->e_escape, c_esc);
@@ -456,6 +473,12 @@ __global__ void __launch_bounds__(256) stats_kernel(Tables T, Grid G, const floa
     const float var = s / ((float)B * (float)(B - 1));
     sigma[v] = var > 0.f ? sqrtf(var) : 0.f;
   }
+}
+
+// LET_d = sum(e x LET) / sum(e) per voxel (keV/um), 0 where no proton step deposited energy
+__global__ void __launch_bounds__(256) letd_kernel(const float *num, const float *den, float *out, uint32_t nvox) {
+  for (uint32_t v = blockIdx.x * blockDim.x + threadIdx.x; v < nvox; v += gridDim.x * blockDim.x)
+    out[v] = den[v] > 0.f ? num[v] / den[v] : 0.f;
 }
 
 }  // namespace pmc

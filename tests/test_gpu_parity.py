@@ -397,6 +397,57 @@ def test_c5_pelvis_full_size_against_oracle_subsample(pm, tables):
         assert np.all(np.abs(pg[m] / po[m] - 1) < tol), (ax, np.max(np.abs(pg[m] / po[m] - 1) / tol))
 
 
+# ------------------------------------------------------------------ LET_d scoring
+def test_letd_deterministic_column_matches_oracle(pm, tables):
+    # fluctuations off: every history is the same CSDA track, LET_d per slab compared element by element
+    hu, vox = np.zeros((100, 1, 1), dtype=np.int16), (50.0, 50.0, 0.2)
+    o = _setup(pm, tables, inputs.make_materials_c1(), hu, vox, straggling=0, mcs=0, elastic=0, nonelastic=0)
+    spot = inputs.plan_single_spot((25.0, 25.0, 0.0), 150.0, 0.0)
+    pm.set_option("score_letd", 1.0); o.set_option("score_letd", 1.0)
+    try:
+        pm.simulate(spot, 64, 3); o.simulate(spot, 64, 3)
+        lg, lo = pm.letd().cpu().numpy().astype(np.float64)[:, 0, 0], o.letd()[:, 0, 0]
+    finally:
+        pm.set_option("score_letd", 0.0)
+    k_end = int(np.max(np.nonzero(lo)[0]))
+    assert np.all(lg[k_end + 1:] == 0) and np.all(lo[k_end + 1:] == 0)
+    assert np.max(np.abs(lg[:k_end - 1] / lo[:k_end - 1] - 1)) < 2e-4      # fp32 range-table differences per slab
+    assert abs(lg[k_end] / lo[k_end] - 1) < 0.05                          # the stopping slab: e0 / residual range
+
+
+def test_letd_full_physics_matches_oracle(pm, tables):
+    from paper_1409_8336_b200 import PmcError
+    w = inputs.workload("c1")
+    o = _setup(pm, tables, w["materials"], w["hu"], w["vox"])
+    n = 200_000
+    with pytest.raises(PmcError) as e:                                    # nothing scored yet
+        pm.simulate(w["spots"], 100, 1); pm.letd()
+    assert e.value.code == -2
+    d0, _ = pm.simulate(w["spots"], n, 31)
+    pm.set_option("score_letd", 1.0); o.set_option("score_letd", 1.0)
+    try:
+        dg, _ = pm.simulate(w["spots"], n, 31); lg = pm.letd().cpu().numpy().astype(np.float64)
+        do, _ = o.simulate(w["spots"], n, 32); lo = o.letd()
+        do2, _ = o.simulate(w["spots"], n, 33); lo2 = o.letd()             # second oracle run: the noise yardstick
+    finally:
+        pm.set_option("score_letd", 0.0)
+    assert torch.allclose(dg, d0, rtol=2e-4, atol=1e-16)                  # scoring LET_d does not change the dose
+    dg = dg.cpu().numpy().astype(np.float64)
+    assert np.all(np.isfinite(lg)) and np.all(lg >= 0) and np.all((lg > 0) <= (dg > 0))
+    # dose-weighted LET_d per slab, up to the distal 10 % of the depth dose
+    def prof(l, d):
+        return (l * d).sum(axis=(1, 2)) / np.maximum(d.sum(axis=(1, 2)), 1e-300)
+    pg, po, po2 = prof(lg, dg), prof(lo, do), prof(lo2, do2)
+    dd = do.sum(axis=(1, 2)); m = dd > 0.1 * dd.max()
+    noise = np.abs(po2[m] / po[m] - 1)
+    assert np.all(np.abs(pg[m] / po[m] - 1) < 0.01 + 4 * np.maximum(noise, np.median(noise))), (pg[m] / po[m])[:80]
+    assert abs(np.mean(pg[m] / po[m]) - 1) < 3e-3                         # no systematic offset along the depth
+    # voxel by voxel in the high-dose region: GPU-vs-oracle scatter is the oracle-vs-oracle scatter
+    hi = do > 0.1 * do.max()
+    rg, ro = lg[hi] / lo[hi] - 1, lo2[hi] / lo[hi] - 1
+    assert abs(np.median(rg)) < 3e-3 and rg.std() < 1.25 * ro.std() + 1e-3, (np.median(rg), rg.std(), ro.std())
+
+
 # ------------------------------------------------------------------ edge and degenerate cases
 def test_simulate_edge_cases(pm, tables):
     from paper_1409_8336_b200 import PmcError
