@@ -259,6 +259,26 @@ def main():
     h2d = int(w["hu"].nbytes + spots.nbytes)
     d2h = int(2 * nvox * 4)
 
+    # ---- SURVEY 8(f) rows built so far, measured on the same workload (not part of the timed steps above)
+    extras = None
+    if rank == 0:
+        pm.load_ct(hu_dev, w["vox"])
+        pm.set_option("score_letd", 1.0)
+        pm.simulate(spots, n_hist, w["seed"] + 200)
+        d_a, _ = pm.simulate(spots, n_hist, w["seed"] + 201); let_ms = pm.timing()["total_ms"]; d_a = d_a.clone()
+        pm.set_option("score_letd", 0.0)
+        d_b, _ = pm.simulate(spots, n_hist, w["seed"] + 202); plain_ms = pm.timing()["total_ms"]
+        tissue = torch.as_tensor(w["hu"] >= -950, device=dev)
+        d_a *= tissue; d_b = d_b * tissue
+        pm.gamma_index(d_a, d_b, w["vox"], 0.02, 0.2, 0.1)
+        g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        g0.record()
+        for _ in range(5):
+            _, g_rate = pm.gamma_index(d_a, d_b, w["vox"], 0.02, 0.2, 0.1)
+        g1.record(); torch.cuda.synchronize(dev)
+        extras = {"letd_scoring_ms_per_step": let_ms, "same_without_letd_ms": plain_ms,
+                  "gamma_index_2pct_2mm_ms_per_call": g0.elapsed_time(g1) / 5, "gamma_pass_rate_two_seeds": g_rate}
+
     if rank == 0:
         # ---- roofline of the dominant kernel (transport_kernel): plain-ALU issue bound
         sm_mhz = clocks["sm_mhz"] or 1965.0
@@ -291,7 +311,7 @@ def main():
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "steps": e2e_steps},
             "gpu_launches": int(launches),
-            "roofline": roofline, "cpu_baseline": cpu,
+            "roofline": roofline, "cpu_baseline": cpu, "extras": extras,
             "kernel_ms_per_step": {k: v / args.steps for k, v in klass.items()},
             "counters_last_step": {k: cnt_last[k] for k in ("n_steps", "n_elastic", "n_nonelastic",
                                                             "n_secondary_protons", "n_generations", "n_missed")},

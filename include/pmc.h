@@ -162,6 +162,20 @@ int  pmc_nonelastic(pmc_ctx *ctx, int Z, int A, double e_mev, uint64_t n, uint64
  * float, caller-owned.  Errors: PMC_E_STATE if the last pmc_simulate did not score LET_d. */
 int  pmc_get_letd(pmc_ctx *ctx, float *letd_dev);
 
+/* PAPER.md:L166 ("3D gamma index ... 2 %/2 mm ... also computed on the GPU", ref [34]; Reading R10): gamma index of
+ * the evaluated dose grid against the reference grid, both DEVICE arrays of nx*ny*nz float (x fastest), voxel sizes
+ * in cm.  For every reference voxel r with D_ref(r) >= low_dose_frac * max(D_ref):
+ *   gamma(r) = min over evaluated voxel centres r' with |r' - r| <= search_cm of
+ *              sqrt(|r' - r|^2 / dta_cm^2 + (D_eval(r') - D_ref(r))^2 / (dd_frac * max(D_ref))^2)
+ * (global dose criterion, no sub-voxel interpolation); other voxels get -1.  search_cm <= 0 selects 2 * dta_cm.
+ * gamma_dev: DEVICE, nx*ny*nz float, caller-owned, overwritten.  pass_rate_host (HOST, may be NULL): fraction of the
+ * evaluated voxels with gamma <= 1 (1 if none is evaluated).  Needs no tables, materials or CT.
+ * Errors: PMC_E_INVALID_ARG (null pointers, non-positive sizes or criteria), PMC_E_UNSUPPORTED (nz > 65535, search
+ * sphere of more than 4e6 voxels). */
+int  pmc_gamma_index(pmc_ctx *ctx, const float *ref_dev, const float *eval_dev, int nx, int ny, int nz,
+                     double dx_cm, double dy_cm, double dz_cm, double dd_frac, double dta_cm, double low_dose_frac,
+                     double search_cm, float *gamma_dev, double *pass_rate_host);
+
 int  pmc_get_counters(pmc_ctx *ctx, pmc_counters *out_host);
 int  pmc_get_timing(pmc_ctx *ctx, pmc_timing *out_host);
 const char *pmc_last_error(pmc_ctx *ctx);     /* owned by ctx, valid until the next call on ctx */

@@ -8,7 +8,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpmc.so")
 SOURCES = ["pmc_api.cu"]
-HEADERS = ["pmc_device.cuh", "pmc_transport.cuh", "pmc_nuclear.cuh"]
+HEADERS = ["pmc_device.cuh", "pmc_transport.cuh", "pmc_nuclear.cuh", "pmc_gamma.cuh"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "--compiler-options", "-fPIC", "-shared"]
 

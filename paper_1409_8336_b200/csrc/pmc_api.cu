@@ -6,12 +6,14 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <algorithm>
 #include <string>
 #include <vector>
 
 #include "pmc_device.cuh"
 #include "pmc_transport.cuh"
 #include "pmc_nuclear.cuh"
+#include "pmc_gamma.cuh"
 
 using namespace pmc;
 
@@ -85,6 +87,7 @@ struct pmc_ctx {
   bool score_let = false, have_let = false;
   DevBuf<SpotDev> d_spots; DevBuf<double> d_cdf;
   DevBuf<SecRec> d_slots; DevBuf<uint32_t> d_counts; DevBuf<unsigned long long> d_base; DevBuf<ResRec> d_res;
+  DevBuf<GammaOffset> d_goff; DevBuf<unsigned long long> d_gscr;
   uint32_t *h_pinned = nullptr;     // pinned readback word(s)
   uint32_t qcap = 0;
   int n_sm = 148; size_t smem_transport = 0;
@@ -361,7 +364,7 @@ void pmc_destroy(pmc_ctx *c) {
   c->d_nuc.release(); c->d_nuc1.release(); c->d_hu_own.release();
   c->qa.release(); c->qb.release(); c->qev.release(); c->qel.release(); c->qne.release(); c->qres.release(); c->d_resza.release(); c->d_resp.release();
   c->d_head.release(); c->d_cnt.release(); c->d_tally.release(); c->d_out.release(); c->d_let.release();
-  c->d_spots.release(); c->d_cdf.release(); c->d_res.release(); c->d_slots.release(); c->d_counts.release(); c->d_base.release();
+  c->d_spots.release(); c->d_cdf.release(); c->d_res.release(); c->d_goff.release(); c->d_gscr.release(); c->d_slots.release(); c->d_counts.release(); c->d_base.release();
   if (c->h_pinned) cudaFreeHost(c->h_pinned);
   if (c->ev[0]) { cudaEventDestroy(c->ev[0]); cudaEventDestroy(c->ev[1]); }
   for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
@@ -607,6 +610,43 @@ int pmc_get_letd(pmc_ctx *c, float *letd_dev) {
   const size_t nvox = (size_t)c->G.nx * c->G.ny * c->G.nz;
   letd_kernel<<<c->n_sm * 8, 256, 0, c->stream>>>(c->d_let.p, c->d_let.p + nvox, letd_dev, (uint32_t)nvox);
   CK(cudaStreamSynchronize(c->stream)); CK(cudaGetLastError());
+  return PMC_OK;
+}
+
+int pmc_gamma_index(pmc_ctx *c, const float *ref_dev, const float *eval_dev, int nx, int ny, int nz, double dx, double dy, double dz,
+                    double dd_frac, double dta_cm, double low_dose_frac, double search_cm, float *gamma_dev, double *pass_rate_host) {
+  if (!c || !ref_dev || !eval_dev || !gamma_dev) return fail(c, PMC_E_INVALID_ARG, "null argument");
+  if (nx < 1 || ny < 1 || nz < 1 || !(dx > 0) || !(dy > 0) || !(dz > 0) || (double)nx * ny * nz >= 2147483648.0) return fail(c, PMC_E_INVALID_ARG, "bad grid");
+  if (!(dd_frac > 0) || !(dta_cm > 0) || !(low_dose_frac >= 0)) return fail(c, PMC_E_INVALID_ARG, "criteria must be positive");
+  if (nz > 65535) return fail(c, PMC_E_UNSUPPORTED, "nz > 65535");
+  if (!(search_cm > 0)) search_cm = 2.0 * dta_cm;
+  cudaSetDevice(c->device);
+  // lattice offsets inside the search sphere, nearest first (Reading R10: voxel centres, no interpolation)
+  const int rx = (int)std::floor(search_cm / dx + 1e-9), ry = (int)std::floor(search_cm / dy + 1e-9), rz = (int)std::floor(search_cm / dz + 1e-9);
+  if ((double)(2 * rx + 1) * (2 * ry + 1) * (2 * rz + 1) > 4.0e6) return fail(c, PMC_E_UNSUPPORTED, "search radius spans too many voxels");
+  std::vector<std::pair<double, GammaOffset>> offs;
+  for (int k = -rz; k <= rz; ++k) for (int j = -ry; j <= ry; ++j) for (int i = -rx; i <= rx; ++i) {
+    const double d2 = (i * dx) * (i * dx) + (j * dy) * (j * dy) + (k * dz) * (k * dz);
+    if (d2 > search_cm * search_cm * (1 + 1e-12)) continue;
+    GammaOffset f{}; f.i = (int16_t)i; f.j = (int16_t)j; f.k = (int16_t)k; f.d2_over_dta2 = (float)(d2 / (dta_cm * dta_cm));
+    offs.push_back({d2, f});
+  }
+  std::stable_sort(offs.begin(), offs.end(), [](const auto &a, const auto &b) { return a.first < b.first; });
+  std::vector<GammaOffset> h(offs.size());
+  for (size_t i = 0; i < offs.size(); ++i) h[i] = offs[i].second;
+  cudaStream_t s = c->stream;
+  CK(c->d_goff.upload(h, s)); CK(c->d_gscr.alloc(3));
+  CK(cudaMemsetAsync(c->d_gscr.p, 0, 3 * sizeof(unsigned long long), s));
+  const uint32_t nvox = (uint32_t)((size_t)nx * ny * nz);
+  GammaParams G{}; G.nx = nx; G.ny = ny; G.nz = nz; G.n_off = (int)h.size(); G.inv_dd_frac = (float)(1.0 / dd_frac); G.low_dose_frac = (float)low_dose_frac;
+  uint32_t *dmax_bits = reinterpret_cast<uint32_t *>(c->d_gscr.p + 2);
+  gamma_max_kernel<<<c->n_sm * 8, 256, 0, s>>>(ref_dev, nvox, dmax_bits);
+  const dim3 blk(32, 8, 1), grd((nx + 31) / 32, (ny + 7) / 8, nz);
+  gamma_kernel<<<grd, blk, 0, s>>>(ref_dev, eval_dev, c->d_goff.p, G, dmax_bits, gamma_dev, c->d_gscr.p);
+  unsigned long long cnt[2] = {0, 0};
+  CK(cudaMemcpyAsync(cnt, c->d_gscr.p, sizeof(cnt), cudaMemcpyDeviceToHost, s));
+  CK(cudaStreamSynchronize(s)); CK(cudaGetLastError());
+  if (pass_rate_host) *pass_rate_host = cnt[0] ? (double)cnt[1] / (double)cnt[0] : 1.0;
   return PMC_OK;
 }
 

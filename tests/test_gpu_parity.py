@@ -362,6 +362,26 @@ def test_c4_head_and_neck_full_size_against_oracle_subsample(pm, tables):
     assert abs(ratio * np.sqrt(n_g / n_o) - 1) < 0.25
 
 
+def test_c4_two_seeds_eq5_and_gamma(pm, tables):
+    """PAPER.md:L172 Eq.5: two runs that differ only in the seed scatter by sqrt(2) x the reported statistical error;
+    and their 3-D gamma index (2 %/2 mm, L166) passes everywhere.  Pins the batch sigma of the CUDA path at full size."""
+    w = inputs.workload("c4")
+    _setup(pm, tables, w["materials"], w["hu"], w["vox"])
+    n = w["n_histories"]
+    d1, s1 = pm.simulate(w["spots"], n, 101); d1, s1 = d1.clone(), s1.clone()
+    d2, s2 = pm.simulate(w["spots"], n, 202)
+    tissue = torch.as_tensor(w["hu"] >= -950, device=d1.device)
+    hi = tissue & (d1 > 0.5 * d1[tissue].max())
+    assert int(hi.sum()) > 1000
+    delta = ((d1[hi] - d2[hi]) / d1[hi]).double()
+    sig = (0.5 * (s1[hi] / d1[hi] + s2[hi] / d2[hi])).double()
+    ratio = float(delta.pow(2).mean().sqrt() / (np.sqrt(2.0) * sig.pow(2).mean().sqrt()))
+    assert abs(ratio - 1) < 0.1, ratio                                     # 10-batch sigma estimator, RMS over > 1e3 voxels
+    a, b = d1 * tissue, d2 * tissue                                        # dose to tissue (air voxels spike, see above)
+    g, rate = pm.gamma_index(a, b, w["vox"], 0.02, 0.2, 0.1)
+    assert rate > 0.995 and float(g.max()) < 3.0, rate
+
+
 def test_c5_pelvis_full_size_against_oracle_subsample(pm, tables):
     """C5 (512x512x200 pelvis with Ti implants, 11033 spots, 100-230 MeV) at BASELINE's full 1e8 histories on the GPU
     (6 sub-groups of 2^24 histories, 2.1 GB of per-batch tallies); the oracle runs a 5e5-history subsample."""
