@@ -129,7 +129,7 @@ int  pmc_load_ct_host(pmc_ctx *ctx, const int16_t *hu_host, int nx, int ny, int 
 
 /* Options: "straggling" "mcs" "elastic" "nonelastic" (0/1), "s_max_wet_cm", "n_batches",
  * "chunk_histories" (histories per sub-group), "history_offset" (first history id, for sharding
- * a run over several GPUs), "dose_aggregate" (0/1 warp-aggregated dose atomics), "score_letd" (0/1, see pmc_get_letd),
+ * a run over several GPUs), "dose_aggregate" (0/1, default 0: merge the lanes of a warp that score into the same voxel before the atomic), "score_letd" (0/1, see pmc_get_letd),
  * "profile" (0/1, default 1: a CUDA-event pair is recorded on the context's stream around every kernel launch and
  * resolved into pmc_timing at the end of the call; no extra synchronisation). */
 int  pmc_set_option(pmc_ctx *ctx, const char *key, double value);

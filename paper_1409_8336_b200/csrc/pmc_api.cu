@@ -72,7 +72,7 @@ struct pmc_ctx {
   std::vector<double> h_lnR, h_lnR2, h_lnrlo, h_lnrhi, h_lnE, h_lnE2, h_sne, h_sel, h_mass, h_ek, h_ec;
   std::vector<int> ez, ea;
   double e_cut = 0.1, highland = 1.07, kappa_g = 10, s_max = 0.2; int n_batches = 10;
-  bool opt_strag = true, opt_mcs = true, opt_el = true, opt_ne = true; int aggregate = 1; bool profile = true;
+  bool opt_strag = true, opt_mcs = true, opt_el = true, opt_ne = true; int aggregate = 0; bool profile = true;
   uint64_t chunk = 1u << 24, history_offset = 0;
   std::vector<HostMat> mats;
   // device tables

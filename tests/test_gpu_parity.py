@@ -540,9 +540,9 @@ def test_streams_are_schedule_independent(pm, tables):
     pm.set_option("chunk_histories", 1000.0)
     d1, _ = pm.simulate(w["spots"], n, 77); c1 = pm.counters()
     pm.set_option("chunk_histories", float(1 << 21))
-    pm.set_option("dose_aggregate", 0.0)
+    pm.set_option("dose_aggregate", 1.0)                                  # warp-merged atomics (default: plain RED)
     d2, _ = pm.simulate(w["spots"], n, 77); c2 = pm.counters()
-    pm.set_option("dose_aggregate", 1.0)
+    pm.set_option("dose_aggregate", 0.0)
     for c in (c1, c2):
         for k in ("n_steps", "n_elastic", "n_nonelastic", "n_secondary_protons", "n_inc_tries"):
             assert c[k] == c0[k], k
