@@ -505,6 +505,25 @@ def test_simulate_edge_cases(pm, tables):
         pm.simulate(bad, 10, 1)
 
 
+def test_ragged_grid_and_clamped_hu(pm, tables):
+    """Odd, anisotropic grid (37 x 23 x 41 voxels of 1.3 x 2.1 x 1.7 mm) with HU outside the table on both sides:
+    below the first bin (-2000 -> air) and above the last (5000 -> the Ti bin, PAPER.md:L49 '>3060 = metal implant'),
+    a bone slab and a lung slab; oblique beam.  Same clamping, indexing and face logic on both sides."""
+    mats = inputs.make_materials_24()
+    nz, ny, nx = 41, 23, 37
+    hu = np.zeros((nz, ny, nx), dtype=np.int16)
+    hu[:, :, :3] = -2000; hu[10:14] = 1200; hu[14:20] = -700; hu[24:27, 8:14, 14:22] = 5000
+    vox = (0.13, 0.21, 0.17)
+    o = _setup(pm, tables, mats, hu, vox)
+    spot = inputs.plan_single_spot((2.4, 2.3, -1.0), 90.0, 0.25, direction=(0.05, 0.02, 1.0), sigma_e=0.8, div=0.004)
+    dg, sg, do, so, cg, co = _dose_parity(pm, o, hu, vox, mats, spot, 120_000, 17, check_range=False, min_pass=0.98)
+    rho = _density(hu, mats)
+    for sel in (hu == 5000, hu == 1200, hu == -700):
+        a, b = (dg * rho)[sel].sum(), (do * rho)[sel].sum()
+        assert b > 0 and abs(a / b - 1) < 1.5e-2, (a, b)
+    assert cg["e_air"] > 0 and abs(cg["e_air"] / co["e_air"] - 1) < 0.02
+
+
 def test_call_order_and_argument_errors(tables):
     from paper_1409_8336_b200 import Pmc, PmcError
     p = Pmc(0)
