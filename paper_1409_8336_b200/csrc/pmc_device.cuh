@@ -232,7 +232,13 @@ constexpr float MU_HARD = 0.5f;
 __device__ __forceinline__ float gauss_pair(uint32_t a, uint32_t b) {
   return fsqrt(-2.0f * __logf(u01(a))) * -__cosf(TWO_PI * u01(b) - 3.14159265358979f);
 }
-__device__ float straggle(const Tables &T, Rng &g, float e_start, float mean_loss, float rhoL, float zoa) {
+// `spare`: 32 random bits the caller has left over (u01() uses only the top 24 bits of a word, so the low bytes of
+// the four words of the caller's own draw block make one more word); they serve the second hard collision, so that
+// a further Philox block is needed only from the third on (1.4 % of the steps).
+__device__ __forceinline__ uint32_t low_bytes(uint4 r) {
+  return (r.x & 0xFFu) | ((r.y & 0xFFu) << 8) | ((r.z & 0xFFu) << 16) | ((r.w & 0xFFu) << 24);
+}
+__device__ float straggle(const Tables &T, Rng &g, float e_start, float mean_loss, float rhoL, float zoa, uint32_t spare) {
   if (rhoL <= 0.f || mean_loss <= 0.f) return mean_loss;
   const float gam = 1.0f + e_start * (1.0f / MP), g2m = gam * gam, b2 = 1.0f - fdiv(1.0f, g2m), bg2 = g2m - 1.0f;
   const float tmax = fdiv(2.0f * ME * bg2, 1.0f + 2.0f * gam * (ME / MP) + (ME / MP) * (ME / MP));
@@ -245,18 +251,20 @@ __device__ float straggle(const Tables &T, Rng &g, float e_start, float mean_los
   } else {
     const float itmax = fdiv(1.0f, tmax);
     const float tc0 = fminf(1e-3f, 0.01f * tmax);                            // Reading R4: Gaussian below tc0
-    float tc = fmaxf(tc0, fdiv(1.0f, fdiv(MU_HARD, xi) + itmax));
+    // kappa > 1 (the last centimetre of the range): twice as many hard collisions, the soft gamma is less skewed
+    float tc = fmaxf(tc0, fdiv(1.0f, fdiv(xi > tmax ? 2.0f * MU_HARD : MU_HARD, xi) + itmax));
     tc = fminf(tc, tmax);
     const float itc = fdiv(1.0f, tc), ltc = __logf(tmax * itc);
     const float mu_c = xi * (itc - itmax);                                   // candidates (before thinning)
     const float mean_hard = xi * (ltc - b2 * (1.0f - tc * itmax));
     // Poisson(mu_c) number of candidates by inversion with one uniform, each candidate handled as soon as the
     // inversion shows it exists.  One 32-bit word per candidate: 20 bits place it on the 1/T^2 spectrum, the other
-    // 12 decide the thinning; candidate 0 uses the last word of r, the next four one more block, ...
+    // 12 decide the thinning; candidate 0 uses the last word of r, candidate 1 the caller's spare bits, the next four
+    // one more block, ...
     float pk = __expf(-mu_c), cdf = pk; const float up = u01(r.z);
     float hard = 0.f;
-    uint4 q = make_uint4(r.w, 0u, 0u, 0u);
-    int k = 0, avail = 1;
+    uint4 q = make_uint4(r.w, spare, 0u, 0u);
+    int k = 0, avail = 2;
     while (up > cdf && k < 64) {
       if (avail == 0) { q = g.next4(); avail = 4; }
       const uint32_t w = q.x; q.x = q.y; q.y = q.z; q.z = q.w; --avail;

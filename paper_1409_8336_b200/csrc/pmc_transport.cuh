@@ -150,7 +150,7 @@ __global__ void __launch_bounds__(256) sampler_kernel(Tables T, Grid G, const Sp
         const float ef = (float)E, lnEv = logf(fminf(fmaxf(ef, T.e_min), T.e_max));
         const float lnRv = ln_range(T, T.lnR, T.lnR2, air_table, e_index(T, lnEv)), Rg = expf(lnRv);
         float loss = mean_loss(T, T.lnE, T.lnE2, air_table, ef, lnEv, lnRv, Rg, (float)L * air_wf);
-        if (T.opt_strag) loss = straggle(T, g, ef, loss, (float)L * air_rho, air_zoa);
+        if (T.opt_strag) loss = straggle(T, g, ef, loss, (float)L * air_rho, air_zoa, low_bytes(q));
         e_air = loss; E -= loss;
         if (E <= T.e_cut) { e_air += E; ok = false; }
       }
@@ -303,7 +303,7 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM) tr
       else {
         loss = mean_loss(T, s_lnE, s_lnE2, tab, e0, lnEv, lnRv, Rg, L * wf);
         let = fdiv(0.1f * loss, L);                              // keV/um of this step (Reading R9)
-        if (T.opt_strag) loss = straggle(T, g, e0, loss, L * rho, m.zoa);
+        if (T.opt_strag) loss = straggle(T, g, e0, loss, L * rho, m.zoa, low_bytes(r));
       }
       p.e = e0 - loss; dep = loss;
       bool alive = cls != 3;
