@@ -154,6 +154,16 @@ class Oracle:
                                          C.c_uint64(n_histories), C.c_uint64(seed), _dp(dose), _dp(sigma)))
         return dose.reshape(self.shape), sigma.reshape(self.shape)
 
+    def set_dose_influence(self, roi_voxels):
+        roi = np.ascontiguousarray(roi_voxels, dtype=np.int32)
+        self.n_roi = int(roi.size)
+        self._chk(self.lib.opmc_set_dose_influence(self.ctx, roi.ctypes.data_as(C.POINTER(C.c_int32)), C.c_int(self.n_roi)))
+
+    def dose_influence(self, nspots):
+        out = np.zeros((nspots, self.n_roi), dtype=np.float64)
+        self._chk(self.lib.opmc_get_dose_influence(self.ctx, _dp(out)))
+        return out
+
     def letd(self):
         """LET_d map (keV/um) of the last simulate() made with set_option("score_letd", 1)."""
         out = np.zeros(self.shape, dtype=np.float64)

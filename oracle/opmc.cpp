@@ -495,6 +495,8 @@ struct opmc_ctx {
   std::vector<Nucleus> nuc;                   // per element (A > 1)
   std::vector<int16_t> hu; int nx = 0, ny = 0, nz = 0; double d[3] = {0, 0, 0}, org[3] = {0, 0, 0};
   bool opt_strag = true, opt_mcs = true, opt_el = true, opt_ne = true; int threads = 0;
+  // per-spot dose influence on a list of ROI voxels (Reading R11)
+  std::vector<int32_t> roi_vox, roi_map; std::vector<double> dij; int dij_spots = 0;
   bool score_let = false; std::vector<double> let_num, let_den;   // LET_d tallies (Reading R9)
   opmc_counters cnt{};
   std::string err;
@@ -502,7 +504,7 @@ struct opmc_ctx {
 
 namespace {
 
-struct Particle { V3 r, d; double E; int idx[3]; uint32_t pid; uint32_t block0; };
+struct Particle { V3 r, d; double E; int idx[3]; uint32_t pid; uint32_t block0; int spot = 0; };
 struct Ledger { double dep = 0, esc = 0, neu = 0, gam = 0, q = 0, air = 0; };
 
 const Material &material_of(const opmc_ctx *c, int hu) {
@@ -551,6 +553,15 @@ inline double highland(const Tables &T, double e, double rhoL, double x0) {   //
   if (rhoL <= 0) return 0;
   double pc = std::sqrt(e * (e + 2 * MP)), bcp = pc * pc / (e + MP), t = rhoL / x0;
   return T.highland * 13.6 / bcp * std::sqrt(t) * std::max(0.0, 1 + 0.038 * std::log(t));
+}
+
+// energy e (MeV) deposited in voxel vox by a history of spot `spot` -> row spot, column roi_map[vox] of the influence matrix
+inline void score_influence(opmc_ctx *c, int spot, size_t vox, double e) {
+  if (c->roi_map.empty() || e == 0) return;
+  const int32_t j = c->roi_map[vox];
+  if (j < 0) return;
+  #pragma omp atomic
+  c->dij[(size_t)spot * c->roi_vox.size() + j] += e;
 }
 
 struct StepResult { int cls; double L; };    // cls: 0 none, 1 boundary, 2 nuclear, 3 range-out
@@ -612,6 +623,7 @@ bool transport_step(opmc_ctx *c, Particle &p, Rng &g, double *tally, Ledger &led
   #pragma omp atomic
   tally[vox] += dep;
   led.dep += dep;
+  score_influence(c, p.spot, vox, dep);
   if (c->score_let && dep > 0 && L > 0) {
     // dose-averaged LET (Reading R9): every proton step weighs its LET, the table's mean energy loss
     // over the step divided by the step length (keV/um = 0.1 MeV/cm; a proton that ranges out: its energy over its
@@ -644,6 +656,7 @@ bool transport_step(opmc_ctx *c, Particle &p, Rng &g, double *tally, Ledger &led
     #pragma omp atomic
     tally[vox] += e;
     led.dep += e;
+    score_influence(c, p.spot, vox, e);
   };
   // NB: the event voxel is the START voxel of the step (interior end point => same voxel)
   if (is_el) {
@@ -690,6 +703,7 @@ bool sample_primary(opmc_ctx *c, const opmc_spot *spots, const std::vector<doubl
   double u = g.u(); int s = (int)(std::lower_bound(cdf.begin(), cdf.end(), u) - cdf.begin());
   if (s >= (int)cdf.size()) s = (int)cdf.size() - 1;
   const opmc_spot &sp = spots[s];
+  p.spot = s;
   V3 ax = unit(V3{sp.dir[0], sp.dir[1], sp.dir[2]});
   V3 a = std::fabs(ax.z) >= 0.9 ? V3{0, 1, 0} : V3{0, 0, 1};
   V3 ex = unit(cross(a, ax)), ey = cross(ax, ex);
@@ -856,6 +870,7 @@ int opmc_load_ct(opmc_ctx *c, const int16_t *hu, int nx, int ny, int nz, double 
   c->nx = nx; c->ny = ny; c->nz = nz; c->d[0] = dx; c->d[1] = dy; c->d[2] = dz;
   for (int k = 0; k < 3; ++k) c->org[k] = origin ? origin[k] : 0.0;
   c->hu.assign(hu, hu + (size_t)nx * ny * nz);
+  c->roi_vox.clear(); c->roi_map.clear(); c->dij.clear();
   return 0;
 }
 
@@ -878,6 +893,8 @@ int opmc_simulate(opmc_ctx *c, const opmc_spot *spots, int nspots, uint64_t n, u
   std::vector<double> cdf = spot_cdf(spots, nspots), tally(nv), s1(nv, 0.0), s2(nv, 0.0);
   c->cnt = opmc_counters{};
   if (c->score_let) { c->let_num.assign(nv, 0.0); c->let_den.assign(nv, 0.0); }
+  c->dij_spots = nspots;
+  if (!c->roi_map.empty()) c->dij.assign((size_t)nspots * c->roi_vox.size(), 0.0);
 #ifdef _OPENMP
   if (c->threads > 0) omp_set_num_threads(c->threads);
 #endif
@@ -902,6 +919,12 @@ int opmc_simulate(opmc_ctx *c, const opmc_spot *spots, int nspots, uint64_t n, u
       s1[v] += db; s2[v] += db * db;
     }
   }
+  // influence matrix: MeV -> Gy per primary history of the call (rows then add up to the dose when B divides n)
+  for (size_t i = 0; !c->roi_map.empty() && i < (size_t)nspots; ++i)
+    for (size_t j = 0; j < c->roi_vox.size(); ++j) {
+      int hu = c->hu[c->roi_vox[j]]; const Material &m = material_of(c, hu);
+      c->dij[i * c->roi_vox.size() + j] *= MEV_PER_G_TO_GY / (density(m, hu) * c->d[0] * c->d[1] * c->d[2] * (double)n);
+    }
   for (size_t v = 0; v < nv; ++v) {                  // PAPER.md:L138 "total and RMS dose" (Reading R8)
     double mean = s1[v] / B, var = (s2[v] - B * mean * mean) / ((double)B * (B - 1));
     dose[v] = mean; sigma[v] = var > 0 ? std::sqrt(var) : 0.0;
@@ -934,6 +957,29 @@ int opmc_nonelastic(opmc_ctx *c, int Z, int A, double e, uint64_t n, uint64_t se
   off[n] = (uint32_t)pos; *n_out = pos;
   c->cnt.n_nonelastic = n; c->cnt.n_inc_tries = chk.inc_tries; c->cnt.max_event_residual = chk.max_resid; c->cnt.n_zab_violations = chk.zab_bad;
   if (overflow) return fail(c, "capacity too small"), -3;
+  return 0;
+}
+
+// Per-spot dose influence ("MC-based IMPT optimisation"; Reading R11): roi_voxels = n_roi linear voxel
+// indices (x fastest); the next opmc_simulate calls also fill D[spot][roi] = dose (Gy per primary history of the call)
+// that histories of that spot give to that voxel.  n_roi = 0 switches it off.
+int opmc_set_dose_influence(opmc_ctx *c, const int32_t *roi_voxels, int n_roi) {
+  if (!c || n_roi < 0 || (n_roi > 0 && !roi_voxels)) return fail(c, "bad argument");
+  if (c->hu.empty()) return fail(c, "load the CT first");
+  c->roi_vox.clear(); c->roi_map.clear(); c->dij.clear();
+  if (n_roi == 0) return 0;
+  c->roi_map.assign(c->hu.size(), -1);
+  for (int j = 0; j < n_roi; ++j) {
+    if (roi_voxels[j] < 0 || (size_t)roi_voxels[j] >= c->hu.size() || c->roi_map[roi_voxels[j]] >= 0) { c->roi_map.clear(); return fail(c, "ROI voxel out of range or repeated"); }
+    c->roi_map[roi_voxels[j]] = j;
+  }
+  c->roi_vox.assign(roi_voxels, roi_voxels + n_roi);
+  return 0;
+}
+int opmc_get_dose_influence(opmc_ctx *c, double *out) {
+  if (!c || !out) return -1;
+  if (c->roi_vox.empty() || c->dij.size() != (size_t)c->dij_spots * c->roi_vox.size() || c->dij.empty()) return fail(c, "no influence matrix: set the ROI and simulate");
+  std::memcpy(out, c->dij.data(), c->dij.size() * sizeof(double));
   return 0;
 }
 

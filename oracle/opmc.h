@@ -87,6 +87,9 @@ int  opmc_simulate(opmc_ctx *, const opmc_spot *spots, int nspots, uint64_t n_hi
 int  opmc_nonelastic(opmc_ctx *, int Z, int A, double e_mev, uint64_t n, uint64_t seed,
                      opmc_secondary *out, uint64_t capacity, uint32_t *event_offsets, uint64_t *n_out);
 int  opmc_get_counters(opmc_ctx *, opmc_counters *);
+/* PAPER.md:L270 (Reading R11): per-spot dose influence on a list of ROI voxels; see opmc.cpp. out: nspots*n_roi doubles. */
+int  opmc_set_dose_influence(opmc_ctx *, const int32_t *roi_voxels, int n_roi);
+int  opmc_get_dose_influence(opmc_ctx *, double *out);
 /* PAPER.md:L282 (Reading R9): dose-averaged LET of the last opmc_simulate call made with option "score_letd" = 1;
  * out: nx*ny*nz doubles, keV/um, 0 where no proton step deposited energy. */
 int  opmc_get_letd(opmc_ctx *, double *out);

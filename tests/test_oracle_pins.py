@@ -585,3 +585,45 @@ def test_letd_invariants_full_physics(oracle_c1):
         for k in ("straggling", "mcs", "elastic", "nonelastic"):
             o.set_option(k, 1)
         o.set_option("score_letd", 0)
+
+
+# ------------------------------------------------------------------ per-spot dose influence (Reading R11)
+def _two_spot_plan():
+    a = inputs.plan_single_spot((3.0, 5.0, 0.0), 100.0, 0.3)
+    b = inputs.plan_single_spot((7.0, 5.0, 0.0), 150.0, 0.3)
+    c = inputs.plan_single_spot((5.0, 5.0, 0.0), 120.0, 0.3)
+    s = np.concatenate([a, b, c]); s[:, 12] = [1.0, 2.0, 0.0]               # the third spot has zero weight
+    return s
+
+
+def test_dose_influence_rows_add_up_to_the_dose(oracle_c1):
+    """Exact bookkeeping identity: every deposit of a history goes to its spot's row, so the rows of D add up to the
+    dose in each ROI voxel (n divisible by the number of batches); a zero-weight spot gets an all-zero row; two beams
+    4 cm apart do not reach each other's axis; the rows scale with the spot weights (2/3 of the histories -> 150 MeV)."""
+    hu, vox = inputs.phantom_c1()
+    o = oracle_c1
+    o.load_ct(hu, vox)
+    nz, ny, nx = hu.shape
+    # ROI: the two beam axes and a transverse line through both, deliberately unordered
+    zs = np.arange(nz)
+    roi = np.concatenate([(zs * ny + 25) * nx + 15, (zs * ny + 25) * nx + 35, (20 * ny + 25) * nx + np.arange(0, 50, 3)[::-1]])
+    roi = np.unique(roi)[::-1].copy()
+    spots = _two_spot_plan()
+    n = 20000
+    o.set_dose_influence(roi)
+    try:
+        dose, _ = o.simulate(spots, n, 9)
+        D = o.dose_influence(3)
+    finally:
+        o.set_dose_influence(np.zeros(0, dtype=np.int32))
+    assert D.shape == (3, roi.size) and np.all(D >= 0) and np.all(D[2] == 0)
+    assert np.allclose(D.sum(axis=0), dose.ravel()[roi], rtol=1e-10, atol=1e-300)
+    on_a = np.isin(roi, (zs * ny + 25) * nx + 15); on_b = np.isin(roi, (zs * ny + 25) * nx + 35)
+    assert D[0][on_a].sum() > 100 * D[0][on_b].sum() and D[1][on_b].sum() > 100 * D[1][on_a].sum()
+    # entrance dose per history is ~S(E)/area: row sums at z = 0..10 scale like weight x S: S(100)/S(150) = 7.290/5.445
+    ent_a = D[0][on_a & (roi // (nx * ny) < 10)].sum(); ent_b = D[1][on_b & (roi // (nx * ny) < 10)].sum()
+    assert abs((ent_b / ent_a) / (2.0 * 5.445 / 7.290) - 1) < 0.08
+    with pytest.raises(Exception):
+        o.dose_influence(3)                                               # switched off again
+    with pytest.raises(Exception):
+        o.set_dose_influence(np.array([0, 0], dtype=np.int32))            # repeated voxel
