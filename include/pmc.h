@@ -154,6 +154,17 @@ int  pmc_simulate_host(pmc_ctx *ctx, const pmc_spot *spots_host, int nspots, uin
 int  pmc_nonelastic(pmc_ctx *ctx, int Z, int A, double e_mev, uint64_t n, uint64_t seed,
                     pmc_secondary *out_dev, uint64_t capacity, uint32_t *event_offsets_dev, uint64_t *n_out_host);
 
+/* PAPER.md:L270 ("MC-based IMPT optimisation" needs the dose of every spot separately; Reading R11):
+ * per-spot dose influence on a list of region-of-interest voxels.  roi_voxels_host: HOST array of n_roi distinct linear
+ * voxel indices (x fastest) of the loaded CT, copied; dij_dev: DEVICE array of dij_capacity floats, caller-owned and
+ * borrowed until the next pmc_set_dose_influence / pmc_load_ct / pmc_destroy.  Every following pmc_simulate call also
+ * overwrites dij_dev[spot * n_roi + k] with the dose (Gy per primary history of the call) that the histories of that
+ * spot, with all their secondaries and local deposits, give to voxel roi_voxels[k]; the rows add up to the dose in
+ * that voxel (exactly so when n_batches divides n_histories).  n_roi = 0 switches it off.
+ * Errors: PMC_E_STATE (no CT), PMC_E_INVALID_ARG (index out of range or repeated, null pointers); pmc_simulate returns
+ * PMC_E_CAPACITY if nspots * n_roi exceeds dij_capacity. */
+int  pmc_set_dose_influence(pmc_ctx *ctx, const int32_t *roi_voxels_host, int n_roi, float *dij_dev, uint64_t dij_capacity);
+
 /* PAPER.md:L282 (Fig 9; Reading R9): dose-averaged LET scored "simultaneously" with the dose.  With option
  * "score_letd" = 1, pmc_simulate also tallies, for every step of every proton (primaries and secondaries; heavy
  * recoils and fragments do not enter, L282), e x LET and e per voxel, where e is the energy the step deposits and LET

@@ -19,7 +19,7 @@ _I = C.POINTER(C.c_int32)
 
 EXPORTS = ["pmc_create", "pmc_destroy", "pmc_load_physics_tables", "pmc_set_hu_materials", "pmc_load_ct",
            "pmc_load_ct_host", "pmc_set_option", "pmc_simulate", "pmc_simulate_host", "pmc_nonelastic",
-           "pmc_get_counters", "pmc_get_timing", "pmc_get_letd", "pmc_gamma_index", "pmc_last_error", "pmc_philox4x32_10", "pmc_range_of_energy",
+           "pmc_get_counters", "pmc_get_timing", "pmc_get_letd", "pmc_gamma_index", "pmc_set_dose_influence", "pmc_last_error", "pmc_philox4x32_10", "pmc_range_of_energy",
            "pmc_energy_of_range", "pmc_straggle", "pmc_elastic", "pmc_first_steps"]
 
 
@@ -179,6 +179,19 @@ class Pmc:
         self._chk(self.lib.pmc_simulate_host(self.ctx, spots.ctypes.data_as(C.c_void_p), C.c_int(spots.shape[0]),
                                              C.c_uint64(n_histories), C.c_uint64(seed),
                                              dose_host.ctypes.data_as(C.c_void_p), sigma_host.ctypes.data_as(C.c_void_p)))
+
+    def set_dose_influence(self, roi_voxels, nspots):
+        """Score D[spot][roi] (Gy per primary) in the following simulate() calls; returns the CUDA tensor (nspots, n_roi)
+        the library writes into.  roi_voxels: linear voxel indices (x fastest); an empty list switches it off."""
+        roi = np.ascontiguousarray(roi_voxels, dtype=np.int32)
+        if roi.size == 0:
+            self._chk(self.lib.pmc_set_dose_influence(self.ctx, None, C.c_int(0), None, C.c_uint64(0)))
+            self._dij = None
+            return None
+        self._dij = self.torch.zeros((int(nspots), int(roi.size)), dtype=self.torch.float32, device=self.device)
+        self._chk(self.lib.pmc_set_dose_influence(self.ctx, roi.ctypes.data_as(C.c_void_p), C.c_int(roi.size), _ptr(self._dij),
+                                                  C.c_uint64(self._dij.numel())))
+        return self._dij
 
     def letd(self, out=None):
         """-> LET_d map (keV/um), CUDA float32 tensor (nz, ny, nx), of the last simulate() with score_letd = 1."""

@@ -85,6 +85,7 @@ struct pmc_ctx {
   QueueMem qa, qb, qev, qel, qne, qres; DevBuf<uint32_t> d_resza; DevBuf<float> d_resp;
   DevBuf<uint32_t> d_head; DevBuf<Counters> d_cnt; DevBuf<float> d_tally, d_out, d_let;
   bool score_let = false, have_let = false;
+  DevBuf<int32_t> d_roimap, d_roivox; uint32_t n_roi = 0; float *dij_dev = nullptr; uint64_t dij_cap = 0;
   DevBuf<SpotDev> d_spots; DevBuf<double> d_cdf;
   DevBuf<SecRec> d_slots; DevBuf<uint32_t> d_counts; DevBuf<unsigned long long> d_base; DevBuf<ResRec> d_res;
   DevBuf<GammaOffset> d_goff; DevBuf<unsigned long long> d_gscr;
@@ -333,7 +334,7 @@ int load_ct_common(pmc_ctx *c, const int16_t *hu_dev, int nx, int ny, int nz, do
   c->G.vol = (float)(dx * dy * dz);
   for (int k = 0; k < 3; ++k) c->G.d[k] = (float)(k == 0 ? dx : k == 1 ? dy : dz);
   for (int k = 0; k < 3; ++k) c->origin[k] = origin ? origin[k] : 0.0;   // applied on the host to the spot positions
-  c->have_ct = true;
+  c->have_ct = true; c->n_roi = 0; c->dij_dev = nullptr;      // a ROI belongs to the grid it was given for
   return PMC_OK;
 }
 
@@ -363,7 +364,7 @@ void pmc_destroy(pmc_ctx *c) {
   c->d_sigbin.release(); c->d_ek.release(); c->d_ec.release(); c->d_mass.release(); c->d_bins.release(); c->d_lut.release();
   c->d_nuc.release(); c->d_nuc1.release(); c->d_hu_own.release();
   c->qa.release(); c->qb.release(); c->qev.release(); c->qel.release(); c->qne.release(); c->qres.release(); c->d_resza.release(); c->d_resp.release();
-  c->d_head.release(); c->d_cnt.release(); c->d_tally.release(); c->d_out.release(); c->d_let.release();
+  c->d_head.release(); c->d_cnt.release(); c->d_tally.release(); c->d_out.release(); c->d_let.release(); c->d_roimap.release(); c->d_roivox.release();
   c->d_spots.release(); c->d_cdf.release(); c->d_res.release(); c->d_goff.release(); c->d_gscr.release(); c->d_slots.release(); c->d_counts.release(); c->d_base.release();
   if (c->h_pinned) cudaFreeHost(c->h_pinned);
   if (c->ev[0]) { cudaEventDestroy(c->ev[0]); cudaEventDestroy(c->ev[1]); }
@@ -500,6 +501,12 @@ static int simulate_impl(pmc_ctx *c, const pmc_spot *spots_in, int nspots, uint6
   CK(c->d_tally.alloc(nvox_s * B));
   cudaStream_t s = c->stream;
   CK(cudaMemsetAsync(c->d_tally.p, 0, nvox_s * B * 4, s)); CK(cudaMemsetAsync(c->d_cnt.p, 0, sizeof(Counters), s));
+  const bool roi_on = c->n_roi > 0 && !dbg_out;
+  if (roi_on) {
+    if (nspots >= (1 << 24)) return fail(c, PMC_E_UNSUPPORTED, "dose influence: at most 2^24 - 1 spots");
+    if ((uint64_t)nspots * c->n_roi > c->dij_cap) return fail(c, PMC_E_CAPACITY, "dose influence: nspots x n_roi exceeds the capacity of dij_dev");
+    CK(cudaMemsetAsync(c->dij_dev, 0, (size_t)nspots * c->n_roi * 4, s));
+  }
   const bool let_on = c->score_let && !dbg_out;
   c->have_let = false;
   if (let_on) { CK(c->d_let.alloc(2 * nvox_s)); CK(cudaMemsetAsync(c->d_let.p, 0, 2 * nvox_s * 4, s)); }
@@ -514,6 +521,7 @@ static int simulate_impl(pmc_ctx *c, const pmc_spot *spots_in, int nspots, uint6
     const uint32_t nc = (uint32_t)std::min<uint64_t>(chunk, n - cs);
     RunParams P{}; P.seed = seed; P.hist0 = c->history_offset + cs; P.n = nc; P.max_steps = max_steps; P.dbg_out = dbg_out ? dbg_out + 8ull * cs : nullptr;
     P.aggregate = c->aggregate; P.local0 = cs; P.n_total = n; P.B = (uint32_t)B; P.nvox = nvox;
+    P.roi_map = roi_on ? c->d_roimap.p : nullptr; P.dij = roi_on ? c->dij_dev : nullptr; P.n_roi = roi_on ? c->n_roi : 0u;
     P.let_num = let_on ? c->d_let.p : nullptr; P.let_den = let_on ? c->d_let.p + nvox_s : nullptr;
     P.b_over_n = (float)((double)B / (double)n); P.inv_nx = 1.0f / (float)c->G.nx; P.inv_ny = 1.0f / (float)c->G.ny;
     CK(cudaMemsetAsync(c->qa.q.count, 0, 4, s));
@@ -529,6 +537,8 @@ static int simulate_impl(pmc_ctx *c, const pmc_spot *spots_in, int nspots, uint6
       stats_kernel<<<grid_v, 256, 0, s>>>(c->T, c->G, c->d_tally.p, dose_dev, sigma_dev, B, n, nvox); }
     c->timing.launches_total++;
   }
+  if (roi_on && n > 0)
+    influence_finish_kernel<<<grid_v, 256, 0, s>>>(c->T, c->G, c->d_roivox.p, c->n_roi, (uint32_t)nspots, (float)(1.0 / (double)n), c->dij_dev);
   CK(cudaEventRecord(e1, s));
   CK(cudaGetLastError());
   rc = fetch_counters(c);
@@ -600,6 +610,24 @@ int pmc_nonelastic(pmc_ctx *c, int Z, int A, double e_mev, uint64_t n, uint64_t 
   rc = fetch_counters(c); if (rc) return rc;
   c->counters.n_nonelastic = n;
   if (total > capacity) return fail(c, PMC_E_CAPACITY, "capacity too small");
+  return PMC_OK;
+}
+
+int pmc_set_dose_influence(pmc_ctx *c, const int32_t *roi_voxels_host, int n_roi, float *dij_dev, uint64_t dij_capacity) {
+  if (!c || n_roi < 0) return fail(c, PMC_E_INVALID_ARG, "bad argument");
+  if (n_roi == 0) { c->n_roi = 0; c->dij_dev = nullptr; c->dij_cap = 0; return PMC_OK; }
+  if (!roi_voxels_host || !dij_dev || dij_capacity < (uint64_t)n_roi) return fail(c, PMC_E_INVALID_ARG, "null ROI list / output, or capacity below one row");
+  if (!c->have_ct) return fail(c, PMC_E_STATE, "load the CT first");
+  cudaSetDevice(c->device);
+  const size_t nvox = (size_t)c->G.nx * c->G.ny * c->G.nz;
+  std::vector<int32_t> map(nvox, -1), vox(roi_voxels_host, roi_voxels_host + n_roi);
+  for (int j = 0; j < n_roi; ++j) {
+    if (vox[j] < 0 || (size_t)vox[j] >= nvox || map[vox[j]] >= 0) return fail(c, PMC_E_INVALID_ARG, "ROI voxel out of range or repeated");
+    map[vox[j]] = j;
+  }
+  CK(c->d_roimap.upload(map, c->stream)); CK(c->d_roivox.upload(vox, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  c->n_roi = (uint32_t)n_roi; c->dij_dev = dij_dev; c->dij_cap = dij_capacity;
   return PMC_OK;
 }
 

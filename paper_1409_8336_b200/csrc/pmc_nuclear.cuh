@@ -336,7 +336,7 @@ __device__ __forceinline__ void evap_machine(const Tables &T, uint32_t n, uint32
 }
 
 // ------------------------------------------------------------------ event-queue kernels of the transport scheduler
-struct ResQueue { Queue q; uint32_t *za; float *px, *py, *pz; };   // q.e = E*, q.aux = next product index
+struct ResQueue { Queue q; uint32_t *za; float *px, *py, *pz; };   // q.e = E*, q.aux = spot << 8 | next product index
 
 // K3: intranuclear cascades over the non-elastic queue (PAPER.md:L128(3), L136), one event per lane at a time
 __global__ void __launch_bounds__(128) inc_kernel(Tables T, RunParams P, Queue in, uint32_t *head, Queue out, ResQueue rq,
@@ -347,10 +347,10 @@ __global__ void __launch_bounds__(128) inc_kernel(Tables T, RunParams P, Queue i
   auto load = [&](uint32_t i, const Nucleus *&N, float &t_in, Rng &g) {
     p = queue_load(in, i);
     g.init(P.seed, P.hist0 + p.hist, p.pid, p.blk);
-    N = &T.nuc[p.aux]; t_in = p.e;
+    N = &T.nuc[aux_low(p.aux)]; t_in = p.e;
   };
   auto store = [&](uint32_t, Rng &g, const OutNuc *outn, int n_out, const Residual &R) {
-    const Nucleus &N = T.nuc[p.aux];
+    const Nucleus &N = T.nuc[aux_low(p.aux)];
     float dep = 0.f; uint32_t kchild = 0; double msum = 0;
     for (int k = 0; k < n_out; ++k) {
       const OutNuc &o = outn[k];
@@ -358,13 +358,13 @@ __global__ void __launch_bounds__(128) inc_kernel(Tables T, RunParams P, Queue i
       if (o.type == 0) {                                                   // L79: only protons are followed
         if (o.ke > T.e_cut) {
           Particle s = p; s.d = unit(to_lab(p.d, o.dir.x, o.dir.y, o.dir.z)); s.e = o.ke;
-          s.pid = g.child_id(kchild++); s.blk = 0u; s.aux = 0u; c_sec++;
+          s.pid = g.child_id(kchild++); s.blk = 0u; s.aux = aux_with(p.aux, 0u); c_sec++;
           if (!queue_push(out, s)) atomicOr(&cnt->overflow, 16u);
         } else dep += o.ke;
       } else c_neu += (double)o.ke;                                        // neutrons: not transported
     }
     c_q += msum + R.mass_gs - MP_D - N.mass;
-    if (dep != 0.f) { atomicAdd(tally + batch_base(P, p.hist) + (uint32_t)p.vox, dep); c_dep += (double)dep; }
+    if (dep != 0.f) { atomicAdd(tally + batch_base(P, p.hist) + (uint32_t)p.vox, dep); c_dep += (double)dep; score_influence(P, p.aux, p.vox, dep); }
     // residual -> evaporation queue (keeps the event frame: p.d is the incident direction)
     const uint32_t slot = warp_alloc(rq.q.count);
     if (slot >= rq.q.cap) atomicOr(&cnt->overflow, 32u);
@@ -372,7 +372,7 @@ __global__ void __launch_bounds__(128) inc_kernel(Tables T, RunParams P, Queue i
       const Queue &q = rq.q;
       q.x[slot] = p.r.x; q.y[slot] = p.r.y; q.z[slot] = p.r.z; q.u[slot] = p.d.x; q.v[slot] = p.d.y; q.w[slot] = p.d.z;
       q.e[slot] = (float)R.estar; q.vox[slot] = p.vox; q.hist[slot] = p.hist; q.pid[slot] = p.pid; q.blk[slot] = g.blk;
-      q.aux[slot] = kchild; rq.za[slot] = ((uint32_t)R.Z << 16) | (uint32_t)R.A;
+      q.aux[slot] = aux_with(p.aux, kchild); rq.za[slot] = ((uint32_t)R.Z << 16) | (uint32_t)R.A;
       rq.px[slot] = (float)R.P[0]; rq.py[slot] = (float)R.P[1]; rq.pz[slot] = (float)R.P[2];
     }
   };
@@ -392,14 +392,14 @@ __global__ void __launch_bounds__(128) evap_kernel(Tables T, RunParams P, ResQue
     g.init(P.seed, P.hist0 + p.hist, p.pid, p.blk);
     R.Z = (int)(rq.za[i] >> 16); R.A = (int)(rq.za[i] & 0xffffu); R.estar = (double)p.e;
     R.P[0] = rq.px[i]; R.P[1] = rq.py[i]; R.P[2] = rq.pz[i]; R.mass_gs = nmass(T, R.Z, R.A);
-    m0 = R.mass_gs; msum = 0; kchild = p.aux; dep = 0.f;
+    m0 = R.mass_gs; msum = 0; kchild = aux_low(p.aux); dep = 0.f;
   };
   auto emit = [&](uint32_t, Rng &g, const Emission &em) {
     msum += nmass(T, EJ_Z[em.j], EJ_A[em.j]);
     if (em.j == 1) {
       if (em.ke > T.e_cut) {
         Particle s = p; s.d = unit(to_lab(p.d, em.dir.x, em.dir.y, em.dir.z)); s.e = em.ke;
-        s.pid = g.child_id(kchild++); s.blk = 0u; s.aux = 0u; c_sec++;
+        s.pid = g.child_id(kchild++); s.blk = 0u; s.aux = aux_with(p.aux, 0u); c_sec++;
         if (!queue_push(out, s)) atomicOr(&cnt->overflow, 64u);
       } else dep += em.ke;
     } else if (em.j == 0) c_neu += (double)em.ke;
@@ -410,7 +410,7 @@ __global__ void __launch_bounds__(128) evap_kernel(Tables T, RunParams P, ResQue
     if (R.A == 1 && R.Z == 0) c_neu += kres; else dep += (float)kres;
     c_gam += R.estar;                                                       // L79: no photon evaporation
     c_q += msum + R.mass_gs - m0;
-    if (dep != 0.f) { atomicAdd(tally + batch_base(P, p.hist) + (uint32_t)p.vox, dep); c_dep += (double)dep; }
+    if (dep != 0.f) { atomicAdd(tally + batch_base(P, p.hist) + (uint32_t)p.vox, dep); c_dep += (double)dep; score_influence(P, p.aux, p.vox, dep); }
   };
   evap_machine(T, n, head, load, emit, done);
   flush(&cnt->e_deposit, c_dep); flush(&cnt->e_neutron, c_neu); flush(&cnt->e_q, c_q); flush(&cnt->e_gamma, c_gam);

@@ -19,9 +19,22 @@ struct RunParams {
   uint32_t B, nvox;
   float b_over_n, inv_nx, inv_ny;     // B / n_total, 1 / nx, 1 / ny
   float *let_num, *let_den;           // LET_d tallies [nvox] (Reading R9) or nullptr
+  // per-spot dose influence (Reading R11): roi_map[vox] = column or -1, dij[spot][column] in MeV
+  const int32_t *roi_map; float *dij; uint32_t n_roi;
   int max_steps; float *dbg_out;      // pmc_first_steps: stop after max_steps, write [hist][8]
   int aggregate;                      // warp-aggregated dose atomics
 };
+
+// The queue word `aux` carries the spot index of the history in its upper 24 bits through every generation; the low
+// byte is the target element (event queues) or the next product index (residual queue).
+__device__ __forceinline__ uint32_t aux_spot(uint32_t a) { return a >> 8; }
+__device__ __forceinline__ uint32_t aux_low(uint32_t a) { return a & 0xFFu; }
+__device__ __forceinline__ uint32_t aux_with(uint32_t a, uint32_t low) { return (a & ~0xFFu) | (low & 0xFFu); }
+__device__ __forceinline__ void score_influence(const RunParams &P, uint32_t aux, int vox, float e) {
+  if (P.roi_map == nullptr || e == 0.f) return;
+  const int32_t j = P.roi_map[vox];
+  if (j >= 0) atomicAdd(P.dij + (size_t)aux_spot(aux) * P.n_roi + (uint32_t)j, e);
+}
 
 // floor(h B / n_total) * nvox without a 64-bit division: float estimate, exact correction
 __device__ __forceinline__ uint32_t batch_base(const RunParams &P, uint32_t hist) {
@@ -166,7 +179,7 @@ __global__ void __launch_bounds__(256) sampler_kernel(Tables T, Grid G, const Sp
       }
       p.r = {loc[0], loc[1], loc[2]}; p.d = unit(V3{(float)dir[0], (float)dir[1], (float)dir[2]}); p.e = (float)E;
       p.vox = (idx[2] * G.ny + idx[1]) * G.nx + idx[0];
-      p.hist = i; p.pid = 0u; p.blk = g.blk; p.aux = 0u;
+      p.hist = i; p.pid = 0u; p.blk = g.blk; p.aux = (uint32_t)lo << 8;
       if (!queue_push(out, p)) atomicOr(&cnt->overflow, 1u);
     }
   }
@@ -336,6 +349,7 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM) tr
       }
     }
     deposit(tally, tbase + (uint32_t)dep_vox, dep, dep != 0.f, P.aggregate, P.let_num, P.let_den, (uint32_t)dep_vox, let > 0.f ? dep : 0.f, let);
+    if (P.roi_map != nullptr && dep != 0.f) score_influence(P, p.aux, dep_vox, dep);
   }
   flush(&cnt->n_steps, c_steps); (void)c_ev;
   flush(&cnt->e_deposit, c_dep); flush(&cnt->e_escape, c_esc);
@@ -376,7 +390,7 @@ __global__ void __launch_bounds__(256) event_kernel(Tables T, Grid G, RunParams 
           const float w = is_el ? pel[e] : pne[e];
           if (w > 0.f && (el < 0 || u >= 0.f)) { el = e; u -= w; }
         }
-        p.aux = (uint32_t)el; p.blk = g.blk;
+        p.aux = aux_with(p.aux, (uint32_t)el); p.blk = g.blk;
         if (is_el) { c_el++; if (!queue_push(q_el, p)) atomicOr(&cnt->overflow, 2u); }
         else { c_ne++; if (!queue_push(q_ne, p)) atomicOr(&cnt->overflow, 4u); }
       } else if (!queue_push(next, p)) atomicOr(&cnt->overflow, 8u);
@@ -430,24 +444,24 @@ __global__ void __launch_bounds__(256) elastic_kernel(Tables T, RunParams P, Que
     if (i < n) {
       Particle p = queue_load(in, i);
       Rng g; g.init(P.seed, P.hist0 + p.hist, p.pid, p.blk);
-      const int el = (int)p.aux, Z = T.elem_z[el], A = T.elem_a[el];
+      const int el = (int)aux_low(p.aux), Z = T.elem_z[el], A = T.elem_a[el];
       const float M = (float)T.mass[Z * T.adim + A];
       const ElasticOut o = elastic_event(A, M, p.e, g.next4());
       const V3 d0 = p.d;
       float dep = 0.f;
       Particle s = p;
-      p.d = unit(to_lab(d0, o.dir_out.x, o.dir_out.y, o.dir_out.z)); p.e = o.T_out; p.aux = 0u;
+      p.d = unit(to_lab(d0, o.dir_out.x, o.dir_out.y, o.dir_out.z)); p.e = o.T_out; p.aux = aux_with(p.aux, 0u);
       bool push_rec = false;
       if (A == 1 && o.T_rec > T.e_cut) {
         s.d = unit(to_lab(d0, o.dir_rec.x, o.dir_rec.y, o.dir_rec.z)); s.e = o.T_rec;
-        s.pid = g.child_id(0u); s.blk = 0u; s.aux = 0u; push_rec = true; c_sec++;
+        s.pid = g.child_id(0u); s.blk = 0u; s.aux = aux_with(p.aux, 0u); push_rec = true; c_sec++;
       } else dep += o.T_rec;
       p.blk = g.blk;
       const bool push_p = p.e > T.e_cut;
       if (!push_p) dep += p.e;
       if (push_p) { if (!queue_push(out, p)) atomicOr(&cnt->overflow, 8u); }
       if (push_rec) { if (!queue_push(out, s)) atomicOr(&cnt->overflow, 8u); }
-      if (dep != 0.f) { atomicAdd(tally + batch_base(P, p.hist) + (uint32_t)p.vox, dep); c_dep += (double)dep; }
+      if (dep != 0.f) { atomicAdd(tally + batch_base(P, p.hist) + (uint32_t)p.vox, dep); c_dep += (double)dep; score_influence(P, p.aux, p.vox, dep); }
     }
   }
   flush(&cnt->e_deposit, c_dep); flush(&cnt->n_secondary, c_sec);
@@ -472,6 +486,17 @@ __global__ void __launch_bounds__(256) stats_kernel(Tables T, Grid G, const floa
     dose[v] = mu;
     const float var = s / ((float)B * (float)(B - 1));
     sigma[v] = var > 0.f ? sqrtf(var) : 0.f;
+  }
+}
+
+// influence matrix MeV -> Gy per primary history of the call: D[i][j] *= Gy/(MeV/g) / (rho_j V n)
+__global__ void __launch_bounds__(256) influence_finish_kernel(Tables T, Grid G, const int32_t *roi_vox, uint32_t n_roi, uint32_t nspots,
+                                                               float inv_n, float *dij) {
+  const size_t total = (size_t)n_roi * nspots;
+  for (size_t k = blockIdx.x * (size_t)blockDim.x + threadIdx.x; k < total; k += (size_t)gridDim.x * blockDim.x) {
+    const int hu = G.hu[roi_vox[k % n_roi]];
+    const MatBin &m = T.bins[hu_to_bin(T, T.hu_lut, hu)];
+    dij[k] *= 1.602176634e-10f * inv_n / (bin_density(m, hu) * G.vol);
   }
 }
 

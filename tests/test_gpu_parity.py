@@ -468,6 +468,52 @@ def test_letd_full_physics_matches_oracle(pm, tables):
     assert abs(np.median(rg)) < 3e-3 and rg.std() < 1.25 * ro.std() + 1e-3, (np.median(rg), rg.std(), ro.std())
 
 
+# ------------------------------------------------------------------ per-spot dose influence
+def test_dose_influence_matches_oracle(pm, tables):
+    from paper_1409_8336_b200 import PmcError
+    w = inputs.workload("c1")
+    hu, vox = w["hu"], w["vox"]
+    o = _setup(pm, tables, w["materials"], hu, vox)
+    nz, ny, nx = hu.shape
+    a = inputs.plan_single_spot((3.0, 5.0, 0.0), 100.0, 0.3); b = inputs.plan_single_spot((7.0, 5.0, 0.0), 150.0, 0.3)
+    c = inputs.plan_single_spot((5.0, 5.0, 0.0), 120.0, 0.3); d = inputs.plan_single_spot((5.0, 5.0, 0.0), 70.0, 0.5)
+    spots = np.concatenate([a, b, c, d]); spots[:, 12] = [1.0, 2.0, 0.0, 1.0]
+    # ROI: a 7 x 7 column around each of the three beam axes, every second slab, shuffled
+    cols = [(x, y) for cx in (15, 25, 35) for x in range(cx - 3, cx + 4) for y in range(22, 29)]
+    roi = np.array([(z * ny + y) * nx + x for z in range(0, nz, 2) for (x, y) in cols], dtype=np.int32)
+    roi = np.random.default_rng(3).permutation(roi)
+    n = 200_000                                                            # divisible by the 10 batches
+    D = pm.set_dose_influence(roi, len(spots)); o.set_dose_influence(roi)
+    try:
+        dose, _ = pm.simulate(spots, n, 51)
+        Dg = D.cpu().numpy().astype(np.float64)
+        dose_o, _ = o.simulate(spots, n, 52)
+        Do = o.dose_influence(len(spots))
+        with pytest.raises(PmcError) as e:                                # more spots than the matrix has rows
+            pm.simulate(np.concatenate([spots, spots]), 100, 1)
+        assert e.value.code == -3
+    finally:
+        pm.set_dose_influence(np.zeros(0, dtype=np.int32), 0); o.set_dose_influence(np.zeros(0, dtype=np.int32))
+    dg = dose.cpu().numpy().astype(np.float64).ravel()[roi]
+    # exact bookkeeping on the GPU: the rows add up to the dose (fp32 atomics, two different summation orders)
+    assert np.all(Dg >= 0) and np.all(Dg[2] == 0)
+    assert np.allclose(Dg.sum(axis=0), dg, rtol=3e-4, atol=1e-6 * dg.max())
+    # against the oracle, spot by spot: integral over the ROI, and the depth profile on the spot's own axis
+    zz, xx = roi // (nx * ny), roi % nx
+    for i, cx in ((0, 15), (1, 35), (3, 25)):
+        assert abs(Dg[i].sum() / Do[i].sum() - 1) < 0.01, (i, Dg[i].sum(), Do[i].sum())
+        own = np.abs(xx - cx) <= 3
+        pg = np.bincount(zz[own], weights=Dg[i][own], minlength=nz)[::2]; po = np.bincount(zz[own], weights=Do[i][own], minlength=nz)[::2]
+        m = po > 0.1 * po.max()
+        assert np.max(np.abs(pg[m] / po[m] - 1)) < 0.04, (i, np.max(np.abs(pg[m] / po[m] - 1)))
+        assert abs(int(np.argmax(pg)) - int(np.argmax(po))) <= 1           # each spot's Bragg peak where its energy puts it
+        other = ~own & (np.abs(xx - 25) > 3 if i != 3 else np.abs(xx - 25) > 3)
+        assert Dg[i][other].sum() < 0.02 * Dg[i].sum()                    # (almost) nothing on the other beams' axes
+    # the dose itself is unchanged by the extra scoring
+    d0, _ = pm.simulate(spots, n, 51)
+    assert torch.allclose(d0, dose, rtol=2e-4, atol=1e-16)
+
+
 # ------------------------------------------------------------------ edge and degenerate cases
 def test_simulate_edge_cases(pm, tables):
     from paper_1409_8336_b200 import PmcError
