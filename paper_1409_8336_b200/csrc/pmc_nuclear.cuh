@@ -244,8 +244,9 @@ __device__ bool chan_setup(const Tables &T, int Z, int A, float estar, double Mp
   return true;
 }
 __device__ __forceinline__ float chan_f(const Chan &c, int j, float e, float ref) {
-  const float sinv = j == 0 ? c.alpha * (1.0f + c.beta / e) : (1.0f + c.cj) * (1.0f - c.kV / e);
-  return c.pref * sinv * e * __expf(2.0f * sqrtf(c.ad * (c.emax - e)) - ref);
+  // sigma_inv(e) x e written without the division: alpha (e + beta) for neutrons, (1 + c_j)(e - k_j V_j) for charged
+  const float sinv_e = j == 0 ? c.alpha * (e + c.beta) : (1.0f + c.cj) * (e - c.kV);
+  return c.pref * sinv_e * __expf(2.0f * fsqrt(c.ad * (c.emax - e)) - ref);
 }
 struct Emission { int j; float ke; V3 dir; };
 // one emission from R (updated in place); returns false when no channel is open
