@@ -160,7 +160,7 @@ __device__ __forceinline__ void boost(V3 beta, V3 &p, float &E) {
   const float b2 = dot(beta, beta);
   if (b2 <= 0.f) return;
   const float gam = rsqrtf(1.0f - b2), bp = dot(beta, p);
-  const float f = gam * gam / (gam + 1.0f) * bp + gam * E;      // (gam-1)/b2 = gam^2/(gam+1)
+  const float f = fdiv(gam * gam, gam + 1.0f) * bp + gam * E;      // (gam-1)/b2 = gam^2/(gam+1)
   p = p + f * beta;
   E = gam * (E + bp);
 }
@@ -293,17 +293,17 @@ __device__ float straggle(const Tables &T, Rng &g, float e_start, float mean_los
 __device__ __forceinline__ float cug_sigma_pp(float p) {
   if (p < 0.44f) return 34.0f * __powf(p * 2.5f, -2.104f);
   if (p < 0.8f) { float d = p - 0.7f; d *= d; return 23.5f + 1000.0f * d * d; }
-  if (p < 2.0f) return 1250.0f / (p + 50.0f) - 4.0f * (p - 1.3f) * (p - 1.3f);
-  return 77.0f / (p + 1.5f);
+  if (p < 2.0f) return fdiv(1250.0f, p + 50.0f) - 4.0f * (p - 1.3f) * (p - 1.3f);
+  return fdiv(77.0f, p + 1.5f);
 }
 __device__ __forceinline__ float cug_sigma_np(float p) {
   if (p < 0.446f) { const float l = __logf(p); return 6.3555f * __expf(-3.2481f * l - 0.377f * l * l); }
-  if (p < 0.8f) { const float a = fabsf(p - 0.95f); return 33.0f + 196.0f * a * a * sqrtf(a); }
+  if (p < 0.8f) { const float a = fabsf(p - 0.95f); return 33.0f + 196.0f * a * a * fsqrt(a); }
   if (p < 2.0f) return 31.0f * rsqrtf(p);
-  return 77.0f / (p + 1.5f);
+  return fdiv(77.0f, p + 1.5f);
 }
 __device__ __forceinline__ float cug_b_pp(float p) {
-  if (p < 2.0f) { float p2 = p * p, p4 = p2 * p2, p8 = p4 * p4; return 5.5f * p8 / (7.7f + p8); }
+  if (p < 2.0f) { float p2 = p * p, p4 = p2 * p2, p8 = p4 * p4; return fdiv(5.5f * p8, 7.7f + p8); }
   return 5.334f + 0.67f * (p - 2.0f);
 }
 __device__ __forceinline__ float cug_b_np(float p) {
@@ -312,21 +312,21 @@ __device__ __forceinline__ float cug_b_np(float p) {
   if (p < 1.6f) return -1.63f * p + 7.16f;
   return cug_b_pp(p);
 }
-__device__ __forceinline__ float cug_a_np(float p) { return p < 0.8f ? 1.0f : 0.64f / (p * p); }
+__device__ __forceinline__ float cug_a_np(float p) { return p < 0.8f ? 1.0f : fdiv(0.64f, p * p); }
 
 // |t| from exp(-B t) truncated to [0, tmax]
 __device__ __forceinline__ float trunc_exp(float B, float tmax, float u) {
   if (B * tmax < 1e-6f) return u * tmax;
-  return -__logf(1.0f - u * (1.0f - __expf(-B * tmax))) / B;
+  return fdiv(-__logf(1.0f - u * (1.0f - __expf(-B * tmax))), B);
 }
 // cos(theta_cm) of NN elastic scattering: dsigma/dt ~ exp(B t) (+ a exp(B u) for np).  Uses 2 uniforms.
 __device__ __forceinline__ float sample_nn_cos(bool same, float p_lab_gev, float pcm_mev, uint32_t r0, uint32_t r1) {
   const float tmax = 4.0f * pcm_mev * pcm_mev * 1e-6f;
   const float B = same ? cug_b_pp(p_lab_gev) : cug_b_np(p_lab_gev);
   bool backward = false;
-  if (!same) { const float a = cug_a_np(p_lab_gev); backward = u01(r0) < a / (1.0f + a); }
+  if (!same) { const float a = cug_a_np(p_lab_gev); backward = u01(r0) * (1.0f + a) < a; }
   const float t = trunc_exp(B, tmax, u01(r1));
-  const float c = 1.0f - 2.0f * t / tmax;
+  const float c = 1.0f - fdiv(2.0f * t, tmax);
   return backward ? -c : c;
 }
 
