@@ -139,6 +139,7 @@ struct Tables {
   std::vector<int> ez, ea;
   double e_cut = 0.1, highland = 1.07, kappa_g = 10, s_max = 0.2;
   int n_batches = 10;
+  std::vector<double> mol_c0, mol_c1, mol_c2; double mol_dth = 0;      // Moliere tables (Reading R12)
   bool loaded = false;
 
   static double spline(const double *y, const double *y2, int n, double x0, double h, double x) {
@@ -497,6 +498,7 @@ struct opmc_ctx {
   bool opt_strag = true, opt_mcs = true, opt_el = true, opt_ne = true; int threads = 0;
   // per-spot dose influence on a list of ROI voxels (Reading R11)
   std::vector<int32_t> roi_vox, roi_map; std::vector<double> dij; int dij_spots = 0;
+  int mcs_model = 0;                          // 0 Highland x 1.07 (the paper's results), 1 full Moliere (L59; Reading R12)
   bool score_let = false; std::vector<double> let_num, let_den;   // LET_d tallies (Reading R9)
   opmc_counters cnt{};
   std::string err;
@@ -564,6 +566,48 @@ inline void score_influence(opmc_ctx *c, int spot, size_t vox, double e) {
   c->dij[(size_t)spot * c->roi_vox.size() + j] += e;
 }
 
+// Full Moliere theory (Bethe 1953; Reading R12).  Space angle after mass thickness t = rho dx of a mixture:
+//   chi_c^2 = 0.157 t sum_i w_i Z_i(Z_i+1)/A_i / (p beta)^2,   chi_a,i^2 = 2.007e-5 Z_i^(2/3) [1 + 3.34 (Z_i alpha/beta)^2] / p^2,
+//   ln chi_a^2 = Z(Z+1)/A-weighted mean of ln chi_a,i^2,  b = ln(chi_c^2/chi_a^2) + 1 - 2 C_Euler,  B - ln B = b,
+//   f(theta) theta dtheta = x dx [2 e^{-x^2} + f1(x)/B + f2(x)/B^2],  x = theta / (chi_c sqrt(B)).
+// x is drawn by inverting the tabulated cumulative C0 + C1/B + C2/B^2 (uniform in x^2 inside a bin), beyond the table
+// from the single-scattering tail 1/(B x^2).  Fewer than 20 collisions (Omega < 20): outside the theory -> Highland.
+inline bool moliere_angle(const opmc_ctx *c, const Material &m, double rho, double e, double dx, Rng &g, double &theta) {
+  const Tables &T = c->T;
+  const double p2 = e * (e + 2 * MP), E = e + MP, beta2 = p2 / (E * E), pb = p2 / E, t = dx * rho;
+  double zs = 0, zl = 0;
+  for (int i = 0; i < T.n_elem; ++i) {
+    if (m.w[i] <= 0) continue;
+    const double Z = T.ez[i], q = m.w[i] * Z * (Z + 1) / T.ea[i];
+    const double za = Z / 137.035999 , chia2 = 2.007e-5 * std::pow(Z, 2.0 / 3.0) * (1 + 3.34 * za * za / beta2) / p2;
+    zs += q; zl += q * std::log(chia2);
+  }
+  if (zs <= 0 || t <= 0) return false;
+  const double chic2 = 0.157 * zs * t / (pb * pb), ln_omega = std::log(chic2) - zl / zs;
+  if (ln_omega < std::log(20.0)) return false;
+  const double b = ln_omega + 1 - 2 * 0.5772156649015329;
+  double B = b + std::log(b);
+  for (int it = 0; it < 8; ++it) B -= (B - std::log(B) - b) / (1 - 1 / B);
+  const int n = (int)T.mol_c0.size(); const double dth = T.mol_dth, xmax = (n - 1) * dth;
+  auto C = [&](int k) { return T.mol_c0[k] + T.mol_c1[k] / B + T.mol_c2[k] / (B * B); };
+  const double tail = 1 / (B * xmax * xmax), total = C(n - 1) + tail, U = g.u() * total;
+  double x;
+  if (U >= C(n - 1)) x = 1 / std::sqrt(B * std::max(total - U, 1e-300));
+  else {
+    int k = 0;
+    while (k < n - 2 && C(k + 1) <= U) ++k;
+    const double c0 = C(k), c1 = C(k + 1), f = c1 > c0 ? std::min(std::max((U - c0) / (c1 - c0), 0.0), 1.0) : 0.5;
+    const double x0 = k * dth, x1 = (k + 1) * dth;
+    x = std::sqrt(x0 * x0 + f * (x1 * x1 - x0 * x0));
+  }
+  theta = std::min(std::sqrt(chic2 * B) * x, PI);
+  return true;
+}
+inline V3 deflect_by(Rng &g, V3 d, double th) {
+  double ph = 2 * PI * g.u();
+  return unit(to_lab(d, std::sin(th) * std::cos(ph), std::sin(th) * std::sin(ph), std::cos(th)));
+}
+
 struct StepResult { int cls; double L; };    // cls: 0 none, 1 boundary, 2 nuclear, 3 range-out
 
 // One condensed-history step (Reading R3 "H1").  Deposits into `tally` (MeV).
@@ -593,7 +637,9 @@ bool transport_step(opmc_ctx *c, Particle &p, Rng &g, double *tally, Ledger &led
   if (c->opt_mcs && dx > 0) {
     tau = g.u() * dx;
     p.r = p.r + tau * p.d;
-    dnew = deflect(g, p.d, highland(T, e0, dx * rho, m.x0));
+    double th_m;
+    if (c->mcs_model == 1 && moliere_angle(c, m, rho, e0, dx, g, th_m)) dnew = deflect_by(g, p.d, th_m);
+    else dnew = deflect(g, p.d, highland(T, e0, dx * rho, m.x0));
   }
   double ell = dx - tau; int ax2, sg2; double d2 = dist_to_face(c, p.r, dnew, p.idx, ax2, sg2);
   double L; int cls;
@@ -837,6 +883,10 @@ int opmc_load_physics_tables(opmc_ctx *c, const opmc_tables *t) {
   T.ez.assign(t->elem_z, t->elem_z + T.n_elem); T.ea.assign(t->elem_a, t->elem_a + T.n_elem);
   for (int s = 0; s < T.n_sr; ++s) for (int i = 1; i < T.n_e; ++i)
     if (!(T.lnR[s * T.n_e + i] > T.lnR[s * T.n_e + i - 1])) return fail(c, "range table not monotone");
+  if (t->mol_n > 1 && t->mol_c0 && t->mol_c1 && t->mol_c2) {
+    T.mol_c0.assign(t->mol_c0, t->mol_c0 + t->mol_n); T.mol_c1.assign(t->mol_c1, t->mol_c1 + t->mol_n); T.mol_c2.assign(t->mol_c2, t->mol_c2 + t->mol_n);
+    T.mol_dth = t->mol_dtheta;
+  }
   T.e_cut = t->e_cut; T.highland = t->highland_factor; T.kappa_g = t->kappa_gauss; T.s_max = t->s_max_wet_cm; T.n_batches = t->n_batches;
   c->nuc.assign(T.n_elem, Nucleus());
   for (int i = 0; i < T.n_elem; ++i) if (T.ea[i] > 1) {
@@ -881,6 +931,7 @@ int opmc_set_option(opmc_ctx *c, const char *key, double v) {
   else if (k == "elastic") c->opt_el = v != 0; else if (k == "nonelastic") c->opt_ne = v != 0;
   else if (k == "s_max_wet_cm") c->T.s_max = v; else if (k == "n_batches") c->T.n_batches = (int)v;
   else if (k == "threads") c->threads = (int)v; else if (k == "score_letd") c->score_let = v != 0;
+  else if (k == "mcs_model") { if ((v != 0 && v != 1) || (v == 1 && c->T.mol_c0.empty())) return fail(c, "mcs_model: 0 or 1 (1 needs the Moliere tables)"); c->mcs_model = (int)v; }
   else return fail(c, "unknown option");
   return 0;
 }

@@ -41,6 +41,8 @@ typedef struct {                 /* all input
   const double *evap_k, *evap_c;                /* [6][zdim] Dostrovsky k_j, c_j vs daughter Z */
   double e_cut, highland_factor, kappa_gauss, s_max_wet_cm;
   int32_t n_batches;
+  /* Moliere option (Reading R12): cumulative functions C_k[m] = int_0^{m dtheta} theta f^(k) dtheta, k = 0,1,2 */
+  int32_t mol_n; double mol_dtheta; const double *mol_c0, *mol_c1, *mol_c2;
 } opmc_tables;
 
 typedef struct {                 /* PAPER.md:L49, Eq.1, Eq.2 */

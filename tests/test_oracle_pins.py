@@ -627,3 +627,55 @@ def test_dose_influence_rows_add_up_to_the_dose(oracle_c1):
         o.dose_influence(3)                                               # switched off again
     with pytest.raises(Exception):
         o.set_dose_influence(np.array([0, 0], dtype=np.int32))            # repeated voxel
+
+
+# ------------------------------------------------------------------ full Moliere MCS option (Reading R12)
+def test_moliere_tables_against_closed_forms(tables):
+    """The cumulative Moliere functions the generator integrates numerically, against what the mathematics fixes:
+    f0 = 2 exp(-x^2); f1(0) = 2 (1 - C_Euler); f2(0) = Gamma''(3); int x f1 dx = 0 (the correction terms carry no
+    probability), with the part beyond the table taken from the Rutherford tail f1 -> 2/x^4."""
+    c0, c1, c2, h = tables["mol_c0"], tables["mol_c1"], tables["mol_c2"], tables["mol_dtheta"]
+    x = np.arange(tables["mol_n"]) * h
+    assert np.max(np.abs(c0 - (1 - np.exp(-x * x)))) < 1e-4
+    euler = 0.5772156649015329
+    f0 = lambda c: (4 * 2 * c[1] / h ** 2 - 2 * c[2] / (2 * h) ** 2) / 3          # C(x) = f(0) x^2/2 + O(x^4): Richardson
+    assert abs(f0(c1) / (2 * (1 - euler)) - 1) < 2e-3
+    gamma2_3 = 2 * ((1.5 - euler) ** 2 + np.pi ** 2 / 6 - 1.25)                    # Gamma''(3) = Gamma(3) [psi(3)^2 + psi'(3)]
+    assert abs(f0(c2) / gamma2_3 - 1) < 2e-3
+    xmax = x[-1]
+    assert abs(c1[-1] + 1 / xmax ** 2) < 3e-4 and abs(c2[-1]) < 1e-3
+    assert c1.min() < -0.3 and 1.0 < x[np.argmin(c1)] < 2.2                       # f1 changes sign once near x ~ 1.5-2
+
+
+def test_moliere_single_step_core_and_rutherford_tail(tables):
+    """One 2 mm step of 150 MeV protons in water with the Moliere option: the core of the space-angle distribution
+    agrees with Highland's fit to Moliere theory (median of a 2-D Gaussian of width theta0 = 1.177 theta0, within 6 %),
+    and far out the probability follows single Rutherford scattering, P(theta > t) = chi_c^2 / t^2."""
+    o = Oracle(tables, inputs.make_materials_c1())
+    hu, vox = inputs.phantom_c1()
+    o.load_ct(hu, vox)
+    for k, v in (("straggling", 0), ("elastic", 0), ("nonelastic", 0), ("mcs_model", 1)):
+        o.set_option(k, v)
+    n = 400_000
+    r = o.first_steps(inputs.plan_single_spot((5.1, 5.1, 0.0), 150.0, 0.0), n, 5, 1)
+    th = np.hypot(r[:, 3], r[:, 4])
+    e, t = 150.0, 0.2
+    pc2 = e * (e + 2 * M_P); pb = pc2 / (e + M_P)
+    theta0 = 13.6 / pb * np.sqrt(t / 36.08) * (1 + 0.038 * np.log(t / 36.08))      # Highland, X0(water) = 36.08 g/cm2
+    assert abs(np.median(th) / (1.1774 * theta0) - 1) < 0.06
+    zs = 0.1119 * 2 / 1.0 + 0.8881 * 72 / 16.0                                      # sum w Z(Z+1)/A of water (A = 1, 16)
+    chic2 = 0.157 * zs * t / pb ** 2
+    for mult in (8.0, 16.0):
+        tc = mult * theta0
+        p_tail, p_ruth = np.mean(th > tc), chic2 / tc ** 2
+        assert abs(p_tail / p_ruth - 1) < 0.25 + 3 / np.sqrt(n * p_ruth), (mult, p_tail, p_ruth)
+    # the Gaussian model has no such tail at all
+    o.set_option("mcs_model", 0)
+    r0 = o.first_steps(inputs.plan_single_spot((5.1, 5.1, 0.0), 150.0, 0.0), n, 5, 1)
+    assert np.mean(np.hypot(r0[:, 3], r0[:, 4]) > 8 * theta0) == 0.0
+    # fewer than 20 collisions in the step (Omega < 20): outside Moliere theory, both models take the Highland branch
+    o.set_option("s_max_wet_cm", 2e-5)
+    a = o.first_steps(inputs.plan_single_spot((5.1, 5.1, 0.0), 150.0, 0.0), 2000, 7, 3)
+    o.set_option("mcs_model", 1)
+    b = o.first_steps(inputs.plan_single_spot((5.1, 5.1, 0.0), 150.0, 0.0), 2000, 7, 3)
+    assert np.array_equal(a, b)
