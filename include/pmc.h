@@ -57,6 +57,10 @@ typedef struct pmc_tables {
   double kappa_gauss;                           /* Reading R4: Vavilov kappa above which straggling is Gaussian */
   double s_max_wet_cm;                          /* Reading R3.2: step cap in g/cm2 of the table medium; <=0: none */
   int32_t n_batches;                            /* 10 */
+  /* Full Moliere option (Reading R12; may be 0/NULL if "mcs_model" stays 0): cumulative Moliere
+   * functions C_k[m] = int_0^{m mol_dtheta} x f^(k)(x) dx, k = 0, 1, 2, on a uniform grid of the reduced angle x */
+  int32_t mol_n; double mol_dtheta;
+  const double *mol_c0, *mol_c1, *mol_c2;       /* [mol_n] */
 } pmc_tables;
 
 /* One HU bin of the HU -> material conversion (§II.A.1; Eq.1/Eq.2; L59). */
@@ -127,7 +131,8 @@ int  pmc_load_ct(pmc_ctx *ctx, const int16_t *hu_dev, int nx, int ny, int nz,
 int  pmc_load_ct_host(pmc_ctx *ctx, const int16_t *hu_host, int nx, int ny, int nz,
                       double dx_cm, double dy_cm, double dz_cm, const double *origin_cm);
 
-/* Options: "straggling" "mcs" "elastic" "nonelastic" (0/1), "s_max_wet_cm", "n_batches",
+/* Options: "straggling" "mcs" "elastic" "nonelastic" (0/1), "mcs_model" (0 = Highland x 1.07, the paper's choice;
+ * 1 = full Moliere theory, needs the mol_* tables), "s_max_wet_cm", "n_batches",
  * "chunk_histories" (histories per sub-group), "history_offset" (first history id, for sharding
  * a run over several GPUs), "dose_aggregate" (0/1, default 0: merge the lanes of a warp that score into the same voxel before the atomic), "score_letd" (0/1, see pmc_get_letd),
  * "profile" (0/1, default 1: a CUDA-event pair is recorded on the context's stream around every kernel launch and

@@ -31,7 +31,8 @@ class Tables(C.Structure):
                 ("mass_zdim", C.c_int32), ("mass_adim", C.c_int32), ("nuclear_mass", _D),
                 ("evap_k", _D), ("evap_c", _D),
                 ("e_cut", C.c_double), ("highland_factor", C.c_double), ("kappa_gauss", C.c_double),
-                ("s_max_wet_cm", C.c_double), ("n_batches", C.c_int32)]
+                ("s_max_wet_cm", C.c_double), ("n_batches", C.c_int32),
+                ("mol_n", C.c_int32), ("mol_dtheta", C.c_double), ("mol_c0", _D), ("mol_c1", _D), ("mol_c2", _D)]
 
 
 class HuBin(C.Structure):

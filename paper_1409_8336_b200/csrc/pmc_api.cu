@@ -71,6 +71,7 @@ struct pmc_ctx {
   double e_min = 0, e_max = 0;
   std::vector<double> h_lnR, h_lnR2, h_lnrlo, h_lnrhi, h_lnE, h_lnE2, h_sne, h_sel, h_mass, h_ek, h_ec;
   std::vector<int> ez, ea;
+  std::vector<float> h_mol; int mol_n = 0; double mol_dth = 0; int mcs_model = 0; DevBuf<float> d_mol;
   double e_cut = 0.1, highland = 1.07, kappa_g = 10, s_max = 0.2; int n_batches = 10;
   bool opt_strag = true, opt_mcs = true, opt_el = true, opt_ne = true; int aggregate = 0; bool profile = true;
   uint64_t chunk = 1u << 24, history_offset = 0;
@@ -153,6 +154,7 @@ int sync_tables(pmc_ctx *c) {
   T.e_min = (float)c->e_min; T.e_max = (float)c->e_max;
   T.e_cut = (float)c->e_cut; T.highland = (float)c->highland; T.kappa_g = (float)c->kappa_g; T.s_max = (float)c->s_max;
   T.opt_strag = c->opt_strag; T.opt_mcs = c->opt_mcs; T.opt_el = c->opt_el; T.opt_ne = c->opt_ne;
+  CK(c->d_mol.upload(c->h_mol, s)); T.mol_c = c->d_mol.p; T.mol_n = c->mol_n; T.mol_dth = (float)c->mol_dth; T.mcs_model = c->mol_n > 1 ? c->mcs_model : 0;
   CK(c->d_lnR.upload(to_f(c->h_lnR), s)); CK(c->d_lnR2.upload(to_f(c->h_lnR2, dlne * dlne / 6.0), s));
   std::vector<float> e2(c->h_lnE2.size());
   for (int t = 0; t < c->n_sr; ++t) {
@@ -177,6 +179,8 @@ int sync_tables(pmc_ctx *c) {
       m.rho_lo = (float)h.rho_lo; m.drho = (float)(h.rho_hi - h.rho_lo);
       m.wet = h.table_id == 0 ? (float)h.f_m : 1.0f; m.inv_x0 = (float)(1.0 / h.x0_gcm2); m.zoa = (float)c->mats[b].zoa; m.table = h.table_id;
       for (int i = 0; i < MAX_ELEM; ++i) m.nfac[i] = i < c->n_elem ? (float)(NAVO * h.w[i] / c->ea[i] * 1e-27) : 0.f;
+      double zs = 0; for (int i = 0; i < c->n_elem; ++i) zs += h.w[i] * c->ez[i] * (c->ez[i] + 1.0) / c->ea[i];
+      m.zs = (float)zs;
       // macroscopic cross-section per unit density: a sum of tables that are linear in ln E is linear in ln E
       for (int k = 0; k < c->n_e; ++k) {
         double acc = 0;
@@ -199,7 +203,8 @@ int sync_tables(pmc_ctx *c) {
     c->smem_transport = ((size_t)2 * c->n_sr * c->n_e + (size_t)2 * c->n_sr * c->n_r + (size_t)nb * c->n_e) * 4 + (size_t)nb * sizeof(MatBin) +
                         lut.size() + 16;
     if (c->smem_transport > 200 * 1024) return fail(c, PMC_E_UNSUPPORTED, "tables too large for shared-memory staging");
-    CK(cudaFuncSetAttribute(transport_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_transport));
+    CK(cudaFuncSetAttribute(transport_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_transport));
+    CK(cudaFuncSetAttribute(transport_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_transport));
   }
   CK(cudaStreamSynchronize(s));
   c->tables_dirty = false;
@@ -285,7 +290,8 @@ int run_generations(pmc_ctx *c, RunParams P, uint32_t n0, bool profile) {
     CK(cudaMemsetAsync(c->qel.q.count, 0, 4, s)); CK(cudaMemsetAsync(c->qne.q.count, 0, 4, s)); CK(cudaMemsetAsync(c->qres.q.count, 0, 4, s));
     CK(cudaMemsetAsync(c->qev.q.count, 0, 4, s));
     { Timer t(c, &c->timing.transport_ms, profile);
-      transport_kernel<<<grid_t, TRANSPORT_THREADS, c->smem_transport, s>>>(c->T, c->G, P, cur->q, n_in, c->d_head.p, c->qev.q, c->d_tally.p, c->d_cnt.p); }
+      if (c->T.mcs_model == 1) transport_kernel<1><<<grid_t, TRANSPORT_THREADS, c->smem_transport, s>>>(c->T, c->G, P, cur->q, n_in, c->d_head.p, c->qev.q, c->d_tally.p, c->d_cnt.p);
+      else transport_kernel<0><<<grid_t, TRANSPORT_THREADS, c->smem_transport, s>>>(c->T, c->G, P, cur->q, n_in, c->d_head.p, c->qev.q, c->d_tally.p, c->d_cnt.p); }
     c->timing.launches_total++; c->timing.launches_transport++;
     if (P.dbg_out) break;
     { Timer t(c, &c->timing.elastic_ms, profile);
@@ -364,7 +370,7 @@ void pmc_destroy(pmc_ctx *c) {
   c->d_sigbin.release(); c->d_ek.release(); c->d_ec.release(); c->d_mass.release(); c->d_bins.release(); c->d_lut.release();
   c->d_nuc.release(); c->d_nuc1.release(); c->d_hu_own.release();
   c->qa.release(); c->qb.release(); c->qev.release(); c->qel.release(); c->qne.release(); c->qres.release(); c->d_resza.release(); c->d_resp.release();
-  c->d_head.release(); c->d_cnt.release(); c->d_tally.release(); c->d_out.release(); c->d_let.release(); c->d_roimap.release(); c->d_roivox.release();
+  c->d_head.release(); c->d_cnt.release(); c->d_tally.release(); c->d_out.release(); c->d_let.release(); c->d_mol.release(); c->d_roimap.release(); c->d_roivox.release();
   c->d_spots.release(); c->d_cdf.release(); c->d_res.release(); c->d_goff.release(); c->d_gscr.release(); c->d_slots.release(); c->d_counts.release(); c->d_base.release();
   if (c->h_pinned) cudaFreeHost(c->h_pinned);
   if (c->ev[0]) { cudaEventDestroy(c->ev[0]); cudaEventDestroy(c->ev[1]); }
@@ -396,6 +402,11 @@ int pmc_load_physics_tables(pmc_ctx *c, const pmc_tables *t) {
     for (int i = 1; i < c->n_e; ++i)
       if (!(c->h_lnR[(size_t)s * c->n_e + i] > c->h_lnR[(size_t)s * c->n_e + i - 1])) return fail(c, PMC_E_INVALID_ARG, "range table not monotone");
     if (!(c->h_lnrhi[s] > c->h_lnrlo[s])) return fail(c, PMC_E_INVALID_ARG, "inverse range table abscissa not increasing");
+  }
+  c->h_mol.clear(); c->mol_n = 0; c->mcs_model = 0;
+  if (t->mol_n > 1 && t->mol_c0 && t->mol_c1 && t->mol_c2 && t->mol_dtheta > 0) {
+    c->mol_n = t->mol_n; c->mol_dth = t->mol_dtheta;
+    for (const double *src : {t->mol_c0, t->mol_c1, t->mol_c2}) for (int i = 0; i < t->mol_n; ++i) c->h_mol.push_back((float)src[i]);
   }
   c->e_cut = t->e_cut; c->highland = t->highland_factor; c->kappa_g = t->kappa_gauss; c->s_max = t->s_max_wet_cm; c->n_batches = t->n_batches;
   c->h_nuc.assign(c->n_elem, Nucleus{});
@@ -472,6 +483,7 @@ int pmc_set_option(pmc_ctx *c, const char *key, double v) {
   else if (k == "dose_aggregate") c->aggregate = v != 0;
   else if (k == "profile") c->profile = v != 0;
   else if (k == "score_letd") c->score_let = v != 0;
+  else if (k == "mcs_model") { if ((v != 0 && v != 1) || (v == 1 && c->mol_n < 2)) return fail(c, PMC_E_INVALID_ARG, "mcs_model: 0 or 1 (1 needs the Moliere tables)"); c->mcs_model = (int)v; }
   else return fail(c, PMC_E_INVALID_ARG, "unknown option");
   c->tables_dirty = true;
   return PMC_OK;

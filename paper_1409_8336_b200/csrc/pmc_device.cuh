@@ -78,6 +78,7 @@ struct MatBin {                 // one HU bin, 16 floats
   float inv_x0, zoa;
   int table;
   float nfac[MAX_ELEM];         // N_A w_i / A_i * 1e-27 : (cm^2/g) per mb of element i
+  float zs;                     // sum_i w_i Z_i (Z_i + 1) / A_i (Moliere chi_c^2, Reading R12)
 };
 
 struct Nucleus {                // PAPER.md:L77, Reading R6.1; type 0 = proton, 1 = neutron
@@ -95,6 +96,7 @@ struct Tables {
   float lnr_lo[4], lnr_hi[4], inv_hr[4];
   int hu_lut_lo, hu_lut_n;
   int opt_strag, opt_mcs, opt_el, opt_ne;
+  int mcs_model, mol_n; float mol_dth; const float *mol_c;   // Moliere: C0, C1, C2 back to back, [3][mol_n]
   const float *lnR, *lnR2;      // [n_sr][n_e]; y'' pre-multiplied by h^2/6
   const float *lnE, *lnE2;      // [n_sr][n_r]
   const float *sig_el, *sig_ne; // [n_elem][n_e] mb

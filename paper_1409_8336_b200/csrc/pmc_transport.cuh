@@ -89,6 +89,52 @@ __device__ __forceinline__ V3 deflect(V3 d, float theta0, uint32_t r0, uint32_t 
   return unit(to_lab(d, st * cp, st * sp, ct));
 }
 
+// Full Moliere theory (Bethe 1953; Reading R12): space angle after mass thickness t of the voxel's mixture.
+// chi_c^2 = 0.157 t zs / (p beta)^2; ln chi_a^2 = Z(Z+1)/A-weighted mean of ln{2.007e-5 Z^(2/3) [1 + 3.34 (Z alpha/beta)^2] / p^2};
+// b = ln(chi_c^2 / chi_a^2) + 1 - 2 C_Euler; B - ln B = b; reduced angle x from the tabulated cumulative C0 + C1/B + C2/B^2
+// (bisection, uniform in x^2 inside a bin), beyond the table from the Rutherford tail 1/(B x^2).  Returns a negative
+// number when the step holds fewer than 20 collisions (outside the theory): the caller then uses Highland.
+__device__ __forceinline__ float moliere_angle(const Tables &T, const MatBin &m, float e, float t, float u) {
+  const float p2 = e * (e + 2.0f * MP), E = e + MP, ibeta2 = fdiv(E * E, p2), pb = fdiv(p2, E);
+  if (!(t > 0.f) || !(m.zs > 0.f)) return -1.0f;
+  float zl = 0.f;
+#pragma unroll
+  for (int i = 0; i < MAX_ELEM; ++i) {
+    if (i < T.n_elem && m.nfac[i] > 0.f) {
+      const float Z = (float)T.elem_z[i], za = Z * (1.0f / 137.035999f);
+      const float q = m.nfac[i] * Z * (Z + 1.0f);                            // proportional to w Z (Z+1) / A
+      zl += q * (__logf(2.007e-5f * (1.0f + 3.34f * za * za * ibeta2)) + (2.0f / 3.0f) * __logf(Z) - __logf(p2));
+    }
+  }
+  const float qs = m.zs * (6.02214076e23f * 1e-27f);                          // same normalisation as q
+  const float chic2 = fdiv(0.157f * m.zs * t, pb * pb), ln_omega = __logf(chic2) - fdiv(zl, qs);
+  if (ln_omega < 2.99573227f) return -1.0f;                                  // ln 20
+  const float b = ln_omega + (1.0f - 2.0f * 0.5772156649f);
+  float B = b + __logf(b);
+#pragma unroll
+  for (int it = 0; it < 4; ++it) B -= fdiv(B - __logf(B) - b, 1.0f - fdiv(1.0f, B));
+  const int n = T.mol_n; const float iB = fdiv(1.0f, B), iB2 = iB * iB;
+  const float *c0 = T.mol_c, *c1 = T.mol_c + n, *c2 = T.mol_c + 2 * n;
+  auto C = [&](int k) { return __ldg(c0 + k) + __ldg(c1 + k) * iB + __ldg(c2 + k) * iB2; };
+  const float xmax = (float)(n - 1) * T.mol_dth, tail = fdiv(iB, xmax * xmax), cend = C(n - 1), total = cend + tail, U = u * total;
+  float x;
+  if (U >= cend) x = rsqrtf(B * fmaxf(total - U, 1e-30f));
+  else {
+    int lo = 0, hi = n - 1;                                                   // C(lo) <= U < C(hi)
+    while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (C(mid) <= U) lo = mid; else hi = mid; }
+    const float ca = C(lo), cb = C(hi), f = cb > ca ? fminf(fmaxf(fdiv(U - ca, cb - ca), 0.f), 1.0f) : 0.5f;
+    const float x0 = (float)lo * T.mol_dth, x1 = (float)hi * T.mol_dth;
+    x = fsqrt(x0 * x0 + f * (x1 * x1 - x0 * x0));
+  }
+  return fminf(fsqrt(chic2 * B) * x, 3.14159265f);
+}
+// rotate d by the polar angle th and a uniform azimuth
+__device__ __forceinline__ V3 deflect_by(V3 d, float th, uint32_t r1) {
+  float st, ct, sp, cp;
+  sincos_small(th, &st, &ct); sincos_2pi(u01(r1), &sp, &cp);
+  return unit(to_lab(d, st * cp, st * sp, ct));
+}
+
 // mean energy loss over water-equivalent path dr (g/cm2 of the table medium) from the range table
 // (Eq.2): E - E(R(E) - dr), written with expm1 so that a vanishing step loses nothing.
 __device__ __forceinline__ float mean_loss(const Tables &T, const float *lnE, const float *lnE2, int tab,
@@ -226,6 +272,9 @@ __device__ __forceinline__ void deposit(float *tally, uint32_t tvox, float e, bo
 // Particles that reach an event are appended to the elastic or non-elastic queue; nothing else is written back.
 constexpr int TRANSPORT_THREADS = 256, TRANSPORT_BLOCKS_PER_SM = 4;
 
+// MCS_MODEL: 0 = Highland (the paper's choice), 1 = full Moliere; a template so that the default kernel carries none of
+// the Moliere code or its registers
+template <int MCS_MODEL>
 __global__ void __launch_bounds__(TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM) transport_kernel(Tables T, Grid G, RunParams P, Queue in, uint32_t n_in,
                                                            uint32_t *head, Queue q_ev, float *tally, Counters *cnt) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -300,7 +349,9 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM) tr
       if (T.opt_mcs && dx > 0.f) {
         tau = u01(r.y) * dx;
         p.r = p.r + tau * p.d;
-        dnew = deflect(p.d, highland(T, e0, dx * rho * m.inv_x0), r.z, r.w);
+        float th_m = -1.0f;
+        if (MCS_MODEL == 1) th_m = moliere_angle(T, m, e0, dx * rho, u01(r.z));
+        dnew = th_m >= 0.f ? deflect_by(p.d, th_m, r.w) : deflect(p.d, highland(T, e0, dx * rho * m.inv_x0), r.z, r.w);
       }
       const float ell = dx - tau; int ax2, sg2; const float d2 = dist_to_face(p.r, dnew, sz, ax2, sg2);
       float L; int cls;

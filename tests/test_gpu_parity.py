@@ -514,6 +514,43 @@ def test_dose_influence_matches_oracle(pm, tables):
     assert torch.allclose(d0, dose, rtol=2e-4, atol=1e-16)
 
 
+# ------------------------------------------------------------------ full Moliere MCS option
+def test_moliere_option_matches_oracle(pm, tables):
+    from scipy import stats
+    w = inputs.workload("c1")
+    o = _setup(pm, tables, w["materials"], w["hu"], w["vox"], elastic=0, nonelastic=0, straggling=0)
+    pm.set_option("mcs_model", 1.0); o.set_option("mcs_model", 1.0)
+    try:
+        # one 2 mm step at 150 MeV and at 70 MeV: the whole space-angle distribution, core and single-scattering tail
+        for e_mev in (150.0, 70.0):
+            spot = inputs.plan_single_spot((5.1, 5.1, 0.0), e_mev, 0.0)
+            n = 400_000
+            g = pm.first_steps(spot, n, 5, 1).astype(np.float64); r = o.first_steps(spot, n, 6, 1)
+            tg, to = np.hypot(g[:, 3], g[:, 4]), np.hypot(r[:, 3], r[:, 4])
+            assert stats.ks_2samp(tg, to).pvalue > 1e-3
+            t0 = np.median(to)
+            for mult in (3.0, 6.0, 12.0):                                  # tail counts: Poisson
+                a, b = np.sum(tg > mult * t0), np.sum(to > mult * t0)
+                assert abs(a - b) < 5 * np.sqrt(a + b + 1), (e_mev, mult, a, b)
+            assert np.sum(to > 6.0 * t0) > 100                             # the tail is there (a Gaussian has e^-25)
+        # 40 steps at 230 MeV: lateral spread and angle-displacement covariance of the multi-step walk
+        spot = inputs.plan_single_spot((5.1, 5.1, 0.0), 230.0, 0.0)
+        g = pm.first_steps(spot, 200_000, 5, 40).astype(np.float64); r = o.first_steps(spot, 200_000, 6, 40)
+        for col in (0, 3):
+            assert abs(np.percentile(np.abs(g[:, col] - (5.1 if col == 0 else 0)), 68.27) /
+                       np.percentile(np.abs(r[:, col] - (5.1 if col == 0 else 0)), 68.27) - 1) < 0.02
+        # full physics on C1 with the Moliere option on both sides
+        for k in ("elastic", "nonelastic", "straggling"):
+            pm.set_option(k, 1.0); o.set_option(k, 1.0)
+        _dose_parity(pm, o, w["hu"], w["vox"], w["materials"], w["spots"], 100_000, 23, min_pass=0.985)
+        # without the tables the option is refused
+        from paper_1409_8336_b200 import PmcError
+    finally:
+        pm.set_option("mcs_model", 0.0)
+    with pytest.raises(PmcError):
+        pm.set_option("mcs_model", 2.0)
+
+
 # ------------------------------------------------------------------ edge and degenerate cases
 def test_simulate_edge_cases(pm, tables):
     from paper_1409_8336_b200 import PmcError
