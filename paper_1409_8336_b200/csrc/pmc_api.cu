@@ -203,8 +203,10 @@ int sync_tables(pmc_ctx *c) {
     c->smem_transport = ((size_t)2 * c->n_sr * c->n_e + (size_t)2 * c->n_sr * c->n_r + (size_t)nb * c->n_e) * 4 + (size_t)nb * sizeof(MatBin) +
                         lut.size() + 16;
     if (c->smem_transport > 200 * 1024) return fail(c, PMC_E_UNSUPPORTED, "tables too large for shared-memory staging");
-    CK(cudaFuncSetAttribute(transport_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_transport));
-    CK(cudaFuncSetAttribute(transport_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_transport));
+    CK(cudaFuncSetAttribute(transport_kernel<0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_transport));
+    CK(cudaFuncSetAttribute(transport_kernel<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_transport));
+    CK(cudaFuncSetAttribute(transport_kernel<0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_transport));
+    CK(cudaFuncSetAttribute(transport_kernel<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_transport));
   }
   CK(cudaStreamSynchronize(s));
   c->tables_dirty = false;
@@ -290,8 +292,12 @@ int run_generations(pmc_ctx *c, RunParams P, uint32_t n0, bool profile) {
     CK(cudaMemsetAsync(c->qel.q.count, 0, 4, s)); CK(cudaMemsetAsync(c->qne.q.count, 0, 4, s)); CK(cudaMemsetAsync(c->qres.q.count, 0, 4, s));
     CK(cudaMemsetAsync(c->qev.q.count, 0, 4, s));
     { Timer t(c, &c->timing.transport_ms, profile);
-      if (c->T.mcs_model == 1) transport_kernel<1><<<grid_t, TRANSPORT_THREADS, c->smem_transport, s>>>(c->T, c->G, P, cur->q, n_in, c->d_head.p, c->qev.q, c->d_tally.p, c->d_cnt.p);
-      else transport_kernel<0><<<grid_t, TRANSPORT_THREADS, c->smem_transport, s>>>(c->T, c->G, P, cur->q, n_in, c->d_head.p, c->qev.q, c->d_tally.p, c->d_cnt.p); }
+      const bool mol = c->T.mcs_model == 1, dbg = P.dbg_out != nullptr;
+#define PMC_LAUNCH_TRANSPORT(M, D) transport_kernel<M, D><<<grid_t, TRANSPORT_THREADS, c->smem_transport, s>>>(c->T, c->G, P, cur->q, n_in, c->d_head.p, c->qev.q, c->d_tally.p, c->d_cnt.p)
+      if (mol && dbg) PMC_LAUNCH_TRANSPORT(1, true); else if (mol) PMC_LAUNCH_TRANSPORT(1, false);
+      else if (dbg) PMC_LAUNCH_TRANSPORT(0, true); else PMC_LAUNCH_TRANSPORT(0, false);
+#undef PMC_LAUNCH_TRANSPORT
+    }
     c->timing.launches_total++; c->timing.launches_transport++;
     if (P.dbg_out) break;
     { Timer t(c, &c->timing.elastic_ms, profile);

@@ -274,7 +274,9 @@ constexpr int TRANSPORT_THREADS = 256, TRANSPORT_BLOCKS_PER_SM = 4;
 
 // MCS_MODEL: 0 = Highland (the paper's choice), 1 = full Moliere; a template so that the default kernel carries none of
 // the Moliere code or its registers
-template <int MCS_MODEL>
+// DBG: the pmc_first_steps variant (stop after max_steps, write the state of every primary); the production kernel
+// carries neither its registers nor its branches.
+template <int MCS_MODEL, bool DBG>
 __global__ void __launch_bounds__(TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM) transport_kernel(Tables T, Grid G, RunParams P, Queue in, uint32_t n_in,
                                                            uint32_t *head, Queue q_ev, float *tally, Counters *cnt) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -359,7 +361,7 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM) tr
       if (ell >= d2 || lim == 1) { L = tau + d2; p.r = p.r + d2 * dnew; cls = 1; }
       else { L = dx; p.r = p.r + ell * dnew; cls = lim; }
       p.r.x = fminf(fmaxf(p.r.x, 0.f), sz[0]); p.r.y = fminf(fmaxf(p.r.y, 0.f), sz[1]); p.r.z = fminf(fmaxf(p.r.z, 0.f), sz[2]);
-      p.d = dnew; path += L;
+      p.d = dnew; if (DBG) path += L;
       // ---- 6. energy loss from the range table (Eq.2) + straggling (L61)
       float loss;
       if (cls == 3) { loss = e0; let = L > 0.f ? fdiv(0.1f * e0, L) : 0.f; }   // 7. range-out: everything stays here (L71)
@@ -381,18 +383,18 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM) tr
         if (nidx < 0 || nidx >= nmax) { c_esc += (double)p.e; alive = false; }         // L71 (3)
         else p.vox = (iz * G.ny + iy) * G.nx + ix;
       }
-      ++nstep;
-      if (alive && cls == 2 && P.dbg_out == nullptr) {
+      if (DBG) ++nstep;
+      if (alive && cls == 2 && !DBG) {
         // ---- 8. discrete nuclear event at the end point (L71): handed to event_kernel, which picks the class and
         // the target element with all lanes busy instead of one lane of this warp
         p.blk = g.blk; p.vox = dep_vox; c_ev++;
         if (!queue_push(q_ev, p)) atomicOr(&cnt->overflow, 2u);
         alive = false;
       }
-      if (alive && P.max_steps > 0 && nstep >= P.max_steps) alive = false;
+      if (DBG && alive && P.max_steps > 0 && nstep >= P.max_steps) alive = false;
       if (!alive) {
         active = false;
-        if (P.dbg_out && p.pid == 0u) {
+        if (DBG && P.dbg_out && p.pid == 0u) {
           float *o = P.dbg_out + 8ull * p.hist;
           o[0] = ix * sz[0] + p.r.x; o[1] = iy * sz[1] + p.r.y; o[2] = iz * sz[2] + p.r.z;
           o[3] = p.d.x; o[4] = p.d.y; o[5] = p.d.z; o[6] = p.e; o[7] = path;
