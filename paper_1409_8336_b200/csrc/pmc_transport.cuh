@@ -300,8 +300,8 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM) tr
   const int lane = threadIdx.x & 31;
   bool active = false, exhausted = false;
   Particle p; Rng g; int ix = 0, iy = 0, iz = 0, nstep = 0; float path = 0.f; uint32_t tbase = 0;
-  unsigned long long c_steps = 0, c_ev = 0;
-  double c_dep = 0, c_esc = 0;
+  uint32_t c_steps = 0;                 // per-lane partial sums (a lane sees < 1e7 steps and < 1e4 MeV): 32-bit is enough
+  float c_dep = 0.f, c_esc = 0.f;
   const bool nuclear = T.opt_el || T.opt_ne;
 
   while (true) {
@@ -374,20 +374,20 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM) tr
       p.e = e0 - loss; dep = loss;
       bool alive = cls != 3;
       if (alive && p.e <= T.e_cut) { dep += p.e; p.e = 0.f; alive = false; }           // L71 (2)
-      c_dep += (double)dep;
+      c_dep += dep;
       if (alive && cls == 1) {                                                        // boundary: next voxel
         int nidx, nmax;
         if (ax2 == 0) { ix += sg2; nidx = ix; nmax = G.nx; p.r.x = sg2 > 0 ? 0.f : sz[0]; }
         else if (ax2 == 1) { iy += sg2; nidx = iy; nmax = G.ny; p.r.y = sg2 > 0 ? 0.f : sz[1]; }
         else { iz += sg2; nidx = iz; nmax = G.nz; p.r.z = sg2 > 0 ? 0.f : sz[2]; }
-        if (nidx < 0 || nidx >= nmax) { c_esc += (double)p.e; alive = false; }         // L71 (3)
+        if (nidx < 0 || nidx >= nmax) { c_esc += p.e; alive = false; }         // L71 (3)
         else p.vox = (iz * G.ny + iy) * G.nx + ix;
       }
       if (DBG) ++nstep;
       if (alive && cls == 2 && !DBG) {
         // ---- 8. discrete nuclear event at the end point (L71): handed to event_kernel, which picks the class and
         // the target element with all lanes busy instead of one lane of this warp
-        p.blk = g.blk; p.vox = dep_vox; c_ev++;
+        p.blk = g.blk; p.vox = dep_vox;
         if (!queue_push(q_ev, p)) atomicOr(&cnt->overflow, 2u);
         alive = false;
       }
@@ -404,8 +404,8 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM) tr
     deposit(tally, tbase + (uint32_t)dep_vox, dep, dep != 0.f, P.aggregate, P.let_num, P.let_den, (uint32_t)dep_vox, let > 0.f ? dep : 0.f, let);
     if (P.roi_map != nullptr && dep != 0.f) score_influence(P, p.aux, dep_vox, dep);
   }
-  flush(&cnt->n_steps, c_steps); (void)c_ev;
-  flush(&cnt->e_deposit, c_dep); flush(&cnt->e_escape, c_esc);
+  flush(&cnt->n_steps, (unsigned long long)c_steps);
+  flush(&cnt->e_deposit, (double)c_dep); flush(&cnt->e_escape, (double)c_esc);
 }
 
 // ------------------------------------------------------------------ event class and target element (Reading R5)
