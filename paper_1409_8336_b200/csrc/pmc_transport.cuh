@@ -299,7 +299,7 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM) tr
   const float sz[3] = {G.d[0], G.d[1], G.d[2]};
   const int lane = threadIdx.x & 31;
   bool active = false, exhausted = false;
-  Particle p; Rng g; int ix = 0, iy = 0, iz = 0, nstep = 0; float path = 0.f; uint32_t tbase = 0;
+  Particle p; int ix = 0, iy = 0, iz = 0, nstep = 0; float path = 0.f; uint32_t tbase = 0;
   uint32_t c_steps = 0;                 // per-lane partial sums (a lane sees < 1e7 steps and < 1e4 MeV): 32-bit is enough
   float c_dep = 0.f, c_esc = 0.f;
   const bool nuclear = T.opt_el || T.opt_ne;
@@ -315,7 +315,6 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM) tr
         const uint32_t idx = base + (uint32_t)__popc(need & ((1u << lane) - 1u));
         if (idx < n_in) {
           p = queue_load(in, idx);
-          g.init(P.seed, P.hist0 + p.hist, p.pid, p.blk);
           int t; divmod(p.vox, G.nx, P.inv_nx, t, ix); divmod(t, G.ny, P.inv_ny, iz, iy);
           active = true; nstep = 0; path = 0.f; tbase = batch_base(P, p.hist);
         } else exhausted = true;
@@ -325,6 +324,8 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM) tr
 
     float dep = 0.f, let = 0.f; int dep_vox = p.vox;
     if (active) {
+      // the stream is re-keyed from (seed, history, particle, block) every step: only the block counter lives across steps
+      Rng g; g.init(P.seed, P.hist0 + p.hist, p.pid, p.blk);
       // ---- material of the current voxel
       const int hu = G.hu[p.vox];
       const int bin = hu_to_bin(T, s_lut, hu);
@@ -392,6 +393,7 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM) tr
         alive = false;
       }
       if (DBG && alive && P.max_steps > 0 && nstep >= P.max_steps) alive = false;
+      p.blk = g.blk;
       if (!alive) {
         active = false;
         if (DBG && P.dbg_out && p.pid == 0u) {
