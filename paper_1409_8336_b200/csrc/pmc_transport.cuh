@@ -163,19 +163,20 @@ __global__ void __launch_bounds__(256) sampler_kernel(Tables T, Grid G, const Sp
     int lo = 0, hi = nspots - 1;
     while (lo < hi) { int mid = (lo + hi) >> 1; if (cdf[mid] < us) lo = mid + 1; else hi = mid; }
     const SpotDev sp = spots[lo];
-    const double rr = sqrt(-2.0 * log(u01d(r.y)));
-    double s2, c2; sincospi(2.0 * u01d(r.z), &s2, &c2);
+    // Gaussian deviates in fp32 (relative error 1e-7 of sigma), accumulated onto the fp64 spot position
+    const double rr = (double)sqrtf(-2.0f * logf(u01(r.y)));
+    float s2f, c2f; sincospif(2.0f * u01(r.z), &s2f, &c2f); const double s2 = s2f, c2 = c2f;
     double pos[3], dir[3];
     for (int k = 0; k < 3; ++k) { pos[k] = sp.pos[k] + sp.sx * rr * c2 * sp.ex[k] + sp.sy * rr * s2 * sp.ey[k]; dir[k] = sp.ax[k]; }
     if (sp.divx > 0 || sp.divy > 0) {
       uint4 q = g.next4();
-      const double r2 = sqrt(-2.0 * log(u01d(q.x))); double s4, c4; sincospi(2.0 * u01d(q.y), &s4, &c4);
+      const double r2 = (double)sqrtf(-2.0f * logf(u01(q.x))); float s4f, c4f; sincospif(2.0f * u01(q.y), &s4f, &c4f); const double s4 = s4f, c4 = c4f;
       double n2 = 0;
       for (int k = 0; k < 3; ++k) { dir[k] = sp.ax[k] + sp.divx * r2 * c4 * sp.ex[k] + sp.divy * r2 * s4 * sp.ey[k]; n2 += dir[k] * dir[k]; }
       n2 = 1.0 / sqrt(n2); for (int k = 0; k < 3; ++k) dir[k] *= n2;
     }
     double E = sp.e;
-    if (sp.sigma_e > 0) { uint4 q = g.next4(); E += sp.sigma_e * sqrt(-2.0 * log(u01d(q.x))) * cospi(2.0 * u01d(q.y)); }
+    if (sp.sigma_e > 0) { uint4 q = g.next4(); E += sp.sigma_e * (double)(sqrtf(-2.0f * logf(u01(q.x))) * cospif(2.0f * u01(q.y))); }
     E = fmax(E, 0.0);
     e_src = E;
     const double size[3] = {G.nx * (double)G.d[0], G.ny * (double)G.d[1], G.nz * (double)G.d[2]};
