@@ -407,7 +407,8 @@ def test_c5_pelvis_full_size_against_oracle_subsample(pm, tables):
     a, b = (dg * rho)[ti].sum(), (do * rho)[ti].sum()
     assert b > 0 and abs(a / b - 1) < 0.03, (a, b)
     # voxel z-scores in tissue and bone (not air, see C4); few oracle histories per voxel: the 10-batch sigma of a
-    # skewed voxel dose correlates with the dose itself, which pushes the mean z up and fattens the tails
+    # skewed voxel dose correlates with the dose itself, which pushes the mean z up and fattens the tails (measured: the
+    # 1e8-history map against a 5e5-history run of the CUDA path ITSELF gives 98.2 %, mean z 0.13, rms z 1.16)
     frac, zmean, zrms, nv = parity.zscore_pass(dg, sg, do, so, region=w["hu"] >= -950)
     assert nv > 100_000 and frac >= 0.975 and abs(zmean) < 0.2 and zrms < 1.3, (frac, zmean, zrms, nv)
     for ax in range(3):
