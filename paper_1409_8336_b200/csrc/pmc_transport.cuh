@@ -528,20 +528,42 @@ __global__ void __launch_bounds__(256) elastic_kernel(Tables T, RunParams P, Que
 // deviations over the B batches (Welford), then mean dose and standard error.
 __global__ void __launch_bounds__(256) stats_kernel(Tables T, Grid G, const float *tally, float *dose, float *sigma, int B,
                                                     uint64_t n_total, uint32_t nvox) {
-  for (uint32_t v = blockIdx.x * blockDim.x + threadIdx.x; v < nvox; v += gridDim.x * blockDim.x) {
-    const int hu = G.hu[v];
-    const MatBin &m = T.bins[hu_to_bin(T, T.hu_lut, hu)];
-    const float inv_m = 1.602176634e-10f / (bin_density(m, hu) * G.vol);
-    float mu = 0.f, s = 0.f;
+  // four consecutive voxels per thread (16-byte loads from each batch grid keep enough bytes in flight for HBM);
+  // a ragged tail or an unaligned grid size falls back to one voxel per thread
+  const bool vec = (nvox & 3u) == 0u;
+  const uint32_t nitems = vec ? nvox >> 2 : nvox;
+  const float ib = 1.0f / ((float)B * (float)(B - 1));
+  for (uint32_t it = blockIdx.x * blockDim.x + threadIdx.x; it < nitems; it += gridDim.x * blockDim.x) {
+    const uint32_t v0 = vec ? it << 2 : it; const int nv = vec ? 4 : 1;
+    float inv_m[4], mu[4] = {0.f, 0.f, 0.f, 0.f}, s[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      if (k < nv) {
+        const int hu = G.hu[v0 + k];
+        const MatBin &m = T.bins[hu_to_bin(T, T.hu_lut, hu)];
+        inv_m[k] = 1.602176634e-10f / (bin_density(m, hu) * G.vol);
+      } else inv_m[k] = 0.f;
+    }
     for (int b = 0; b < B; ++b) {
       const uint64_t h0 = ((uint64_t)b * n_total + B - 1) / B, h1 = ((uint64_t)(b + 1) * n_total + B - 1) / B;
-      const float t = tally[(size_t)b * nvox + v];
-      const float d = h1 > h0 ? t * inv_m / (float)(h1 - h0) : 0.f;
-      const float delta = d - mu; mu += delta / (float)(b + 1); s += delta * (d - mu);
+      const float inb = h1 > h0 ? 1.0f / (float)(h1 - h0) : 0.f, ibp = 1.0f / (float)(b + 1);
+      float t[4] = {0.f, 0.f, 0.f, 0.f};
+      if (vec) { const float4 q = *reinterpret_cast<const float4 *>(tally + (size_t)b * nvox + v0); t[0] = q.x; t[1] = q.y; t[2] = q.z; t[3] = q.w; }
+      else t[0] = tally[(size_t)b * nvox + v0];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        const float d = t[k] * inv_m[k] * inb;
+        const float delta = d - mu[k]; mu[k] += delta * ibp; s[k] += delta * (d - mu[k]);
+      }
     }
-    dose[v] = mu;
-    const float var = s / ((float)B * (float)(B - 1));
-    sigma[v] = var > 0.f ? sqrtf(var) : 0.f;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      if (k < nv) {
+        dose[v0 + k] = mu[k];
+        const float var = s[k] * ib;
+        sigma[v0 + k] = var > 0.f ? sqrtf(var) : 0.f;
+      }
+    }
   }
 }
 
