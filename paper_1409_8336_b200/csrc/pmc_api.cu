@@ -544,7 +544,7 @@ static int simulate_impl(pmc_ctx *c, const pmc_spot *spots_in, int nspots, uint6
     P.b_over_n = (float)((double)B / (double)n); P.inv_nx = 1.0f / (float)c->G.nx; P.inv_ny = 1.0f / (float)c->G.ny;
     CK(cudaMemsetAsync(c->qa.q.count, 0, 4, s));
     { Timer t(c, &c->timing.sampler_ms, profile);
-      sampler_kernel<<<(nc + 255) / 256, 256, 0, s>>>(c->T, c->G, c->d_spots.p, c->d_cdf.p, nspots, P, c->qa.q, c->d_cnt.p, air_rho, air_wf, air_ix0, air_zoa, air_tab); }
+      sampler_kernel<<<(int)std::min<uint32_t>((nc + 255) / 256, (uint32_t)c->n_sm * 8), 256, 0, s>>>(c->T, c->G, c->d_spots.p, c->d_cdf.p, nspots, P, c->qa.q, c->d_cnt.p, air_rho, air_wf, air_ix0, air_zoa, air_tab); }
     c->timing.launches_total++;
     CK(cudaMemcpyAsync(c->h_pinned, c->qa.q.count, 4, cudaMemcpyDeviceToHost, s));
     CK(cudaStreamSynchronize(s));

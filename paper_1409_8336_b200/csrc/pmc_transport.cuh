@@ -152,8 +152,15 @@ __device__ __forceinline__ double u01d(uint32_t x) { return ((double)x + 0.5) * 
 __global__ void __launch_bounds__(256) sampler_kernel(Tables T, Grid G, const SpotDev *spots, const double *cdf, int nspots,
                                                      RunParams P, Queue out, Counters *cnt, float air_rho, float air_wf,
                                                      float air_inv_x0, float air_zoa, int air_table) {
-  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  // Block-stride loop (same trip count for every thread of a block) so that a block makes ONE allocation in the
+  // output queue per trip and one ledger flush per warp at the end: 3e5 same-address atomics per 1e7 histories cost
+  // more than the sampling itself.
+  __shared__ uint32_t s_cnt[8], s_base;
   double e_src = 0, e_esc = 0, e_air = 0; unsigned long long missed = 0;
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  for (uint32_t i0 = blockIdx.x * blockDim.x; i0 < P.n; i0 += gridDim.x * blockDim.x) {
+  const uint32_t i = i0 + threadIdx.x;
+  bool push = false; Particle p{};
   if (i < P.n) {
     const uint64_t hist = P.hist0 + i;
     Rng g; g.init(P.seed, hist, 0u, 0u);
@@ -178,7 +185,7 @@ __global__ void __launch_bounds__(256) sampler_kernel(Tables T, Grid G, const Sp
     double E = sp.e;
     if (sp.sigma_e > 0) { uint4 q = g.next4(); E += sp.sigma_e * (double)(sqrtf(-2.0f * logf(u01(q.x))) * cospif(2.0f * u01(q.y))); }
     E = fmax(E, 0.0);
-    e_src = E;
+    e_src += E;
     const double size[3] = {G.nx * (double)G.d[0], G.ny * (double)G.d[1], G.nz * (double)G.d[2]};
     auto ray_box = [&](const double *o, const double *dd, double &tin) {
       double t0 = 0, t1 = 1e300;
@@ -191,7 +198,7 @@ __global__ void __launch_bounds__(256) sampler_kernel(Tables T, Grid G, const Sp
       tin = t0; return t0 < t1;
     };
     double tin; bool ok = ray_box(pos, dir, tin);
-    if (!ok) { e_esc = E; missed = 1; }
+    if (!ok) { e_esc += E; missed += 1; }
     else if (tin > 0) {
       // single air step to the CT edge: hinge, Highland, mean loss + straggling
       uint4 q = g.next4();
@@ -203,7 +210,7 @@ __global__ void __launch_bounds__(256) sampler_kernel(Tables T, Grid G, const Sp
         dn[0] = d1.x; dn[1] = d1.y; dn[2] = d1.z;
       }
       double t2;
-      if (!ray_box(rh, dn, t2)) { e_esc = E; missed = 1; ok = false; }
+      if (!ray_box(rh, dn, t2)) { e_esc += E; missed += 1; ok = false; }
       else {
         const double L = tau + t2;
         for (int k = 0; k < 3; ++k) { pos[k] = rh[k] + t2 * dn[k]; dir[k] = dn[k]; }
@@ -211,12 +218,12 @@ __global__ void __launch_bounds__(256) sampler_kernel(Tables T, Grid G, const Sp
         const float lnRv = ln_range(T, T.lnR, T.lnR2, air_table, e_index(T, lnEv)), Rg = expf(lnRv);
         float loss = mean_loss(T, T.lnE, T.lnE2, air_table, ef, lnEv, lnRv, Rg, (float)L * air_wf);
         if (T.opt_strag) loss = straggle(T, g, ef, loss, (float)L * air_rho, air_zoa, low_bytes(q));
-        e_air = loss; E -= loss;
+        e_air += loss; E -= loss;
         if (E <= T.e_cut) { e_air += E; ok = false; }
       }
     }
     if (ok) {
-      Particle p; int idx[3]; const int nn[3] = {G.nx, G.ny, G.nz}; float loc[3];
+      int idx[3]; const int nn[3] = {G.nx, G.ny, G.nz}; float loc[3];
       for (int k = 0; k < 3; ++k) {
         const double rv = fmin(fmax(pos[k], 0.0), size[k]), dk = (double)G.d[k];
         int ii = (int)floor(rv / dk);
@@ -227,8 +234,27 @@ __global__ void __launch_bounds__(256) sampler_kernel(Tables T, Grid G, const Sp
       p.r = {loc[0], loc[1], loc[2]}; p.d = unit(V3{(float)dir[0], (float)dir[1], (float)dir[2]}); p.e = (float)E;
       p.vox = (idx[2] * G.ny + idx[1]) * G.nx + idx[0];
       p.hist = i; p.pid = 0u; p.blk = g.blk; p.aux = (uint32_t)lo << 8;
-      if (!queue_push(out, p)) atomicOr(&cnt->overflow, 1u);
+      push = true;
     }
+  }
+  // one queue allocation per block and trip
+  const unsigned wm = __ballot_sync(0xffffffffu, push);
+  if (lane == 0) s_cnt[wid] = (uint32_t)__popc(wm);
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    uint32_t tot = 0;
+    for (int k = 0; k < (int)(blockDim.x >> 5); ++k) { const uint32_t c = s_cnt[k]; s_cnt[k] = tot; tot += c; }
+    s_base = tot ? atomicAdd(out.count, tot) : 0u;
+  }
+  __syncthreads();
+  if (push) {
+    const uint32_t slot = s_base + s_cnt[wid] + (uint32_t)__popc(wm & ((1u << lane) - 1u));
+    if (slot < out.cap) {
+      out.x[slot] = p.r.x; out.y[slot] = p.r.y; out.z[slot] = p.r.z; out.u[slot] = p.d.x; out.v[slot] = p.d.y; out.w[slot] = p.d.z;
+      out.e[slot] = p.e; out.vox[slot] = p.vox; out.hist[slot] = p.hist; out.pid[slot] = p.pid; out.blk[slot] = p.blk; out.aux[slot] = p.aux;
+    } else atomicOr(&cnt->overflow, 1u);
+  }
+  __syncthreads();
   }
   flush(&cnt->e_source, e_src); flush(&cnt->e_escape, e_esc); flush(&cnt->e_air, e_air); flush(&cnt->n_missed, missed);
 }
