@@ -29,8 +29,8 @@ UNIT = "histories/s"
 # algorithmic thread-instructions of one condensed-history step of the transport kernel
 ALGO_INST_PER_STEP = 520.0
 # dram__bytes_read.sum + dram__bytes_write.sum of the first-generation transport launch of a 1e7-history C4 step, per
-# history (one `ncu --set full` capture, profiles/r01_transport_full.md): 546.2 MB + 117.7 MB
-NCU_DRAM_BYTES_PER_HISTORY_C4 = 66.4
+# history (one `ncu --set full` capture, profiles/r01_transport_full.md): 641.4 MB + 186.3 MB
+NCU_DRAM_BYTES_PER_HISTORY_C4 = 82.8
 ISSUE_LANES_PER_SM_PER_CLK = 128.0     # 4 schedulers x 32 lanes
 N_SM = 148
 
