@@ -47,7 +47,8 @@ class Counters(C.Structure):
                                           "n_missed", "n_inc_tries")] + \
                [(k, C.c_double) for k in ("e_source", "e_deposit", "e_escape", "e_neutron", "e_gamma", "e_q", "e_air",
                                           "max_ledger_residual", "max_event_residual")] + \
-               [("n_zab_violations", C.c_uint64)]
+               [(k, C.c_uint64) for k in ("n_zab_violations", "n_inc_guard_trips", "n_inc_stack_trips", "inc_max_stack",
+                                          "inc_max_out")]
 
 
 SECONDARY_DTYPE = np.dtype([("Z", "<i2"), ("A", "<i2"), ("origin", "u1"), ("pad", "u1", (3,)),
@@ -86,6 +87,27 @@ def cugnon(which, p_gev):
 def inc_uniform_sphere(radius_fm, rho_fm3, sigma_mb, t_mev, n, seed):
     return _load().opmc_test_inc_uniform_sphere(C.c_double(radius_fm), C.c_double(rho_fm3), C.c_double(sigma_mb),
                                                 C.c_double(t_mev), C.c_uint64(n), C.c_uint64(seed))
+
+
+def nn_cos(same_type, p_lab_gev, pcm_mev, n, seed):
+    out = np.zeros(n)
+    _load().opmc_test_nn_cos(C.c_int(int(same_type)), C.c_double(p_lab_gev), C.c_double(pcm_mev), C.c_uint64(n),
+                             C.c_uint64(seed), _dp(out))
+    return out
+
+
+def inc_custom(rout, rho, pF, V, t_in, n, seed, coulomb=-1e9, pauli=False, const_sigma_mb=-1.0):
+    """Cascade attempts on a hand-made shell nucleus; rho, pF, V have shape (2, nshell) (proton row, neutron row).
+    Returns (n_out[n], rec[n][4][5]) with rec = type (0 p, 1 n), KE, direction of the first four outgoing nucleons;
+    n_out < 0 marks a rejected attempt with -1 - n_out nucleons out."""
+    rout = np.ascontiguousarray(rout, dtype=np.float64); ns = rout.size
+    arrs = [np.ascontiguousarray(a, dtype=np.float64).reshape(2, ns) for a in (rho, pF, V)]
+    out_n = np.zeros(n, dtype=np.int32); rec = np.zeros((n, 4, 5))
+    rc = _load().opmc_test_inc_custom(C.c_int(ns), _dp(rout), _dp(arrs[0]), _dp(arrs[1]), _dp(arrs[2]), C.c_double(coulomb),
+                                      C.c_int(int(pauli)), C.c_double(const_sigma_mb), C.c_double(t_in), C.c_uint64(n),
+                                      C.c_uint64(seed), out_n.ctypes.data_as(_I), _dp(rec))
+    assert rc == 0
+    return out_n, rec
 
 
 class Oracle:
@@ -210,6 +232,18 @@ class Oracle:
         out = np.zeros((n, 4))
         self.lib.opmc_test_elastic(self.ctx, Z, A, C.c_double(t_mev), C.c_uint64(n), C.c_uint64(seed), _dp(out))
         return out
+
+    def sample_primaries(self, spots, n, seed):
+        spots = np.ascontiguousarray(spots, dtype=np.float64)
+        out = np.zeros((n, 8))
+        assert self.lib.opmc_test_sample_primaries(self.ctx, spots.ctypes.data_as(C.c_void_p), spots.shape[0], C.c_uint64(n),
+                                                   C.c_uint64(seed), _dp(out)) == 0
+        return out
+
+    def event_counts(self):
+        out = np.zeros(16, dtype=np.uint64)
+        self.lib.opmc_test_event_counts(self.ctx, out.ctypes.data_as(C.POINTER(C.c_uint64)))
+        return out[:8].astype(np.int64), out[8:].astype(np.int64)
 
     def nucleus(self, Z, A):
         out = np.zeros((15, 6))

@@ -183,6 +183,7 @@ struct Nucleus {
   double rmax = 0, rout[NSHELL_MAX], rho[2][NSHELL_MAX], pF[2][NSHELL_MAX], EF[2][NSHELL_MAX], V[2][NSHELL_MAX];
   double coulomb = 0;                           // B_C for protons
   bool pauli = true; double const_sigma_mb = -1;  // test switches (closed-form pin only)
+  long step_guard = 1024;                       // Reading R6.8; option "inc_step_guard" (pin test of the guard only)
 };
 inline double nucleon_mass(int type) { return type == 0 ? MP : MN; }   // type 0 = proton, 1 = neutron
 
@@ -221,13 +222,18 @@ Nucleus build_nucleus(const Tables &T, int Z, int A) {
 struct Sec { int Z, A, origin; double ke; V3 dir; };
 struct Residual { int Z, A; double estar; V3 P; double mass_gs; };
 
-struct EventCheck { double max_resid = 0; uint64_t zab_bad = 0; uint64_t inc_tries = 0; };
+struct EventCheck {
+  double max_resid = 0; uint64_t zab_bad = 0; uint64_t inc_tries = 0;
+  // how often the limits of Reading R6.8 end an attempt, and how deep a cascade gets (bookkeeping only)
+  uint64_t guard_trips = 0, stack_trips = 0, max_stack = 0, max_out = 0;
+};
 
 // ------------------------------------------------------------------ INC (Reading R6)
 struct CascNucleon { int type; V3 r, p; int shell; };
 
 // one attempt; returns false if no Pauli-allowed collision happened or the outcome is invalid
-bool inc_attempt(const Tables &T, const Nucleus &N, double t_in, Rng &g, std::vector<Sec> &out, Residual &res) {
+bool inc_attempt(const Tables &T, const Nucleus &N, double t_in, Rng &g, std::vector<Sec> &out, Residual &res,
+                 EventCheck *chk = nullptr) {
   out.clear();
   const int ns = N.nshell;
   // entry: uniform over the disc of radius rmax, travelling along +z (L75 "random point of entry")
@@ -249,7 +255,7 @@ bool inc_attempt(const Tables &T, const Nucleus &N, double t_in, Rng &g, std::ve
     CascNucleon c = stack.back(); stack.pop_back();
     bool alive = true;
     while (alive) {
-      if (++guard > 1024) return false;      // Reading R6.8: a nucleon on a bound orbit in a dilute shell never ends the attempt
+      if (++guard > N.step_guard) { if (chk) chk->guard_trips++; return false; }   // Reading R6.8: a nucleon on a bound orbit in a dilute shell never ends the attempt
       int k = c.shell, ty = c.type;
       double m = nucleon_mass(ty), p2 = dot(c.p, c.p), E = std::sqrt(p2 + m * m), Tk = E - m;
       V3 d = (1.0 / std::sqrt(p2)) * c.p;
@@ -298,7 +304,8 @@ bool inc_attempt(const Tables &T, const Nucleus &N, double t_in, Rng &g, std::ve
         double bc2 = tp == 0 ? N.coulomb : 0.0, bc1 = ty == 0 ? N.coulomb : 0.0;
         if (T2 - N.V[tp][k] > bc2) stack.push_back({tp, c.r, n2, k});
         if (T1 - N.V[ty][k] > bc1) { c.p = n1; } else alive = false;
-        if ((int)stack.size() > 200) return false;
+        if (chk) chk->max_stack = std::max<uint64_t>(chk->max_stack, stack.size());
+        if ((int)stack.size() > 200) { if (chk) chk->stack_trips++; return false; }
         continue;
       }
       // ---- shell boundary (L77 "reflection and refraction", Reading R6.5)
@@ -319,6 +326,7 @@ bool inc_attempt(const Tables &T, const Nucleus &N, double t_in, Rng &g, std::ve
       } else { c.p = pnew; c.shell = k2; }
     }
   }
+  if (chk) chk->max_out = std::max<uint64_t>(chk->max_out, (uint64_t)n_out);
   if (ncoll == 0) return false;                                        // L75: need >= 1 allowed collision
   // ---- residual nucleus (Reading R6.7): exact integers, relativistic invariant mass
   int Ar = N.A + 1 - n_out, Zr = N.Z + 1 - np_out;
@@ -338,7 +346,7 @@ bool inc_attempt(const Tables &T, const Nucleus &N, double t_in, Rng &g, std::ve
 void inc_event(const Tables &T, const Nucleus &N, double t_in, Rng &g, std::vector<Sec> &out, Residual &res, EventCheck &chk) {
   for (int tries = 0; tries < 100000; ++tries) {   // L75 "This is repeated until ..."
     chk.inc_tries++;
-    if (inc_attempt(T, N, t_in, g, out, res)) return;
+    if (inc_attempt(T, N, t_in, g, out, res, &chk)) return;
   }
   // Reading R6.8 (never reached in the configs): give up and form the compound nucleus (Z+1, A+1)
   out.clear();
@@ -500,6 +508,8 @@ struct opmc_ctx {
   std::vector<int32_t> roi_vox, roi_map; std::vector<double> dij; int dij_spots = 0;
   int mcs_model = 0;                          // 0 Highland x 1.07 (the paper's results), 1 full Moliere (L59; Reading R12)
   bool score_let = false; std::vector<double> let_num, let_den;   // LET_d tallies (Reading R9)
+  long inc_step_guard = 1024;                 // Reading R6.8 (option "inc_step_guard": pin test of the guard only)
+  uint64_t ev_el[OPMC_MAX_ELEM] = {0}, ev_ne[OPMC_MAX_ELEM] = {0};   // events per class and target element (pin test bookkeeping)
   opmc_counters cnt{};
   std::string err;
 };
@@ -698,6 +708,11 @@ bool transport_step(opmc_ctx *c, Particle &p, Rng &g, double *tally, Ledger &led
   double u = g.u() * sum; int el = -1;
   for (int i = 0; i < T.n_elem; ++i) if (pe[i] > 0) { el = i; if (u < pe[i]) break; u -= pe[i]; }
   int Z = T.ez[el], A = T.ea[el];
+  {
+    uint64_t &tally_ev = (is_el ? c->ev_el : c->ev_ne)[el];
+    #pragma omp atomic
+    tally_ev++;
+  }
   auto deposit_here = [&](double e) {
     #pragma omp atomic
     tally[vox] += e;
@@ -850,6 +865,8 @@ void merge(opmc_counters &a, const opmc_counters &b, const EventCheck &chk) {
   a.max_ledger_residual = std::max(a.max_ledger_residual, b.max_ledger_residual);
   a.max_event_residual = std::max(a.max_event_residual, chk.max_resid);
   a.n_zab_violations += chk.zab_bad;
+  a.n_inc_guard_trips += chk.guard_trips; a.n_inc_stack_trips += chk.stack_trips;
+  a.inc_max_stack = std::max(a.inc_max_stack, chk.max_stack); a.inc_max_out = std::max(a.inc_max_out, chk.max_out);
 }
 
 int fail(opmc_ctx *c, const char *msg) { if (c) c->err = msg; return -1; }
@@ -892,6 +909,7 @@ int opmc_load_physics_tables(opmc_ctx *c, const opmc_tables *t) {
   for (int i = 0; i < T.n_elem; ++i) if (T.ea[i] > 1) {
     if (T.nmass(T.ez[i], T.ea[i]) <= 0) return fail(c, "element missing from mass table");
     c->nuc[i] = build_nucleus(T, T.ez[i], T.ea[i]);
+    c->nuc[i].step_guard = c->inc_step_guard;
   }
   T.loaded = true;
   return 0;
@@ -931,6 +949,7 @@ int opmc_set_option(opmc_ctx *c, const char *key, double v) {
   else if (k == "elastic") c->opt_el = v != 0; else if (k == "nonelastic") c->opt_ne = v != 0;
   else if (k == "s_max_wet_cm") c->T.s_max = v; else if (k == "n_batches") c->T.n_batches = (int)v;
   else if (k == "threads") c->threads = (int)v; else if (k == "score_letd") c->score_let = v != 0;
+  else if (k == "inc_step_guard") { if (v < 1) return fail(c, "inc_step_guard must be >= 1"); c->inc_step_guard = (long)v; for (Nucleus &n : c->nuc) n.step_guard = c->inc_step_guard; }
   else if (k == "mcs_model") { if ((v != 0 && v != 1) || (v == 1 && c->T.mol_c0.empty())) return fail(c, "mcs_model: 0 or 1 (1 needs the Moliere tables)"); c->mcs_model = (int)v; }
   else return fail(c, "unknown option");
   return 0;
@@ -943,6 +962,7 @@ int opmc_simulate(opmc_ctx *c, const opmc_spot *spots, int nspots, uint64_t n, u
   if (B < 2) return fail(c, "need >= 2 batches");
   std::vector<double> cdf = spot_cdf(spots, nspots), tally(nv), s1(nv, 0.0), s2(nv, 0.0);
   c->cnt = opmc_counters{};
+  for (int i = 0; i < OPMC_MAX_ELEM; ++i) { c->ev_el[i] = 0; c->ev_ne[i] = 0; }
   if (c->score_let) { c->let_num.assign(nv, 0.0); c->let_den.assign(nv, 0.0); }
   c->dij_spots = nspots;
   if (!c->roi_map.empty()) c->dij.assign((size_t)nspots * c->roi_vox.size(), 0.0);
@@ -989,6 +1009,7 @@ int opmc_nonelastic(opmc_ctx *c, int Z, int A, double e, uint64_t n, uint64_t se
   if (!c->T.loaded) return fail(c, "load physics tables first");
   if (A < 2 || c->T.nmass(Z, A) <= 0 || c->T.nmass(Z - 1, A - 1) <= 0 || c->T.nmass(Z, A - 1) <= 0) return fail(c, "unsupported target");
   Nucleus N = build_nucleus(c->T, Z, A);
+  N.step_guard = c->inc_step_guard;
   c->cnt = opmc_counters{};
   EventCheck chk; uint64_t pos = 0; bool overflow = false;
   for (uint64_t ev = 0; ev < n; ++ev) {
@@ -1007,6 +1028,7 @@ int opmc_nonelastic(opmc_ctx *c, int Z, int A, double e, uint64_t n, uint64_t se
   }
   off[n] = (uint32_t)pos; *n_out = pos;
   c->cnt.n_nonelastic = n; c->cnt.n_inc_tries = chk.inc_tries; c->cnt.max_event_residual = chk.max_resid; c->cnt.n_zab_violations = chk.zab_bad;
+  c->cnt.n_inc_guard_trips = chk.guard_trips; c->cnt.n_inc_stack_trips = chk.stack_trips; c->cnt.inc_max_stack = chk.max_stack; c->cnt.inc_max_out = chk.max_out;
   if (overflow) return fail(c, "capacity too small"), -3;
   return 0;
 }
@@ -1101,6 +1123,58 @@ int opmc_test_evap_first(opmc_ctx *c, int Z, int A, double estar, uint32_t mask,
     Rng g(seed, i, 0); Residual R{Z, A, estar, V3{0, 0, 0}, c->T.nmass(Z, A)}; Sec s; double e = 0, cs = 0;
     och[i] = evap_emit(c->T, R, g, mask, s, &e, &cs); oeps[i] = e; ocos[i] = cs;
   }
+  return 0;
+}
+// n samples of cos(theta_cm) of NN elastic scattering at lab momentum p_lab (GeV/c) and CM momentum pcm (MeV/c)
+int opmc_test_nn_cos(int same_type, double p_lab_gev, double pcm_mev, uint64_t n, uint64_t seed, double *out) {
+  for (uint64_t i = 0; i < n; ++i) { Rng g(seed, i, 0); out[i] = sample_nn_cos(g, same_type != 0, p_lab_gev, pcm_mev); }
+  return 0;
+}
+// Cascade attempts on a hand-made nucleus of ns concentric shells (outer radii rout[ns]; per nucleon type t = 0 proton,
+// 1 neutron: density rho[t*ns+k], Fermi momentum pF[t*ns+k], potential depth V[t*ns+k]); incident proton of kinetic
+// energy t_in.  Attempt i uses the stream (seed, i).  out_n[i] = number of nucleons that left the nucleus, or -1 - that
+// number when the attempt was rejected; out_rec[i][4][5] = type, kinetic energy, direction of the first four of them.
+int opmc_test_inc_custom(int ns, const double *rout, const double *rho, const double *pF, const double *V, double coulomb,
+                         int pauli, double const_sigma_mb, double t_in, uint64_t n, uint64_t seed, int32_t *out_n,
+                         double *out_rec) {
+  if (ns < 1 || ns > NSHELL_MAX) return -1;
+  Tables T; T.zdim = 2; T.adim = 2; T.mass = {0, MN, 0, MP};
+  Nucleus N; N.Z = 0; N.A = 1; N.nshell = ns; N.rmax = rout[ns - 1]; N.pauli = pauli != 0; N.const_sigma_mb = const_sigma_mb;
+  N.coulomb = coulomb;
+  for (int t = 0; t < 2; ++t) for (int k = 0; k < ns; ++k) {
+    const double m = nucleon_mass(t);
+    N.rout[k] = rout[k]; N.rho[t][k] = rho[t * ns + k]; N.pF[t][k] = pF[t * ns + k]; N.V[t][k] = V[t * ns + k];
+    N.EF[t][k] = std::sqrt(N.pF[t][k] * N.pF[t][k] + m * m) - m;
+  }
+  for (uint64_t i = 0; i < n; ++i) {
+    Rng g(seed, i, 0); std::vector<Sec> o; Residual R;
+    const bool ok = inc_attempt(T, N, t_in, g, o, R);
+    out_n[i] = ok ? (int32_t)o.size() : -1 - (int32_t)o.size();
+    for (size_t k = 0; k < 4; ++k) {
+      double *r = out_rec + (i * 4 + k) * 5;
+      if (k < o.size()) { r[0] = o[k].Z == 1 ? 0 : 1; r[1] = o[k].ke; r[2] = o[k].dir.x; r[3] = o[k].dir.y; r[4] = o[k].dir.z; }
+      else { r[0] = -1; r[1] = r[2] = r[3] = r[4] = 0; }
+    }
+  }
+  return 0;
+}
+// n primaries of a multi-spot plan straight from the beam-spot sampler: out[n][8] = spot index, x, y, z (grid frame, at
+// the grid entry), u, v, w, E; spot index -1 = the history never enters the grid
+int opmc_test_sample_primaries(opmc_ctx *c, const opmc_spot *spots, int nspots, uint64_t n, uint64_t seed, double *out) {
+  if (!c || !spots || nspots < 1 || c->hu.empty()) return -1;
+  std::vector<double> cdf = spot_cdf(spots, nspots);
+  for (uint64_t h = 0; h < n; ++h) {
+    Rng g(seed, h, 0); Particle p; Ledger led; double e0 = 0;
+    const bool ok = sample_primary(c, spots, cdf, g, p, led, e0);
+    double *o = out + 8 * h;
+    o[0] = ok ? p.spot : -1; o[1] = p.r.x; o[2] = p.r.y; o[3] = p.r.z; o[4] = p.d.x; o[5] = p.d.y; o[6] = p.d.z; o[7] = ok ? p.E : e0;
+  }
+  return 0;
+}
+// events of the last opmc_simulate per class and target element: out[0..7] elastic, out[8..15] non-elastic
+int opmc_test_event_counts(opmc_ctx *c, uint64_t *out) {
+  if (!c || !out) return -1;
+  for (int i = 0; i < OPMC_MAX_ELEM; ++i) { out[i] = c->ev_el[i]; out[OPMC_MAX_ELEM + i] = c->ev_ne[i]; }
   return 0;
 }
 double opmc_test_cugnon(int which, double p) {

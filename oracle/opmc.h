@@ -12,7 +12,11 @@
  * Parity pins (tests/test_oracle_*.py): Philox known answers; CSDA range vs direct
  * integration; Eq.1/Eq.2 identity; Highland 1.07*theta0; Fermi-Eyges hinge moments;
  * straggling cumulants; per-history energy ledger; exact Z/A conservation; Ranft
- * t-distribution; INC collision-probability closed form; evaporation spectra.
+ * t-distribution; INC collision-probability closed form; evaporation spectra; Cugnon joint
+ * and interior values; NN angular law vs its analytic CDF (alone and inside the cascade);
+ * shell-boundary refraction/reflection vs the classical scattering angle; Pauli blocking and
+ * the trapping rule; event rate 1 - exp(-Sigma L) and n_i sigma_i branching; spot
+ * frequencies and divergence; cascade step-guard trip rate (tests/test_oracle_pins_nuclear.py).
  * Parity UNPINNED (comparison material missing from the container): agreement with
  * Chibani's Vavilov sampler (ref [18]), with the INC of ref [13], with Furihata's GEM
  * (ref [21]) and with any Geant4-derived table.
@@ -72,6 +76,9 @@ typedef struct {
   double max_ledger_residual;    /* max over histories of |E0 - sum of all sinks| (MeV) */
   double max_event_residual;     /* max |4-momentum imbalance| over INC/evaporation/elastic events */
   uint64_t n_zab_violations;     /* events where charge or baryon number failed to balance (must be 0) */
+  /* Reading R6.8 bookkeeping: cascade attempts ended by the step guard / by the 200-nucleon stack limit, and the
+     deepest stack of waiting nucleons and the largest number of outgoing nucleons seen in one attempt */
+  uint64_t n_inc_guard_trips, n_inc_stack_trips, inc_max_stack, inc_max_out;
 } opmc_counters;
 
 typedef struct opmc_ctx opmc_ctx;
@@ -82,7 +89,8 @@ int  opmc_load_physics_tables(opmc_ctx *, const opmc_tables *);
 int  opmc_set_hu_materials(opmc_ctx *, const opmc_hu_bin *bins, int nbins);
 int  opmc_load_ct(opmc_ctx *, const int16_t *hu, int nx, int ny, int nz,
                   double dx, double dy, double dz, const double origin[3]);
-/* keys: "straggling" "mcs" "elastic" "nonelastic" (0/1), "s_max_wet_cm", "n_batches", "threads" */
+/* keys: "straggling" "mcs" "elastic" "nonelastic" (0/1), "s_max_wet_cm", "n_batches", "threads", "score_letd", "mcs_model",
+ * "inc_step_guard" (tracking steps per cascade attempt, Reading R6.8; default 1024 - changed only by the pin test of the guard) */
 int  opmc_set_option(opmc_ctx *, const char *key, double value);
 int  opmc_simulate(opmc_ctx *, const opmc_spot *spots, int nspots, uint64_t n_histories, uint64_t seed,
                    double *dose, double *sigma);
@@ -123,6 +131,17 @@ double opmc_test_fermi_p2(opmc_ctx *, int Z, int A, uint64_t n, uint64_t seed);
 int    opmc_test_evap_first(opmc_ctx *, int Z, int A, double estar, uint32_t channel_mask, uint64_t n,
                             uint64_t seed, double *widths, int32_t *out_channel, double *out_eps,
                             double *out_cos);
+/* n samples of cos(theta_cm) of the NN elastic angular law (PAPER.md:L77 ref [20]; Reading R6.6) */
+int    opmc_test_nn_cos(int same_type, double p_lab_gev, double pcm_mev, uint64_t n, uint64_t seed, double *out);
+/* cascade attempts on a hand-made shell nucleus (see opmc.cpp): closed-form pins of refraction/reflection, Pauli
+   blocking and of the NN angular law as the cascade uses it */
+int    opmc_test_inc_custom(int nshell, const double *rout, const double *rho, const double *pF, const double *V,
+                            double coulomb, int pauli, double const_sigma_mb, double t_in, uint64_t n, uint64_t seed,
+                            int32_t *out_n, double *out_rec);
+/* n primaries of a plan from the beam-spot sampler: out[n][8] = spot, x, y, z, u, v, w, E */
+int    opmc_test_sample_primaries(opmc_ctx *, const opmc_spot *spots, int nspots, uint64_t n, uint64_t seed, double *out);
+/* events of the last opmc_simulate per class and element: out[16] = elastic[8], non-elastic[8] */
+int    opmc_test_event_counts(opmc_ctx *, uint64_t *out);
 double opmc_test_cugnon(int which /*0 sigma_pp,1 sigma_np,2 B_pp,3 B_np,4 a_np*/, double p_gev);
 #ifdef __cplusplus
 }
