@@ -152,6 +152,7 @@ int sync_tables(pmc_ctx *c) {
   const double dlne = (std::log(c->e_max) - std::log(c->e_min)) / (c->n_e - 1);
   T.ln_emin = (float)std::log(c->e_min); T.ln_emax = (float)std::log(c->e_max); T.inv_dlne = (float)(1.0 / dlne);
   T.e_min = (float)c->e_min; T.e_max = (float)c->e_max;
+  T.c_l2 = (float)(std::log(2.0) / dlne); T.c_e0 = (float)(std::log(c->e_min) / dlne);
   T.e_cut = (float)c->e_cut; T.highland = (float)c->highland; T.kappa_g = (float)c->kappa_g; T.s_max = (float)c->s_max;
   T.opt_strag = c->opt_strag; T.opt_mcs = c->opt_mcs; T.opt_el = c->opt_el; T.opt_ne = c->opt_ne;
   CK(c->d_mol.upload(c->h_mol, s)); T.mol_c = c->d_mol.p; T.mol_n = c->mol_n; T.mol_dth = (float)c->mol_dth; T.mcs_model = c->mol_n > 1 ? c->mcs_model : 0;
@@ -176,7 +177,10 @@ int sync_tables(pmc_ctx *c) {
     for (int b = 0; b < nb; ++b) {
       const pmc_hu_bin &h = c->mats[b].b; MatBin &m = bins[b];
       m.hu_lo = (float)h.hu_lo; m.dhu = (float)((double)h.hu_hi - h.hu_lo); m.inv_dhu = (float)(1.0 / ((double)h.hu_hi - h.hu_lo));
-      m.rho_lo = (float)h.rho_lo; m.drho = (float)(h.rho_hi - h.rho_lo);
+      m.rho_lo = (float)h.rho_lo; m.drho = (float)(h.rho_hi - h.rho_lo); m.slope = (float)((h.rho_hi - h.rho_lo) / ((double)h.hu_hi - h.hu_lo));
+      m.lnr_lo = T.lnr_lo[h.table_id]; m.lnr_hi = T.lnr_hi[h.table_id]; m.inv_hr = T.inv_hr[h.table_id];
+      m.off_e = 2 * h.table_id * c->n_e; m.off_r = 2 * (c->n_sr * c->n_e + h.table_id * c->n_r);
+      m.off_sig = 2 * c->n_sr * (c->n_e + c->n_r) + b * c->n_e;
       m.wet = h.table_id == 0 ? (float)h.f_m : 1.0f; m.inv_x0 = (float)(1.0 / h.x0_gcm2); m.zoa = (float)c->mats[b].zoa; m.table = h.table_id;
       for (int i = 0; i < MAX_ELEM; ++i) m.nfac[i] = i < c->n_elem ? (float)(NAVO * h.w[i] / c->ea[i] * 1e-27) : 0.f;
       double zs = 0; for (int i = 0; i < c->n_elem; ++i) zs += h.w[i] * c->ez[i] * (c->ez[i] + 1.0) / c->ea[i];
@@ -203,10 +207,10 @@ int sync_tables(pmc_ctx *c) {
     c->smem_transport = ((size_t)2 * c->n_sr * c->n_e + (size_t)2 * c->n_sr * c->n_r + (size_t)nb * c->n_e) * 4 + (size_t)nb * sizeof(MatBin) +
                         lut.size() + 16;
     if (c->smem_transport > 200 * 1024) return fail(c, PMC_E_UNSUPPORTED, "tables too large for shared-memory staging");
-    CK(cudaFuncSetAttribute(transport_kernel<0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_transport));
-    CK(cudaFuncSetAttribute(transport_kernel<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_transport));
-    CK(cudaFuncSetAttribute(transport_kernel<0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_transport));
-    CK(cudaFuncSetAttribute(transport_kernel<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_transport));
+#define PMC_SMEM_ATTR(M, D, X) CK(cudaFuncSetAttribute(transport_kernel<M, D, X>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_transport))
+    PMC_SMEM_ATTR(0, false, false); PMC_SMEM_ATTR(0, false, true); PMC_SMEM_ATTR(1, false, false); PMC_SMEM_ATTR(1, false, true);
+    PMC_SMEM_ATTR(0, true, false); PMC_SMEM_ATTR(1, true, false);
+#undef PMC_SMEM_ATTR
   }
   CK(cudaStreamSynchronize(s));
   c->tables_dirty = false;
@@ -293,9 +297,11 @@ int run_generations(pmc_ctx *c, RunParams P, uint32_t n0, bool profile) {
     CK(cudaMemsetAsync(c->qev.q.count, 0, 4, s));
     { Timer t(c, &c->timing.transport_ms, profile);
       const bool mol = c->T.mcs_model == 1, dbg = P.dbg_out != nullptr;
-#define PMC_LAUNCH_TRANSPORT(M, D) transport_kernel<M, D><<<grid_t, TRANSPORT_THREADS, c->smem_transport, s>>>(c->T, c->G, P, cur->q, n_in, c->d_head.p, c->qev.q, c->d_tally.p, c->d_cnt.p)
-      if (mol && dbg) PMC_LAUNCH_TRANSPORT(1, true); else if (mol) PMC_LAUNCH_TRANSPORT(1, false);
-      else if (dbg) PMC_LAUNCH_TRANSPORT(0, true); else PMC_LAUNCH_TRANSPORT(0, false);
+      const bool extra = !dbg && (P.let_num != nullptr || P.roi_map != nullptr || P.aggregate != 0);
+#define PMC_LAUNCH_TRANSPORT(M, D, X) transport_kernel<M, D, X><<<grid_t, TRANSPORT_THREADS, c->smem_transport, s>>>(c->T, c->G, P, cur->q, n_in, c->d_head.p, c->qev.q, c->d_tally.p, c->d_cnt.p)
+      if (dbg) { if (mol) PMC_LAUNCH_TRANSPORT(1, true, false); else PMC_LAUNCH_TRANSPORT(0, true, false); }
+      else if (mol) { if (extra) PMC_LAUNCH_TRANSPORT(1, false, true); else PMC_LAUNCH_TRANSPORT(1, false, false); }
+      else { if (extra) PMC_LAUNCH_TRANSPORT(0, false, true); else PMC_LAUNCH_TRANSPORT(0, false, false); }
 #undef PMC_LAUNCH_TRANSPORT
     }
     c->timing.launches_total++; c->timing.launches_transport++;
@@ -537,7 +543,10 @@ static int simulate_impl(pmc_ctx *c, const pmc_spot *spots_in, int nspots, uint6
   const int grid_v = c->n_sm * 8;
   for (uint64_t cs = 0; cs < n; cs += chunk) {
     const uint32_t nc = (uint32_t)std::min<uint64_t>(chunk, n - cs);
-    RunParams P{}; P.seed = seed; P.hist0 = c->history_offset + cs; P.n = nc; P.max_steps = max_steps; P.dbg_out = dbg_out ? dbg_out + 8ull * cs : nullptr;
+    RunParams P{}; P.seed = seed; P.hist0 = c->history_offset + cs;
+    for (int r = 0; r < 10; ++r) {                                   // Philox key schedule (Weyl sequence)
+      P.rk.k[2 * r] = (uint32_t)seed + (uint32_t)r * 0x9E3779B9u; P.rk.k[2 * r + 1] = (uint32_t)(seed >> 32) + (uint32_t)r * 0xBB67AE85u;
+    } P.n = nc; P.max_steps = max_steps; P.dbg_out = dbg_out ? dbg_out + 8ull * cs : nullptr;
     P.aggregate = c->aggregate; P.local0 = cs; P.n_total = n; P.B = (uint32_t)B; P.nvox = nvox;
     P.roi_map = roi_on ? c->d_roimap.p : nullptr; P.dij = roi_on ? c->dij_dev : nullptr; P.n_roi = roi_on ? c->n_roi : 0u;
     P.let_num = let_on ? c->d_let.p : nullptr; P.let_den = let_on ? c->d_let.p + nvox_s : nullptr;

@@ -29,6 +29,24 @@ __device__ __forceinline__ uint4 philox4x32_10(uint4 c, uint2 k) {
   return c;
 }
 
+// The same block function with the key schedule (k + r * Weyl constants, r = 0..9) computed once on the host and passed
+// as a kernel parameter: the round keys then sit in the constant bank / uniform registers and a block is exactly
+// 20 IMAD.WIDE + 20 LOP3 (the schedule arithmetic above costs 18 more instructions per block in the step kernel).
+struct RoundKeys { uint32_t k[20]; };
+__device__ __forceinline__ uint4 philox4x32_10(uint4 c, const RoundKeys &K) {
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    const uint32_t h0 = __umulhi(0xD2511F53u, c.x), l0 = 0xD2511F53u * c.x, h1 = __umulhi(0xCD9E8D57u, c.z), l1 = 0xCD9E8D57u * c.z;
+    c = make_uint4(h1 ^ c.y ^ K.k[2 * r], l1, h0 ^ c.w ^ K.k[2 * r + 1], l0);
+  }
+  return c;
+}
+// stream of one particle inside the step kernel (same counters and keys as Rng, hence the same blocks)
+struct RngK {
+  const RoundKeys &K; uint32_t h0, h1, pid, blk;
+  __device__ __forceinline__ uint4 next4() { return philox4x32_10(make_uint4(h0, h1, pid, blk++), K); }
+};
+
 // Per-particle stream: key = seed, counter = (history_lo, history_hi, particle id, block number).  Draws are
 // handed out a block (4 words) at a time, so the only state that travels with a particle is `blk`.
 struct Rng {
@@ -45,6 +63,10 @@ struct Rng {
   }
 };
 __device__ __forceinline__ float u01(uint32_t x) { return ((float)(x >> 8) + 0.5f) * (1.0f / 16777216.0f); }   // (0,1)
+// the hot loop's uniforms: top 23 bits of a word placed in the mantissa of [1,2) (two instructions, no int-to-float
+// conversion): (k + 1/2) 2^-23, k = 0 .. 2^23 - 1; and a 16-bit field: (k + 1/2) 2^-16
+__device__ __forceinline__ float u23(uint32_t x) { return __uint_as_float((x >> 9) | 0x3f800000u) - (1.0f - 1.0f / 16777216.0f); }
+__device__ __forceinline__ float u16f(uint32_t k16) { return fmaf((float)k16, 1.0f / 65536.0f, 0.5f / 65536.0f); }
 
 // Fast fp32 arithmetic of the hot loops (the paper's -use_fast_math build was dosimetrically equivalent, PAPER.md:L203,
 // L248): 2-ulp division, and series for log1p / expm1 / sincos of the small arguments that occur at almost every step
@@ -53,27 +75,39 @@ __device__ __forceinline__ float fdiv(float a, float b) {      // MUFU.RCP + FMU
   float q; asm("div.approx.ftz.f32 %0, %1, %2;" : "=f"(q) : "f"(a), "f"(b)); return q;
 }
 __device__ __forceinline__ float fsqrt(float a) { float q; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(q) : "f"(a)); return q; }
+// single MUFU instructions (the __logf / __expf / rsqrtf forms carry a denormal guard of three more instructions each)
+__device__ __forceinline__ float frcp(float a) { float q; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(q) : "f"(a)); return q; }
+__device__ __forceinline__ float frsq(float a) { float q; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(q) : "f"(a)); return q; }
+__device__ __forceinline__ float flg2(float a) { float q; asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(q) : "f"(a)); return q; }
+__device__ __forceinline__ float fex2(float a) { float q; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(q) : "f"(a)); return q; }
+constexpr float LN2 = 0.69314718056f, LOG2E = 1.44269504089f;
+__device__ __forceinline__ float flog(float a) { return flg2(a) * LN2; }
+__device__ __forceinline__ float fexp(float a) { return fex2(a * LOG2E); }
 // sin and cos of 2 pi u, u in (0,1): MUFU.SIN/COS (absolute error ~5e-7), for azimuths and Box-Muller
 __device__ __forceinline__ void sincos_2pi(float u, float *s, float *c) { const float x = TWO_PI * u - 3.14159265358979f; *s = -__sinf(x); *c = -__cosf(x); }
 __device__ __forceinline__ float log1p_small(float x) {          // ln(1 + x)
   if (fabsf(x) < 0.06f) return x * (1.0f + x * (-0.5f + x * ((1.0f / 3.0f) + x * (-0.25f + x * (0.2f - x * (1.0f / 6.0f))))));
-  return __logf(1.0f + x);                                      // |x| >= 0.06: relative error < 3e-6
+  return flog(1.0f + x);                                        // |x| >= 0.06: relative error < 3e-6
 }
 __device__ __forceinline__ float expm1_small(float x) {          // e^x - 1
   if (fabsf(x) < 0.06f) return x * (1.0f + x * (0.5f + x * ((1.0f / 6.0f) + x * ((1.0f / 24.0f) + x * (1.0f / 120.0f)))));
-  return __expf(x) - 1.0f;
+  return fexp(x) - 1.0f;
 }
 __device__ __forceinline__ void sincos_small(float x, float *s, float *c) {
   if (fabsf(x) < 0.25f) {
     const float x2 = x * x;
     *s = x * (1.0f + x2 * ((-1.0f / 6.0f) + x2 * ((1.0f / 120.0f) - x2 * (1.0f / 5040.0f))));
     *c = 1.0f + x2 * (-0.5f + x2 * ((1.0f / 24.0f) + x2 * ((-1.0f / 720.0f) + x2 * (1.0f / 40320.0f))));
-  } else sincosf(x, s, c);
+  } else { *s = __sinf(x); *c = __cosf(x); }      // |x| <= pi: absolute error 5e-7
 }
 
 // ------------------------------------------------------------------ device tables
-struct MatBin {                 // one HU bin, 16 floats
+struct MatBin {                 // one HU bin, 25 words
   float hu_lo, inv_dhu, dhu, rho_lo, drho;
+  float slope;                  // drho / dhu
+  // the bin's range table, resolved once on the host: abscissa of the inverse table, and the offsets (in floats from the
+  // start of the step kernel's shared memory) of its ln R(ln E) knots, its ln E(ln R) knots and its Sigma/rho row
+  float lnr_lo, lnr_hi, inv_hr; int off_e, off_r, off_sig;
   float wet;                    // f_m of Eq.1/Eq.2 (L55-63) for table 0, 1 for own tables
   float inv_x0, zoa;
   int table;
@@ -94,6 +128,7 @@ struct Tables {
   float ln_emin, ln_emax, inv_dlne, e_min, e_max;
   float e_cut, highland, kappa_g, s_max;
   float lnr_lo[4], lnr_hi[4], inv_hr[4];
+  float c_l2, c_e0;             // (ln E - ln_emin) inv_dlne = c_l2 log2(E) - c_e0
   int hu_lut_lo, hu_lut_n;
   int opt_strag, opt_mcs, opt_el, opt_ne;
   int mcs_model, mol_n; float mol_dth; const float *mol_c;   // Moliere: C0, C1, C2 back to back, [3][mol_n]
@@ -124,6 +159,11 @@ __device__ __forceinline__ EIdx e_index(const Tables &T, float lnE) {
 __device__ __forceinline__ float spline_eval(const float *y, const float *y2, int i, float b) {
   const float a = 1.0f - b;
   return a * y[i] + b * y[i + 1] + ((a * a * a - a) * y2[i] + (b * b * b - b) * y2[i + 1]);
+}
+// the same on knots interleaved with their (pre-scaled) second derivatives: {y_i, y''_i}
+__device__ __forceinline__ float spline_eval2(const float2 *t, int i, float b) {
+  const float a = 1.0f - b; const float2 p = t[i], q = t[i + 1];
+  return fmaf(a, p.x, b * q.x) + fmaf(fmaf(a * a, a, -a), p.y, fmaf(b * b, b, -b) * q.y);
 }
 __device__ __forceinline__ float ln_range(const Tables &T, const float *lnR, const float *lnR2, int tab, EIdx k) {
   return spline_eval(lnR + tab * T.n_e, lnR2 + tab * T.n_e, k.i, k.b);
@@ -223,67 +263,71 @@ __device__ __forceinline__ void flush(unsigned long long *dst, unsigned long lon
 // ------------------------------------------------------------------ straggling (Reading R4)
 // Vavilov(kappa, beta^2) as its defining compound-Poisson process, shifted to the CSDA mean loss.  The collision
 // spectrum xi/T^2 (1 - beta^2 T/Tmax) is split at T_c: collisions above T_c are sampled one by one (Poisson number by
-// inversion, thinning for the (1 - beta^2 T/Tmax) factor; one random word per collision).  Below T_c: the part under the oracle's own cut T_c0 is
+// inversion, thinning for the (1 - beta^2 T/Tmax) factor).  Below T_c: the part under the oracle's own cut T_c0 is
 // Gaussian (Reading R4); the collisions in [T_c0, T_c] add skewness, and the sum of both is drawn as a shifted gamma
 // variate with the exact variance and third cumulant (its fourth cumulant, 3 k3^2 / 2 k2, is within 12 % of the
 // exact xi T_c^3 / 3), through the Wilson-Hilferty cube of one normal deviate - monotone, and the plain Gaussian in
 // the limit T_c -> T_c0.  T_c is chosen so that about MU_HARD hard collisions are expected, which keeps the lanes of
 // a warp in step (MU_HARD = 1/2: the shape parameter of the gamma is then >= 8, its skewness <= 0.71).  kappa >= kappa_G: Gaussian, variance
 // xi Tmax (1 - beta^2/2).
+//
+// Random bits.  One Philox block q of the caller's stream plus `spare`, 32 bits the caller has left over from its own
+// block, serve the normal deviate (23 + 16 bits), the Poisson inversion (23 bits) and the first three hard-collision
+// candidates (16 bits place a candidate on the 1/T^2 spectrum between T_c and Tmax - T_c is a sizeable fraction of Tmax,
+// so 2^-16 steps of 1/T are fine - and 10 bits decide its thinning).  Only a fourth candidate (0.2 % of the steps)
+// needs another block: the lanes of a warp stay together.
 constexpr float MU_HARD = 0.5f;
-__device__ __forceinline__ float gauss_pair(uint32_t a, uint32_t b) {
-  return fsqrt(-2.0f * __logf(u01(a))) * -__cosf(TWO_PI * u01(b) - 3.14159265358979f);
+__device__ __forceinline__ float hard_candidate(uint32_t pos16, uint32_t thin10, float itc, float ditc, float b2itmax) {
+  const float ua = fmaf((float)thin10, 1.0f / 1024.0f, 0.5f / 1024.0f);
+  const float t = frcp(fmaf(-u16f(pos16), ditc, itc));
+  return ua < fmaf(-b2itmax, t, 1.0f) ? t : 0.f;
 }
-// `spare`: 32 random bits the caller has left over (u01() uses only the top 24 bits of a word, so the low bytes of
-// the four words of the caller's own draw block make one more word); they serve the second hard collision, so that
-// a further Philox block is needed only from the third on (1.4 % of the steps).
-__device__ __forceinline__ uint32_t low_bytes(uint4 r) {
-  return (r.x & 0xFFu) | ((r.y & 0xFFu) << 8) | ((r.z & 0xFFu) << 16) | ((r.w & 0xFFu) << 24);
-}
-__device__ float straggle(const Tables &T, Rng &g, float e_start, float mean_loss, float rhoL, float zoa, uint32_t spare) {
+template <class Gen>
+__device__ __forceinline__ float straggle(const Tables &T, Gen &g, float e_start, float mean_loss, float rhoL, float zoa, uint32_t spare) {
   if (rhoL <= 0.f || mean_loss <= 0.f) return mean_loss;
-  const float gam = 1.0f + e_start * (1.0f / MP), g2m = gam * gam, b2 = 1.0f - fdiv(1.0f, g2m), bg2 = g2m - 1.0f;
-  const float tmax = fdiv(2.0f * ME * bg2, 1.0f + 2.0f * gam * (ME / MP) + (ME / MP) * (ME / MP));
-  const float xi = fdiv(0.5f * KBETHE * zoa * rhoL, b2);
+  // beta^2 gamma^2 = g2m - 1; 1/beta^2 = 1 + 1/(beta^2 gamma^2)
+  const float gam = fmaf(e_start, 1.0f / MP, 1.0f), bg2 = fmaf(gam, gam, -1.0f), q = frcp(bg2), ib2 = 1.0f + q, b2 = frcp(ib2);
+  const float den = fmaf(gam, 2.0f * (ME / MP), 1.0f + (ME / MP) * (ME / MP));
+  const float tmax = (2.0f * ME) * bg2 * frcp(den), itmax = den * q * (0.5f / ME);
+  const float xi = (0.5f * KBETHE) * zoa * rhoL * ib2;
+  const uint4 r = g.next4();
+  const float z = fsqrt(-2.0f * LN2 * flg2(u23(r.x))) * __cosf(TWO_PI * u16f(r.y >> 16));
   float loss;
-  uint4 r = g.next4();
-  const float z = gauss_pair(r.x, r.y);
   if (xi >= T.kappa_g * tmax) {
-    loss = mean_loss + fsqrt(xi * tmax * (1.0f - 0.5f * b2)) * z;
+    loss = fmaf(fsqrt(xi * tmax * fmaf(-0.5f, b2, 1.0f)), z, mean_loss);
   } else {
-    const float itmax = fdiv(1.0f, tmax);
-    const float tc0 = fminf(1e-3f, 0.01f * tmax);                            // Reading R4: Gaussian below tc0
-    // kappa > 1 (the last centimetre of the range): twice as many hard collisions, the soft gamma is less skewed
-    float tc = fmaxf(tc0, fdiv(1.0f, fdiv(xi > tmax ? 2.0f * MU_HARD : MU_HARD, xi) + itmax));
-    tc = fminf(tc, tmax);
-    const float itc = fdiv(1.0f, tc), ltc = __logf(tmax * itc);
-    const float mu_c = xi * (itc - itmax);                                   // candidates (before thinning)
-    const float mean_hard = xi * (ltc - b2 * (1.0f - tc * itmax));
-    // Poisson(mu_c) number of candidates by inversion with one uniform, each candidate handled as soon as the
-    // inversion shows it exists.  One 32-bit word per candidate: 20 bits place it on the 1/T^2 spectrum, the other
-    // 12 decide the thinning; candidate 0 uses the last word of r, candidate 1 the caller's spare bits, the next four
-    // one more block, ...
-    float pk = __expf(-mu_c), cdf = pk; const float up = u01(r.z);
-    float hard = 0.f;
-    uint4 q = make_uint4(r.w, spare, 0u, 0u);
-    int k = 0, avail = 2;
-    while (up > cdf && k < 64) {
-      if (avail == 0) { q = g.next4(); avail = 4; }
-      const uint32_t w = q.x; q.x = q.y; q.y = q.z; q.z = q.w; --avail;
-      const float ut = ((float)(w >> 12) + 0.5f) * (1.0f / 1048576.0f), ua = ((float)(w & 0xFFFu) + 0.5f) * (1.0f / 4096.0f);
-      const float t = fdiv(1.0f, itc - ut * (itc - itmax));
-      if (ua < 1.0f - b2 * t * itmax) hard += t;
-      ++k; pk *= fdiv(mu_c, (float)k); cdf += pk;
+    // T_c = 1 / (mu / xi + 1/Tmax) with mu hard collisions expected (twice as many when kappa > 1, the last centimetre of
+    // the range, where the soft gamma would otherwise be too skewed), not below the oracle's cut T_c0 = min(1 keV, Tmax/100)
+    const float itc0 = fmaxf(1e3f, 100.0f * itmax);
+    const float itc = fminf(fmaf(xi > tmax ? 2.0f * MU_HARD : MU_HARD, frcp(xi), itmax), itc0), tc = frcp(itc), tc0 = frcp(itc0);
+    const float ditc = itc - itmax, b2itmax = b2 * itmax;
+    const float mu_c = xi * ditc;                                            // candidates (before thinning)
+    const float mean_hard = xi * (LN2 * flg2(tmax * itc) - b2 * fmaf(-tc, itmax, 1.0f));
+    // Poisson(mu_c) number of candidates by inversion with one uniform
+    const float up = u23(r.z), p0 = fex2(-LOG2E * mu_c), p1 = p0 * mu_c, c1 = p0 + p1, p2 = 0.5f * p1 * mu_c, c2 = c1 + p2;
+    const float h0 = hard_candidate(r.y & 0xFFFFu, spare & 0x3FFu, itc, ditc, b2itmax);
+    const float h1 = hard_candidate(r.w >> 16, (spare >> 10) & 0x3FFu, itc, ditc, b2itmax);
+    float hard = (up > p0 ? h0 : 0.f) + (up > c1 ? h1 : 0.f);
+    if (up > c2) {                                                           // three or more: 1.4 % of the steps
+      hard += hard_candidate(r.w & 0xFFFFu, (spare >> 20) & 0x3FFu, itc, ditc, b2itmax);
+      float pk = p2 * mu_c * (1.0f / 3.0f), cdf = c2 + pk;
+      int k = 3, avail = 0; uint4 w = make_uint4(0u, 0u, 0u, 0u);
+      while (up > cdf && k < 64) {                                           // four or more: one more block per four
+        if (avail == 0) { w = g.next4(); avail = 4; }
+        const uint32_t v = w.x; w.x = w.y; w.y = w.z; w.z = w.w; --avail;
+        hard += hard_candidate(v >> 16, v & 0x3FFu, itc, ditc, b2itmax);
+        ++k; pk *= mu_c * frcp((float)k); cdf += pk;
+      }
     }
     // soft part: k2 = xi tc (1 - b2 tc/2Tmax) of everything below tc; k3 = xi [t^2 (1/2 - b2 t/3Tmax)] from tc0 to tc
-    const float x = b2 * tc * itmax, x0 = b2 * tc0 * itmax;
-    const float k2 = xi * tc * (1.0f - 0.5f * x), sd = fsqrt(k2);
-    const float k3 = xi * (tc * tc * (0.5f - x * (1.0f / 3.0f)) - tc0 * tc0 * (0.5f - x0 * (1.0f / 3.0f)));
+    const float x = b2itmax * tc, x0 = b2itmax * tc0;
+    const float k2 = xi * tc * fmaf(-0.5f, x, 1.0f), sd = fsqrt(k2);
+    const float k3 = xi * (tc * tc * fmaf(-1.0f / 3.0f, x, 0.5f) - tc0 * tc0 * fmaf(-1.0f / 3.0f, x0, 0.5f));
     float soft = sd * z;
-    if (tc > tc0 && k3 > 0.f) {
-      const float sa = fdiv(2.0f * k2 * sd, k3), isa = fdiv(1.0f, sa), c9 = isa * isa * (1.0f / 9.0f);   // sa = sqrt(shape)
-      const float e = fmaxf(z * isa * (1.0f / 3.0f) - c9, -1.0f);
-      soft = sd * sa * (e * (3.0f + e * (3.0f + e)) + c9 * c9 * c9);          // sqrt(k2 a) [(1 + e)^3 - E(1 + e)^3]
+    if (itc < itc0 && k3 > 0.f) {
+      const float A = 2.0f * k2 * sd, isa = k3 * frcp(A), sa = A * frcp(k3), c9 = isa * isa * (1.0f / 9.0f);   // sa = sqrt(shape)
+      const float e = fmaxf(fmaf(z * isa, 1.0f / 3.0f, -c9), -1.0f);
+      soft = sd * sa * fmaf(e, fmaf(e, 3.0f + e, 3.0f), c9 * c9 * c9);       // sqrt(k2 a) [(1 + e)^3 - E(1 + e)^3]
     }
     loss = mean_loss + (hard - mean_hard) + soft;
   }

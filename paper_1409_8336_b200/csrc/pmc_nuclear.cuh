@@ -510,7 +510,8 @@ __global__ void straggle_kernel(Tables T, float e, float mean, float rhoL, float
   const uint64_t i = blockIdx.x * (uint64_t)blockDim.x + threadIdx.x;
   if (i >= n) return;
   Rng g; g.init(seed, i, 0u, 0u);
-  out[i] = straggle(T, g, e, mean, rhoL, zoa, low_bytes(g.next4()));
+  const uint32_t spare = g.next4().x;
+  out[i] = straggle(T, g, e, mean, rhoL, zoa, spare);
 }
 
 }  // namespace pmc

@@ -12,6 +12,7 @@ struct SpotDev {                 // pmc_spot, prepared on the host (axis normali
 
 struct RunParams {
   uint64_t seed; uint64_t hist0;      // first history id of this launch
+  RoundKeys rk;                       // Philox key schedule of `seed` (host-computed)
   uint32_t n;                         // histories in this launch
   // All B batches ("10 groups") are in flight at once, each scoring into its own tally grid:
   // history h (0-based within the call) belongs to batch floor(h B / n_total); tally of batch b starts at b * nvox.
@@ -59,20 +60,6 @@ __device__ __forceinline__ int hu_to_bin(const Tables &T, const uint8_t *lut, in
 __device__ __forceinline__ float bin_density(const MatBin &m, int hu) {
   const float t = fminf(fmaxf((float)hu - m.hu_lo, 0.f), m.dhu);
   return m.rho_lo + m.drho * (t * m.inv_dhu);
-}
-
-// distance along d to the first face of the voxel (voxel-local r in [0, size]); ties: x before y before z
-__device__ __forceinline__ float dist_to_face(const V3 &r, const V3 &d, const float *sz, int &axis, int &sgn) {
-  float best = BIG; axis = -1; sgn = 0;
-  const float rr[3] = {r.x, r.y, r.z}, dd[3] = {d.x, d.y, d.z};
-#pragma unroll
-  for (int a = 0; a < 3; ++a) {
-    if (dd[a] != 0.f) {
-      const float t = fmaxf(fdiv((dd[a] > 0.f ? sz[a] : 0.f) - rr[a], dd[a]), 0.f);
-      if (t < best) { best = t; axis = a; sgn = dd[a] > 0.f ? 1 : -1; }
-    }
-  }
-  return best;
 }
 
 // Highland theta0 with the paper's factor; t = mass thickness / X0
@@ -217,7 +204,7 @@ __global__ void __launch_bounds__(256) sampler_kernel(Tables T, Grid G, const Sp
         const float ef = (float)E, lnEv = logf(fminf(fmaxf(ef, T.e_min), T.e_max));
         const float lnRv = ln_range(T, T.lnR, T.lnR2, air_table, e_index(T, lnEv)), Rg = expf(lnRv);
         float loss = mean_loss(T, T.lnE, T.lnE2, air_table, ef, lnEv, lnRv, Rg, (float)L * air_wf);
-        if (T.opt_strag) loss = straggle(T, g, ef, loss, (float)L * air_rho, air_zoa, low_bytes(q));
+        if (T.opt_strag) loss = straggle(T, g, ef, loss, (float)L * air_rho, air_zoa, q.w);   // q.w: not used by the air step itself
         e_air += loss; E -= loss;
         if (E <= T.e_cut) { e_air += E; ok = false; }
       }
@@ -299,36 +286,56 @@ __device__ __forceinline__ void deposit(float *tally, uint32_t tvox, float e, bo
 // Particles that reach an event are appended to the elastic or non-elastic queue; nothing else is written back.
 constexpr int TRANSPORT_THREADS = 256, TRANSPORT_BLOCKS_PER_SM = 4;
 
+// distance along one axis to the face the particle is heading for (voxel-local r in [0, size], inv = 1/d); BIG if d = 0
+__device__ __forceinline__ float axis_dist(float r, float d, float size) {
+  const float t = fmaxf(((d > 0.f ? size : 0.f) - r) * frcp(d), 0.f);
+  return d != 0.f ? t : BIG;
+}
+// new direction after a polar deflection (st, ct) with azimuth (sp, cp) about the unit vector d, renormalised
+__device__ __forceinline__ V3 rotate(V3 d, float st, float ct, float sp, float cp) {
+  const float s2 = fmaf(d.x, d.x, d.y * d.y);
+  V3 n;
+  if (s2 < 1e-14f) { const float sg = d.z >= 0.f ? 1.0f : -1.0f; n = {st * cp, sg * st * sp, sg * ct}; }
+  else {
+    const float is = frsq(s2), A = st * cp * is, B = st * sp * is, Az = A * d.z;
+    n = {fmaf(Az, d.x, fmaf(-B, d.y, ct * d.x)), fmaf(Az, d.y, fmaf(B, d.x, ct * d.y)), fmaf(-A, s2, ct * d.z)};
+  }
+  const float in = frsq(fmaf(n.x, n.x, fmaf(n.y, n.y, n.z * n.z)));
+  return {n.x * in, n.y * in, n.z * in};
+}
+
 // MCS_MODEL: 0 = Highland (the paper's choice), 1 = full Moliere; a template so that the default kernel carries none of
 // the Moliere code or its registers
 // DBG: the pmc_first_steps variant (stop after max_steps, write the state of every primary); the production kernel
 // carries neither its registers nor its branches.
-template <int MCS_MODEL, bool DBG>
+// EXTRA: LET_d scoring, per-spot dose influence or warp-merged dose atomics are on (the plain kernel carries none of it)
+template <int MCS_MODEL, bool DBG, bool EXTRA>
 __global__ void __launch_bounds__(TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM) transport_kernel(Tables T, Grid G, RunParams P, Queue in, uint32_t n_in,
                                                            uint32_t *head, Queue q_ev, float *tally, Counters *cnt) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  // shared-memory staging of the stopping-power/range and cross-section tables (PAPER.md:L144 used textures)
-  float *s_lnR = reinterpret_cast<float *>(smem_raw);
-  float *s_lnR2 = s_lnR + T.n_sr * T.n_e;
-  float *s_lnE = s_lnR2 + T.n_sr * T.n_e;
-  float *s_lnE2 = s_lnE + T.n_sr * T.n_r;
-  float *s_sig = s_lnE2 + T.n_sr * T.n_r;
+  // shared-memory staging of the stopping-power/range and cross-section tables (PAPER.md:L144 used textures): spline
+  // knots interleaved with their second derivatives (one 8-byte load per knot), ln R(ln E) first, then ln E(ln R), then
+  // Sigma/rho per HU bin, the HU bins and the HU -> bin table; MatBin holds each bin's offsets into these arrays
+  float2 *s_R = reinterpret_cast<float2 *>(smem_raw);
+  float2 *s_E = s_R + T.n_sr * T.n_e;
+  float *s_sig = reinterpret_cast<float *>(s_E + T.n_sr * T.n_r);
   MatBin *s_bins = reinterpret_cast<MatBin *>(s_sig + T.nbins * T.n_e);
   uint8_t *s_lut = reinterpret_cast<uint8_t *>(s_bins + T.nbins);
-  for (int i = threadIdx.x; i < T.n_sr * T.n_e; i += blockDim.x) { s_lnR[i] = T.lnR[i]; s_lnR2[i] = T.lnR2[i]; }
-  for (int i = threadIdx.x; i < T.n_sr * T.n_r; i += blockDim.x) { s_lnE[i] = T.lnE[i]; s_lnE2[i] = T.lnE2[i]; }
+  for (int i = threadIdx.x; i < T.n_sr * T.n_e; i += blockDim.x) s_R[i] = make_float2(T.lnR[i], T.lnR2[i]);
+  for (int i = threadIdx.x; i < T.n_sr * T.n_r; i += blockDim.x) s_E[i] = make_float2(T.lnE[i], T.lnE2[i]);
   for (int i = threadIdx.x; i < T.nbins * T.n_e; i += blockDim.x) s_sig[i] = T.sig_bin[i];
   for (int i = threadIdx.x; i < T.nbins * (int)(sizeof(MatBin) / 4); i += blockDim.x)
     reinterpret_cast<uint32_t *>(s_bins)[i] = reinterpret_cast<const uint32_t *>(T.bins)[i];
   for (int i = threadIdx.x; i < T.hu_lut_n; i += blockDim.x) s_lut[i] = T.hu_lut[i];
   __syncthreads();
+  const float *s_f = reinterpret_cast<const float *>(smem_raw);   // every table offset in MatBin counts floats from here
 
-  const float sz[3] = {G.d[0], G.d[1], G.d[2]};
+  const float szx = G.d[0], szy = G.d[1], szz = G.d[2];
   const int lane = threadIdx.x & 31;
   bool active = false, exhausted = false;
   Particle p; int ix = 0, iy = 0, iz = 0, nstep = 0; float path = 0.f; uint32_t tbase = 0;
   uint32_t c_steps = 0;                 // per-lane partial sums (a lane sees < 1e7 steps and < 1e4 MeV): 32-bit is enough
-  float c_dep = 0.f, c_esc = 0.f;
+  float c_dep = 0.f;
   const bool nuclear = T.opt_el || T.opt_ne;
 
   while (true) {
@@ -351,23 +358,27 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM) tr
 
     float dep = 0.f, let = 0.f; int dep_vox = p.vox;
     if (active) {
-      // the stream is re-keyed from (seed, history, particle, block) every step: only the block counter lives across steps
-      Rng g; g.init(P.seed, P.hist0 + p.hist, p.pid, p.blk);
-      // ---- material of the current voxel
+      // the stream is re-keyed from (history, particle, block) every step: only the block counter lives across steps
+      const uint64_t hid = P.hist0 + p.hist;
+      RngK g{P.rk, (uint32_t)hid, (uint32_t)(hid >> 32), p.pid, p.blk};
+      // ---- material of the current voxel (PAPER.md:L49)
       const int hu = G.hu[p.vox];
-      const int bin = hu_to_bin(T, s_lut, hu);
-      const MatBin &m = s_bins[bin];
-      const float rho = bin_density(m, hu), wf = rho * m.wet;
-      const int tab = m.table;
+      const MatBin &m = s_bins[s_lut[min(max(hu - T.hu_lut_lo, 0), T.hu_lut_n - 1)]];
+      const float rho = fmaf(m.slope, fminf(fmaxf((float)hu - m.hu_lo, 0.f), m.dhu), m.rho_lo), wf = rho * m.wet;
       c_steps++;
+      // draws of the step: r.x nuclear distance, r.y hinge (upper half), r.z and r.w (upper half) the MCS deflection; the
+      // lower halves of r.y and r.w go to the straggling sampler
       const uint4 r = g.next4();
+      const uint32_t spare = __byte_perm(r.y, r.w, 0x5410);
       // ---- 1. nuclear distance, face distance, residual range
-      const float e0 = p.e, lnEv = __logf(fminf(fmaxf(e0, T.e_min), T.e_max));
-      const EIdx k = e_index(T, lnEv);
+      const float e0 = p.e, l2 = flg2(fminf(fmaxf(e0, T.e_min), T.e_max)), lnEv = l2 * LN2;
+      const float te = fmaf(l2, T.c_l2, -T.c_e0);
+      const int ke = min(max((int)te, 0), T.n_e - 2);
+      const EIdx k{ke, te - (float)ke};
       float lam = BIG;
-      if (nuclear) { const float Sig = rho * lerp_tab(s_sig + bin * T.n_e, k); if (Sig > 0.f) lam = fdiv(-__logf(u01(r.x)), Sig); }
-      int ax, sg; const float dface = dist_to_face(p.r, p.d, sz, ax, sg);
-      const float lnRv = ln_range(T, s_lnR, s_lnR2, tab, k), Rg = __expf(lnRv), iwf = fdiv(1.0f, wf);
+      if (nuclear) { const float Sig = rho * lerp_tab(s_f + m.off_sig, k); lam = Sig > 0.f ? -LN2 * flg2(u23(r.x)) * frcp(Sig) : BIG; }
+      const float dface = fminf(fminf(axis_dist(p.r.x, p.d.x, szx), axis_dist(p.r.y, p.d.y, szy)), axis_dist(p.r.z, p.d.z, szz));
+      const float lnRv = spline_eval2(reinterpret_cast<const float2 *>(s_f + m.off_e), k.i, k.b), Rg = fex2(lnRv * LOG2E), iwf = frcp(wf);
       const float R = Rg * iwf, smax = T.s_max > 0.f ? T.s_max * iwf : BIG;
       // ---- 2. step = min (Reading R3.2)
       float dx = lam; int lim = 2;
@@ -377,64 +388,97 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM) tr
       // ---- 3-5. random hinge (PAPER.md:L69 ref [19]): first leg tau, deflect, second leg
       float tau = 0.f; V3 dnew = p.d;
       if (T.opt_mcs && dx > 0.f) {
-        tau = u01(r.y) * dx;
-        p.r = p.r + tau * p.d;
-        float th_m = -1.0f;
-        if (MCS_MODEL == 1) th_m = moliere_angle(T, m, e0, dx * rho, u01(r.z));
-        dnew = th_m >= 0.f ? deflect_by(p.d, th_m, r.w) : deflect(p.d, highland(T, e0, dx * rho * m.inv_x0), r.z, r.w);
+        tau = u16f(r.y >> 16) * dx;
+        p.r = {fmaf(tau, p.d.x, p.r.x), fmaf(tau, p.d.y, p.r.y), fmaf(tau, p.d.z, p.r.z)};
+        float th = -1.0f;
+        if (MCS_MODEL == 1) th = moliere_angle(T, m, e0, dx * rho, u23(r.z));
+        if (th < 0.f) {
+          // Highland theta0 times the Rayleigh radius of two independent projected Gaussians (Reading
+          // R3.4), under one square root: theta = K (e + MP)/pc2 [1 + 0.038 ln t] sqrt(-2 t ln u)
+          const float t = dx * rho * m.inv_x0;
+          const float rad = fsqrt(t * (-2.0f * LN2) * flg2(u23(r.z)));
+          th = (T.highland * 13.6f) * (e0 + MP) * frcp(e0 * (e0 + 2.0f * MP)) * rad * fmaxf(0.f, fmaf(0.038f * LN2, flg2(t), 1.0f));
+        }
+        float st, ct, sp, cp;
+        sincos_small(th, &st, &ct); sincos_2pi(u16f(r.w >> 16), &sp, &cp);
+        dnew = rotate(p.d, st, ct, sp, cp);
       }
-      const float ell = dx - tau; int ax2, sg2; const float d2 = dist_to_face(p.r, dnew, sz, ax2, sg2);
-      float L; int cls;
+      const float ell = dx - tau;
+      const float tx = axis_dist(p.r.x, dnew.x, szx), ty = axis_dist(p.r.y, dnew.y, szy), tz = axis_dist(p.r.z, dnew.z, szz);
+      float d2 = tx; int ax2 = 0;                                // ties: x before y before z
+      if (ty < d2) { d2 = ty; ax2 = 1; }
+      if (tz < d2) { d2 = tz; ax2 = 2; }
       // a face-limited step always ends on a face (dx = distance to the voxel boundary; Reading R3.5)
-      if (ell >= d2 || lim == 1) { L = tau + d2; p.r = p.r + d2 * dnew; cls = 1; }
-      else { L = dx; p.r = p.r + ell * dnew; cls = lim; }
-      p.r.x = fminf(fmaxf(p.r.x, 0.f), sz[0]); p.r.y = fminf(fmaxf(p.r.y, 0.f), sz[1]); p.r.z = fminf(fmaxf(p.r.z, 0.f), sz[2]);
+      const bool onface = ell >= d2 || lim == 1;
+      const float leg = onface ? d2 : ell, L = tau + leg;
+      const int cls = onface ? 1 : lim;
+      p.r.x = fminf(fmaxf(fmaf(leg, dnew.x, p.r.x), 0.f), szx);
+      p.r.y = fminf(fmaxf(fmaf(leg, dnew.y, p.r.y), 0.f), szy);
+      p.r.z = fminf(fmaxf(fmaf(leg, dnew.z, p.r.z), 0.f), szz);
       p.d = dnew; if (DBG) path += L;
+      // boundary step: the neighbour voxel (done before the energy loss, whose registers it would otherwise compete with;
+      // if the proton stops in this step the advanced index is simply not used)
+      bool exits = false;
+      if (cls == 1) {
+        const bool up = (ax2 == 0 ? dnew.x : ax2 == 1 ? dnew.y : dnew.z) > 0.f;
+        const int sg2 = up ? 1 : -1;
+        int nidx, nmax;
+        if (ax2 == 0) { ix += sg2; nidx = ix; nmax = G.nx; p.r.x = up ? 0.f : szx; }
+        else if (ax2 == 1) { iy += sg2; nidx = iy; nmax = G.ny; p.r.y = up ? 0.f : szy; }
+        else { iz += sg2; nidx = iz; nmax = G.nz; p.r.z = up ? 0.f : szz; }
+        exits = nidx < 0 || nidx >= nmax;
+        if (!exits) p.vox = (iz * G.ny + iy) * G.nx + ix;
+      }
       // ---- 6. energy loss from the range table (Eq.2) + straggling (L61)
       float loss;
-      if (cls == 3) { loss = e0; let = L > 0.f ? fdiv(0.1f * e0, L) : 0.f; }   // 7. range-out: everything stays here (L71)
+      if (cls == 3) { loss = e0; if (EXTRA) let = L > 0.f ? fdiv(0.1f * e0, L) : 0.f; }   // 7. range-out: everything stays here (L71)
       else if (L <= 0.f) loss = 0.f;
       else {
-        loss = mean_loss(T, s_lnE, s_lnE2, tab, e0, lnEv, lnRv, Rg, L * wf);
-        let = fdiv(0.1f * loss, L);                              // keV/um of this step (Reading R9)
-        if (T.opt_strag) loss = straggle(T, g, e0, loss, L * rho, m.zoa, low_bytes(r));
+        // E - E(R(E) - dr), written with expm1 so that a vanishing step loses nothing
+        const float dr = L * wf;
+        float lnE1 = T.ln_emin;
+        if (Rg - dr > 0.f) {
+          const float xr = lnRv + log1p_small(-dr * frcp(Rg));
+          const float tr = (xr - m.lnr_lo) * m.inv_hr;
+          const int kr = min(max((int)tr, 0), T.n_r - 2);
+          lnE1 = spline_eval2(reinterpret_cast<const float2 *>(s_f + m.off_r), kr, tr - (float)kr);
+          lnE1 = xr <= m.lnr_lo ? T.ln_emin : (xr >= m.lnr_hi ? T.ln_emax : lnE1);
+        }
+        loss = fminf(fmaxf(-e0 * expm1_small(lnE1 - lnEv), 0.f), e0);
+        if (EXTRA) let = fdiv(0.1f * loss, L);                   // keV/um of this step (Reading R9)
+        if (T.opt_strag) loss = straggle(T, g, e0, loss, L * rho, m.zoa, spare);
       }
       p.e = e0 - loss; dep = loss;
       bool alive = cls != 3;
       if (alive && p.e <= T.e_cut) { dep += p.e; p.e = 0.f; alive = false; }           // L71 (2)
       c_dep += dep;
-      if (alive && cls == 1) {                                                        // boundary: next voxel
-        int nidx, nmax;
-        if (ax2 == 0) { ix += sg2; nidx = ix; nmax = G.nx; p.r.x = sg2 > 0 ? 0.f : sz[0]; }
-        else if (ax2 == 1) { iy += sg2; nidx = iy; nmax = G.ny; p.r.y = sg2 > 0 ? 0.f : sz[1]; }
-        else { iz += sg2; nidx = iz; nmax = G.nz; p.r.z = sg2 > 0 ? 0.f : sz[2]; }
-        if (nidx < 0 || nidx >= nmax) { c_esc += p.e; alive = false; }         // L71 (3)
-        else p.vox = (iz * G.ny + iy) * G.nx + ix;
-      }
+      if (alive && exits) { atomicAdd(&cnt->e_escape, (double)p.e); alive = false; }   // L71 (3): leaves the grid
       if (DBG) ++nstep;
+      p.blk = g.blk;
       if (alive && cls == 2 && !DBG) {
         // ---- 8. discrete nuclear event at the end point (L71): handed to event_kernel, which picks the class and
         // the target element with all lanes busy instead of one lane of this warp
-        p.blk = g.blk; p.vox = dep_vox;
+        p.vox = dep_vox;
         if (!queue_push(q_ev, p)) atomicOr(&cnt->overflow, 2u);
         alive = false;
       }
       if (DBG && alive && P.max_steps > 0 && nstep >= P.max_steps) alive = false;
-      p.blk = g.blk;
       if (!alive) {
         active = false;
         if (DBG && P.dbg_out && p.pid == 0u) {
           float *o = P.dbg_out + 8ull * p.hist;
-          o[0] = ix * sz[0] + p.r.x; o[1] = iy * sz[1] + p.r.y; o[2] = iz * sz[2] + p.r.z;
+          o[0] = ix * szx + p.r.x; o[1] = iy * szy + p.r.y; o[2] = iz * szz + p.r.z;
           o[3] = p.d.x; o[4] = p.d.y; o[5] = p.d.z; o[6] = p.e; o[7] = path;
         }
       }
     }
-    deposit(tally, tbase + (uint32_t)dep_vox, dep, dep != 0.f, P.aggregate, P.let_num, P.let_den, (uint32_t)dep_vox, let > 0.f ? dep : 0.f, let);
-    if (P.roi_map != nullptr && dep != 0.f) score_influence(P, p.aux, dep_vox, dep);
+    if (EXTRA) {
+      deposit(tally, tbase + (uint32_t)dep_vox, dep, dep != 0.f, P.aggregate, P.let_num, P.let_den, (uint32_t)dep_vox, let > 0.f ? dep : 0.f, let);
+      if (P.roi_map != nullptr && dep != 0.f) score_influence(P, p.aux, dep_vox, dep);
+    } else if (dep != 0.f) atomicAdd(tally + tbase + (uint32_t)dep_vox, dep);
   }
   flush(&cnt->n_steps, (unsigned long long)c_steps);
-  flush(&cnt->e_deposit, (double)c_dep); flush(&cnt->e_escape, (double)c_esc);
+  flush(&cnt->e_deposit, (double)c_dep);
 }
 
 // ------------------------------------------------------------------ event class and target element (Reading R5)
