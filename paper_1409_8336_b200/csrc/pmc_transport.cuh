@@ -284,7 +284,10 @@ __device__ __forceinline__ void deposit(float *tally, uint32_t tvox, float e, bo
 // Persistent kernel: every lane pulls a particle from the input queue, steps it in registers until it stops,
 // leaves the grid or reaches a discrete nuclear event, then refills from the queue (warp-aggregated fetch).
 // Particles that reach an event are appended to the elastic or non-elastic queue; nothing else is written back.
-constexpr int TRANSPORT_THREADS = 256, TRANSPORT_BLOCKS_PER_SM = 4;
+#ifndef PMC_TRANSPORT_BLOCKS
+#define PMC_TRANSPORT_BLOCKS 3
+#endif
+constexpr int TRANSPORT_THREADS = 256, TRANSPORT_BLOCKS_PER_SM = PMC_TRANSPORT_BLOCKS;
 
 // distance along one axis to the face the particle is heading for (voxel-local r in [0, size], inv = 1/d); BIG if d = 0
 __device__ __forceinline__ float axis_dist(float r, float d, float size) {
@@ -339,7 +342,7 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM) tr
   const bool nuclear = T.opt_el || T.opt_ne;
 
   while (true) {
-    // ---- refill idle lanes
+    // ---- refill idle lanes (at once: waiting until several lanes are idle was measured slower, 39.4 vs 37.3 ms at 8 lanes)
     const unsigned need = __ballot_sync(0xffffffffu, !active && !exhausted);
     if (need) {
       uint32_t base = 0;
