@@ -26,11 +26,36 @@ if ROOT not in sys.path:
 
 METRIC = "proton histories/sec (full physics, dose on CT grid)"
 UNIT = "histories/s"
-# algorithmic thread-instructions of one condensed-history step of the transport kernel
-ALGO_INST_PER_STEP = 520.0
-# dram__bytes_read.sum + dram__bytes_write.sum of the first-generation transport launch of a 1e7-history C4 step, per
-# history (one `ncu --set full` capture, profiles/r01_transport_full.md): 641.4 MB + 186.3 MB
-NCU_DRAM_BYTES_PER_HISTORY_C4 = 82.8
+# DESIGN.md section 7 "Roofline": algorithmic thread-instructions of ONE condensed-history step of the step kernel, item by
+# item - what the method itself needs with ideal code (every multiply-add fused, no moves, no address arithmetic, no
+# reconvergence instructions), counted against the SASS of profiles/r02_transport_sass_histogram.md.
+ALGO_ITEMS = {
+    "philox4x32_10_two_blocks (2 x 10 rounds x (2 mul.wide + 2 xor3))": 80,
+    "seven_uniforms_to_float (2 each)": 14,
+    "hu_gather_bin_lookup_density": 8,
+    "ln_E_and_table_index": 8,
+    "sigma_lerp_and_nuclear_distance (ln u, 1/Sigma)": 8,
+    "range_spline_and_exp (4 loads, 9 flops, ex2)": 15,
+    "face_distances_two_calls (3 axes x 6 + min/argmin)": 42,
+    "step_length_min_of_four": 8,
+    "hinge_move_highland_rayleigh (rcp, lg2 x 2, sqrt)": 15,
+    "sincos_theta_series_and_azimuth": 15,
+    "direction_rotation_and_renormalisation": 24,
+    "second_leg_position_clamps_axis": 15,
+    "mean_loss (log1p, inverse spline, expm1)": 36,
+    "straggling (kinematics 14, normal 7, T_c/mu/mean 12, Poisson 8, two candidates 14, cumulants 12, Wilson-Hilferty 12, clamp 2)": 81,
+    "energy_update_and_termination": 8,
+    "voxel_index_update_and_bounds": 12,
+    "dose_red (address, atomic)": 4,
+    "loop_vote_refill_check": 10,
+}
+ALGO_INST_PER_STEP = float(sum(ALGO_ITEMS.values()))
+# One-off `ncu --set full` capture of the first-generation step-kernel launch of a 1e7-history C4 step
+# (profiles/r02_transport_full.md; NOT measured in this run): DRAM bytes per history, executed thread-instructions per
+# condensed step, active lanes per warp instruction, issue-slot utilisation.
+NCU_CAPTURE = {"source": "profiles/r02_transport_full.md (one-off ncu capture, not measured in this run)",
+               "dram_bytes_per_history_c4": 82.8, "executed_thread_inst_per_step": 655.0, "lanes_per_warp_inst": 28.8,
+               "issue_slot_utilisation_pct": 78.3}
 ISSUE_LANES_PER_SM_PER_CLK = 128.0     # 4 schedulers x 32 lanes
 N_SM = 148
 
@@ -155,6 +180,7 @@ def main():
     ap.add_argument("--workload", default="c4")
     ap.add_argument("--histories", type=int, default=0, help="histories per step and per rank (0 = the workload's)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extras", action="store_true", help="skip the C2 / C5 / LET_d / gamma-index measurements")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     args = ap.parse_args()
     rank, local_rank, world = _env_int("RANK", 0), _env_int("LOCAL_RANK", 0), _env_int("WORLD_SIZE", 1)
@@ -259,25 +285,10 @@ def main():
     h2d = int(w["hu"].nbytes + spots.nbytes)
     d2h = int(2 * nvox * 4)
 
-    # ---- SURVEY 8(f) rows built so far, measured on the same workload (not part of the timed steps above)
+    # ---- other rows of SURVEY 8(d)/(f), measured after the timed steps on rank 0 (not part of `value`)
     extras = None
-    if rank == 0:
-        pm.load_ct(hu_dev, w["vox"])
-        pm.set_option("score_letd", 1.0)
-        pm.simulate(spots, n_hist, w["seed"] + 200)
-        d_a, _ = pm.simulate(spots, n_hist, w["seed"] + 201); let_ms = pm.timing()["total_ms"]; d_a = d_a.clone()
-        pm.set_option("score_letd", 0.0)
-        d_b, _ = pm.simulate(spots, n_hist, w["seed"] + 202); plain_ms = pm.timing()["total_ms"]
-        tissue = torch.as_tensor(w["hu"] >= -950, device=dev)
-        d_a *= tissue; d_b = d_b * tissue
-        pm.gamma_index(d_a, d_b, w["vox"], 0.02, 0.2, 0.1)
-        g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        g0.record()
-        for _ in range(5):
-            _, g_rate = pm.gamma_index(d_a, d_b, w["vox"], 0.02, 0.2, 0.1)
-        g1.record(); torch.cuda.synchronize(dev)
-        extras = {"letd_scoring_ms_per_step": let_ms, "same_without_letd_ms": plain_ms,
-                  "gamma_index_2pct_2mm_ms_per_call": g0.elapsed_time(g1) / 5, "gamma_pass_rate_two_seeds": g_rate}
+    if rank == 0 and not args.no_extras:
+        extras = measure_extras(pm, w, n_hist, spots, hu_dev, stream, dev, tables)
 
     if rank == 0:
         # ---- roofline of the dominant kernel (transport_kernel): plain-ALU issue bound
@@ -286,9 +297,13 @@ def main():
         achieved = ALGO_INST_PER_STEP * steps_total / (t_transport * 1e-3) / 1e9 if t_transport > 0 else 0.0
         roofline = {"bound": "alu", "kernel": "transport_kernel", "achieved": achieved, "peak": peak,
                     "unit": "Gthread-inst/s", "frac": achieved / peak if peak else None,
-                    "traffic": NCU_DRAM_BYTES_PER_HISTORY_C4 * n_hist if w["name"] == "c4" else None,
-                    "traffic_note": "DRAM bytes of the first-generation launch (ncu capture in profiles/); the kernel is "
-                                    "issue-bound, HBM carries < 1 % of its peak",
+                    "traffic": NCU_CAPTURE["dram_bytes_per_history_c4"] * n_hist if w["name"] == "c4" else None,
+                    "traffic_note": "from a one-off ncu capture (DRAM bytes of the first-generation launch), not measured "
+                                    "in this run; the kernel is issue-bound, HBM carries < 1 % of its peak",
+                    "ncu_capture": NCU_CAPTURE,
+                    "frac_of_executed": (NCU_CAPTURE["executed_thread_inst_per_step"] * steps_total / (t_transport * 1e-3) / 1e9
+                                         / peak) if (t_transport > 0 and peak and w["name"] == "c4") else None,
+                    "algorithmic_items": ALGO_ITEMS,
                     "peak_source": "148 SMs x 4 schedulers x 32 lanes x median SM clock under load (derived, DESIGN.md)",
                     "avg_launch_ms": t_transport / max(1, n_transport), "launches": n_transport,
                     "algorithmic_inst_per_condensed_step": ALGO_INST_PER_STEP,
@@ -321,6 +336,59 @@ def main():
     if world > 1:
         dist.barrier()
         dist.destroy_process_group()
+
+
+def measure_extras(pm, w, n_hist, spots, hu_dev, stream, dev, tables):
+    """LET_d and gamma index on the bench workload; pmc_nonelastic events/s on the paper's Table I workload (C2,
+    PAPER.md:L187-203: 2.6e6 events, p + 16O and p + 40Ca at 200 MeV, records copied to the host); C5 histories/s."""
+    import torch
+    import inputs
+    out = {}
+    pm.load_ct(hu_dev, w["vox"])
+    pm.set_option("score_letd", 1.0)
+    pm.simulate(spots, n_hist, w["seed"] + 200)
+    d_a, _ = pm.simulate(spots, n_hist, w["seed"] + 201); let_ms = pm.timing()["total_ms"]; d_a = d_a.clone()
+    pm.set_option("score_letd", 0.0)
+    d_b, _ = pm.simulate(spots, n_hist, w["seed"] + 202); plain_ms = pm.timing()["total_ms"]
+    with torch.cuda.stream(stream):                      # the library launches on `stream`: mask and time there too
+        tissue = torch.as_tensor(w["hu"] >= -950, device=dev)
+        d_a = d_a * tissue; d_b = d_b * tissue
+    stream.synchronize()
+    pm.gamma_index(d_a, d_b, w["vox"], 0.02, 0.2, 0.1)
+    g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    g0.record(stream)
+    for _ in range(5):
+        _, g_rate = pm.gamma_index(d_a, d_b, w["vox"], 0.02, 0.2, 0.1)
+    g1.record(stream); stream.synchronize()
+    out.update(letd_scoring_ms_per_step=let_ms, same_without_letd_ms=plain_ms,
+               gamma_index_2pct_2mm_ms_per_call=g0.elapsed_time(g1) / 5, gamma_pass_rate_two_seeds=g_rate)
+    # C2: standalone non-elastic collisions
+    c2 = {}
+    n_ev = 2_600_000
+    pm.nonelastic(8, 16, 200.0, 10_000, 1)
+    for name, (z, a) in (("p+16O_200MeV", (8, 16)), ("p+40Ca_200MeV", (20, 40))):
+        t0 = time.perf_counter(); rec, off = pm.nonelastic(z, a, 200.0, n_ev, 7); dt = time.perf_counter() - t0
+        cn = pm.counters()
+        c2[name] = {"events_per_s": n_ev / dt, "events": n_ev, "records": int(len(rec)), "seconds_incl_copy_to_host": dt,
+                    "inc_tries_per_event": cn["n_inc_tries"] / n_ev, "guard_trips": cn["n_inc_guard_trips"],
+                    "capacity_trips": cn["n_inc_cap_trips"], "max_stack": cn["inc_max_stack"], "max_out": cn["inc_max_out"]}
+        del rec, off
+    c2["context"] = "paper Table I (GTX680, fast-math): 3.9e5 (16O) and 2.7e5 (40Ca) events/s"
+    out["c2_pmc_nonelastic"] = c2
+    # C5: the large pelvis case, all 1e8 histories once (after a short warm-up)
+    w5 = inputs.workload("c5")
+    pm.set_hu_materials(w5["materials"])
+    hu5 = torch.as_tensor(w5["hu"], device=dev)
+    pm.load_ct(hu5, w5["vox"])
+    pm.simulate(w5["spots"], 1_000_000, 1)
+    t0 = time.perf_counter(); pm.simulate(w5["spots"], w5["n_histories"], w5["seed"]); dt = time.perf_counter() - t0
+    tm, cn = pm.timing(), pm.counters()
+    out["c5"] = {"workload": w5["label"], "histories_per_s": w5["n_histories"] / (tm["total_ms"] * 1e-3),
+                 "ms_device": tm["total_ms"], "seconds_wall": dt, "steps_per_history": cn["n_steps"] / w5["n_histories"],
+                 "kernel_ms": {k: tm[k] for k in ("sampler_ms", "transport_ms", "elastic_ms", "inc_ms", "evaporation_ms",
+                                                  "statistics_ms")}, "n_spots": w5["n_spots"]}
+    pm.set_hu_materials(w["materials"]); pm.load_ct(hu_dev, w["vox"])
+    return out
 
 
 def _measured_hbm():

@@ -18,6 +18,7 @@
  */
 #ifndef PMC_H
 #define PMC_H
+#include <stddef.h>
 #include <stdint.h>
 #ifdef __cplusplus
 extern "C" {
@@ -99,6 +100,9 @@ typedef struct pmc_counters {    /* totals of the last pmc_simulate / pmc_nonela
   /* energy ledger, MeV: e_source = all the sinks below, up to fp32 rounding */
   double e_source, e_deposit, e_escape, e_neutron, e_gamma, e_q, e_air;
   uint64_t n_zab_violations;     /* events whose charge or baryon number failed to balance (must be 0) */
+  /* Reading R6.8 bookkeeping of the cascade: attempts abandoned by the 1024-step guard, attempts abandoned because the
+   * fixed capacities were reached (16 waiting or 16 outgoing nucleons), and the deepest stack / most outgoing nucleons seen */
+  uint64_t n_inc_guard_trips, n_inc_cap_trips, inc_max_stack, inc_max_out;
 } pmc_counters;
 
 typedef struct pmc_timing {      /* CUDA-event time (ms) per kernel class over the last pmc_simulate call */
@@ -111,11 +115,21 @@ typedef struct pmc_ctx pmc_ctx;
 /* Create a context on CUDA device `device`.  `cuda_stream` is a cudaStream_t owned by the caller (NULL = the
  * legacy default stream); all kernels of this context are launched on it. */
 int  pmc_create(pmc_ctx **out, int device, void *cuda_stream);
+/* The same with the caller's device allocator ("so PyTorch's allocator owns the memory"): every device
+ * buffer of the context - tables, particle queues (6 x 48 B x 1.25 x sub-group), per-batch tallies (4 B x n_batches x
+ * voxels), scratch - is obtained from alloc_fn(bytes, user) (a DEVICE pointer on `device`, 256-byte aligned, or NULL on
+ * failure -> PMC_E_CUDA from the call that needed it) and returned with free_fn(ptr, user); both are called from the
+ * thread that calls into the library, never from a CUDA callback.  Both NULL = cudaMalloc / cudaFree (pmc_create). */
+typedef void *(*pmc_alloc_fn)(size_t bytes, void *user);
+typedef void (*pmc_free_fn)(void *ptr, void *user);
+int  pmc_create_with_allocator(pmc_ctx **out, int device, void *cuda_stream, pmc_alloc_fn alloc_fn, pmc_free_fn free_fn,
+                               void *user);
 void pmc_destroy(pmc_ctx *ctx);
 
 /* load the physics tables (HOST, copied).  Builds the device tables and the
  * 15-shell nucleus models (L77) for every element with A > 1.
- * Errors: null pointers, sizes out of range, non-monotone range table, element missing from the mass table. */
+ * Errors: null pointers, sizes out of range, non-monotone range table, element missing from the mass table, non-zero
+ * sigma_ne_mb for an element with A < 2 (hydrogen has no non-elastic channel below 250 MeV). */
 int  pmc_load_physics_tables(pmc_ctx *ctx, const pmc_tables *tables_host);
 
 /* HU -> density + composition (HOST array, copied).  Needs the physics tables. */
@@ -142,7 +156,7 @@ int  pmc_set_option(pmc_ctx *ctx, const char *key, double value);
 /* PAPER.md:L134-138 (Fig 2): simulate n_histories primaries drawn from the spot list (HOST, nspots entries),
  * in n_batches groups; history h uses the Philox4x32-10 stream keyed (seed, h).  dose_dev / sigma_dev: DEVICE
  * arrays of nx*ny*nz float, overwritten: mean dose in Gy per primary history and its standard error from the
- * batch-to-batch scatter (Reading R8).  n_histories must be < 2^32 per call.
+ * batch-to-batch scatter (Reading R8).  n_batches <= n_histories < 2^32 per call (a batch needs a history, L134).
  * Errors: PMC_E_STATE (tables/materials/CT missing), PMC_E_CAPACITY (particle queue overflow), PMC_E_CUDA. */
 int  pmc_simulate(pmc_ctx *ctx, const pmc_spot *spots_host, int nspots, uint64_t n_histories, uint64_t seed,
                   float *dose_dev, float *sigma_dev);
@@ -187,7 +201,7 @@ int  pmc_get_letd(pmc_ctx *ctx, float *letd_dev);
  * gamma_dev: DEVICE, nx*ny*nz float, caller-owned, overwritten.  pass_rate_host (HOST, may be NULL): fraction of the
  * evaluated voxels with gamma <= 1 (1 if none is evaluated).  Needs no tables, materials or CT.
  * Errors: PMC_E_INVALID_ARG (null pointers, non-positive sizes or criteria), PMC_E_UNSUPPORTED (nz > 65535, search
- * sphere of more than 4e6 voxels). */
+ * sphere of more than 4e6 voxels or reaching more than 32767 voxels along an axis). */
 int  pmc_gamma_index(pmc_ctx *ctx, const float *ref_dev, const float *eval_dev, int nx, int ny, int nz,
                      double dx_cm, double dy_cm, double dz_cm, double dd_frac, double dta_cm, double low_dose_frac,
                      double search_cm, float *gamma_dev, double *pass_rate_host);

@@ -960,6 +960,7 @@ int opmc_simulate(opmc_ctx *c, const opmc_spot *spots, int nspots, uint64_t n, u
   if (!c->T.loaded || c->mats.empty() || c->hu.empty()) return fail(c, "call order: tables, materials, ct, simulate");
   const size_t nv = c->hu.size(); const int B = c->T.n_batches;
   if (B < 2) return fail(c, "need >= 2 batches");
+  if (n < (uint64_t)B) return fail(c, "n_histories must be at least n_batches");   // groups of N/10 histories
   std::vector<double> cdf = spot_cdf(spots, nspots), tally(nv), s1(nv, 0.0), s2(nv, 0.0);
   c->cnt = opmc_counters{};
   for (int i = 0; i < OPMC_MAX_ELEM; ++i) { c->ev_el[i] = 0; c->ev_ne[i] = 0; }

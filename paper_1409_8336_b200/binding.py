@@ -17,7 +17,7 @@ MAX_ELEM = 8
 _D = C.POINTER(C.c_double)
 _I = C.POINTER(C.c_int32)
 
-EXPORTS = ["pmc_create", "pmc_destroy", "pmc_load_physics_tables", "pmc_set_hu_materials", "pmc_load_ct",
+EXPORTS = ["pmc_create", "pmc_create_with_allocator", "pmc_destroy", "pmc_load_physics_tables", "pmc_set_hu_materials", "pmc_load_ct",
            "pmc_load_ct_host", "pmc_set_option", "pmc_simulate", "pmc_simulate_host", "pmc_nonelastic",
            "pmc_get_counters", "pmc_get_timing", "pmc_get_letd", "pmc_gamma_index", "pmc_set_dose_influence", "pmc_last_error", "pmc_philox4x32_10", "pmc_range_of_energy",
            "pmc_energy_of_range", "pmc_straggle", "pmc_elastic", "pmc_first_steps"]
@@ -44,7 +44,8 @@ class Counters(C.Structure):
     _fields_ = [(k, C.c_uint64) for k in ("n_steps", "n_elastic", "n_nonelastic", "n_secondary_protons", "n_missed",
                                           "n_inc_tries", "n_generations")] + \
                [(k, C.c_double) for k in ("e_source", "e_deposit", "e_escape", "e_neutron", "e_gamma", "e_q", "e_air")] + \
-               [("n_zab_violations", C.c_uint64)]
+               [(k, C.c_uint64) for k in ("n_zab_violations", "n_inc_guard_trips", "n_inc_cap_trips", "inc_max_stack",
+                                          "inc_max_out")]
 
 
 class Timing(C.Structure):
@@ -56,6 +57,9 @@ class Timing(C.Structure):
 SECONDARY_DTYPE = np.dtype([("Z", "<i2"), ("A", "<i2"), ("origin", "u1"), ("pad", "u1", (3,)),
                             ("ke", "<f4"), ("dir", "<f4", (3,))])
 assert SECONDARY_DTYPE.itemsize == 24
+
+_ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)      # pmc_alloc_fn
+_FREE_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_void_p)               # pmc_free_fn
 
 _lib = None
 
@@ -90,7 +94,9 @@ def _ptr(t):
 class Pmc:
     """One libpmc context on one CUDA device; methods carry the names of the C calls."""
 
-    def __init__(self, device=0, stream=None):
+    def __init__(self, device=0, stream=None, torch_allocator=True):
+        """torch_allocator: the context's device scratch (queues, tallies, tables) comes from PyTorch's caching allocator
+        through pmc_create_with_allocator, so that torch sees and accounts for it; False: plain cudaMalloc (pmc_create)."""
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("libpmc needs a CUDA device (no CPU fallback)")
@@ -100,16 +106,32 @@ class Pmc:
         self.stream = stream
         self.ctx = C.c_void_p()
         sp = C.c_void_p(stream.cuda_stream if stream is not None else 0)
-        rc = self.lib.pmc_create(C.byref(self.ctx), C.c_int(device), sp)
+        if torch_allocator:
+            raw_stream = stream.cuda_stream if stream is not None else 0
+
+            def _alloc(nbytes, _user):
+                try:
+                    return torch.cuda.caching_allocator_alloc(int(nbytes), device, raw_stream)
+                except Exception:               # out of memory: NULL -> PMC_E_CUDA from the call that needed it
+                    return None
+
+            def _free(ptr, _user):
+                torch.cuda.caching_allocator_delete(ptr)
+
+            self._alloc_cb = _ALLOC_FN(_alloc); self._free_cb = _FREE_FN(_free)     # kept alive with the context
+            rc = self.lib.pmc_create_with_allocator(C.byref(self.ctx), C.c_int(device), sp, self._alloc_cb, self._free_cb, None)
+        else:
+            rc = self.lib.pmc_create(C.byref(self.ctx), C.c_int(device), sp)
         if rc != 0:
             raise PmcError(rc, "pmc_create failed (no usable CUDA device?)")
         self._keep = {}
         self.shape = None
 
     def close(self):
-        if self.ctx:
+        import sys
+        if self.ctx and not sys.is_finalizing():      # at interpreter exit the allocator callbacks may be gone already
             self.lib.pmc_destroy(self.ctx)
-            self.ctx = C.c_void_p()
+        self.ctx = C.c_void_p()
 
     def __del__(self):
         try:

@@ -24,13 +24,27 @@ constexpr double PI_D = 3.14159265358979323846;
 
 struct HostMat { pmc_hu_bin b; double zoa; };
 
+// Device scratch comes from the context's allocator: cudaMalloc / cudaFree by default, or the pair of callbacks given to
+// pmc_create_with_allocator (so that e.g. PyTorch's caching allocator owns the queues and tallies).
+struct Allocator { pmc_alloc_fn alloc = nullptr; pmc_free_fn free = nullptr; void *user = nullptr; };
+struct DevBufBase {
+  const Allocator *A = nullptr;
+  virtual void release() = 0;
+  virtual ~DevBufBase() {}
+};
+// every DevBuf constructed while this points to a list (i.e. while a pmc_ctx is being constructed) is entered into it
+thread_local std::vector<DevBufBase *> *tl_registry = nullptr;
+
 template <typename T>
-struct DevBuf {
+struct DevBuf : DevBufBase {
   T *p = nullptr; size_t n = 0;
+  DevBuf() { if (tl_registry) tl_registry->push_back(this); }
   cudaError_t alloc(size_t count) {
     if (count <= n && p) return cudaSuccess;
     release();
-    cudaError_t e = cudaMalloc(&p, count * sizeof(T));
+    cudaError_t e = cudaSuccess;
+    if (A && A->alloc) { p = static_cast<T *>(A->alloc(count * sizeof(T), A->user)); if (!p) e = cudaErrorMemoryAllocation; }
+    else e = cudaMalloc(&p, count * sizeof(T));
     if (e == cudaSuccess) n = count; else p = nullptr;
     return e;
   }
@@ -40,7 +54,10 @@ struct DevBuf {
     if (h.empty()) return cudaSuccess;
     return cudaMemcpyAsync(p, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice, s);
   }
-  void release() { if (p) cudaFree(p); p = nullptr; n = 0; }
+  void release() override {
+    if (p) { if (A && A->free) A->free(p, A->user); else cudaFree(p); }
+    p = nullptr; n = 0;
+  }
 };
 
 struct QueueMem {
@@ -63,6 +80,7 @@ struct QueueMem {
 }  // namespace
 
 struct pmc_ctx {
+  Allocator allocator; std::vector<DevBufBase *> bufs;   // every device buffer of the context (filled by pmc_create)
   int device = 0; cudaStream_t stream = nullptr;
   std::string err;
   // host copies
@@ -330,6 +348,7 @@ int fetch_counters(pmc_ctx *c) {
   pmc_counters &o = c->counters;
   o.n_steps = h.n_steps; o.n_elastic = h.n_elastic; o.n_nonelastic = h.n_nonelastic; o.n_secondary_protons = h.n_secondary;
   o.n_missed = h.n_missed; o.n_inc_tries = h.n_inc_tries; o.n_zab_violations = h.n_zab_bad;
+  o.n_inc_guard_trips = h.n_inc_guard; o.n_inc_cap_trips = h.n_inc_cap; o.inc_max_stack = h.inc_max_stack; o.inc_max_out = h.inc_max_out;
   o.e_source = h.e_source; o.e_deposit = h.e_deposit; o.e_escape = h.e_escape; o.e_neutron = h.e_neutron; o.e_gamma = h.e_gamma;
   o.e_q = h.e_q; o.e_air = h.e_air;
   if (h.overflow) { char b[96]; snprintf(b, sizeof b, "internal queue overflow (mask 0x%x)", h.overflow); return fail(c, PMC_E_CAPACITY, b); }
@@ -350,7 +369,7 @@ int air_params(pmc_ctx *c, float &rho, float &wf, float &inv_x0, float &zoa, int
 int load_ct_common(pmc_ctx *c, const int16_t *hu_dev, int nx, int ny, int nz, double dx, double dy, double dz, const double *origin) {
   c->G.hu = hu_dev; c->G.nx = nx; c->G.ny = ny; c->G.nz = nz; c->G.d[0] = (float)dx; c->G.d[1] = (float)dy; c->G.d[2] = (float)dz;
   c->G.vol = (float)(dx * dy * dz);
-  for (int k = 0; k < 3; ++k) c->G.d[k] = (float)(k == 0 ? dx : k == 1 ? dy : dz);
+  for (int k = 0; k < 3; ++k) { c->G.dd[k] = k == 0 ? dx : k == 1 ? dy : dz; c->G.d[k] = (float)c->G.dd[k]; }
   for (int k = 0; k < 3; ++k) c->origin[k] = origin ? origin[k] : 0.0;   // applied on the host to the spot positions
   c->have_ct = true; c->n_roi = 0; c->dij_dev = nullptr;      // a ROI belongs to the grid it was given for
   return PMC_OK;
@@ -360,13 +379,19 @@ int load_ct_common(pmc_ctx *c, const int16_t *hu_dev, int nx, int ny, int nz, do
 
 extern "C" {
 
-int pmc_create(pmc_ctx **out, int device, void *cuda_stream) {
-  if (!out) return PMC_E_INVALID_ARG;
+int pmc_create_with_allocator(pmc_ctx **out, int device, void *cuda_stream, pmc_alloc_fn alloc_fn, pmc_free_fn free_fn, void *user) {
+  if (!out || ((alloc_fn == nullptr) != (free_fn == nullptr))) return PMC_E_INVALID_ARG;
   *out = nullptr;
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev <= 0 || device < 0 || device >= ndev) return PMC_E_CUDA;   // no CPU fallback
   if (cudaSetDevice(device) != cudaSuccess) return PMC_E_CUDA;
+  std::vector<DevBufBase *> reg;
+  tl_registry = &reg;
   pmc_ctx *c = new pmc_ctx();
+  tl_registry = nullptr;
+  c->bufs = reg;
+  c->allocator.alloc = alloc_fn; c->allocator.free = free_fn; c->allocator.user = user;
+  for (DevBufBase *b : c->bufs) b->A = &c->allocator;
   c->device = device; c->stream = (cudaStream_t)cuda_stream;
   cudaDeviceProp prop{};
   if (cudaGetDeviceProperties(&prop, device) == cudaSuccess) c->n_sm = prop.multiProcessorCount;
@@ -374,16 +399,15 @@ int pmc_create(pmc_ctx **out, int device, void *cuda_stream) {
   return PMC_OK;
 }
 
+int pmc_create(pmc_ctx **out, int device, void *cuda_stream) {
+  return pmc_create_with_allocator(out, device, cuda_stream, nullptr, nullptr, nullptr);
+}
+
 void pmc_destroy(pmc_ctx *c) {
   if (!c) return;
   cudaSetDevice(c->device);
   cudaStreamSynchronize(c->stream);
-  c->d_lnR.release(); c->d_lnR2.release(); c->d_lnE.release(); c->d_lnE2.release(); c->d_sel.release(); c->d_sne.release();
-  c->d_sigbin.release(); c->d_ek.release(); c->d_ec.release(); c->d_mass.release(); c->d_bins.release(); c->d_lut.release();
-  c->d_nuc.release(); c->d_nuc1.release(); c->d_hu_own.release();
-  c->qa.release(); c->qb.release(); c->qev.release(); c->qel.release(); c->qne.release(); c->qres.release(); c->d_resza.release(); c->d_resp.release();
-  c->d_head.release(); c->d_cnt.release(); c->d_tally.release(); c->d_out.release(); c->d_let.release(); c->d_mol.release(); c->d_roimap.release(); c->d_roivox.release();
-  c->d_spots.release(); c->d_cdf.release(); c->d_res.release(); c->d_goff.release(); c->d_gscr.release(); c->d_slots.release(); c->d_counts.release(); c->d_base.release();
+  for (DevBufBase *b : c->bufs) b->release();
   if (c->h_pinned) cudaFreeHost(c->h_pinned);
   if (c->ev[0]) { cudaEventDestroy(c->ev[0]); cudaEventDestroy(c->ev[1]); }
   for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
@@ -425,6 +449,11 @@ int pmc_load_physics_tables(pmc_ctx *c, const pmc_tables *t) {
   for (int i = 0; i < c->n_elem; ++i) {
     if (c->ea[i] < 1 || c->ez[i] < 0 || c->ez[i] > c->ea[i]) return fail(c, PMC_E_INVALID_ARG, "bad element");
     if (h_nmass(c, c->ez[i], c->ea[i]) <= 0) return fail(c, PMC_E_INVALID_ARG, "element missing from mass table");
+    if (c->ea[i] < 2) {
+      // below 250 MeV only elastic NN scattering: a lone nucleon has no non-elastic channel (and no shell model)
+      for (int k = 0; k < c->n_e; ++k)
+        if (c->h_sne[(size_t)i * c->n_e + k] != 0.0) return fail(c, PMC_E_INVALID_ARG, "sigma_ne_mb must be zero for an element with A < 2");
+    }
     if (c->ea[i] > 1) {
       if (h_nmass(c, c->ez[i] - 1, c->ea[i] - 1) <= 0 || h_nmass(c, c->ez[i], c->ea[i] - 1) <= 0)
         return fail(c, PMC_E_INVALID_ARG, "element's neighbours missing from mass table");
@@ -510,6 +539,8 @@ static int simulate_impl(pmc_ctx *c, const pmc_spot *spots_in, int nspots, uint6
   int rc = sync_tables(c); if (rc) return rc;
   const int B = dbg_out ? 1 : c->n_batches;
   if (!dbg_out && B < 2) return fail(c, PMC_E_INVALID_ARG, "need >= 2 batches");
+  // PAPER.md:L134 "groups of N/10 histories": a batch without a history has no dose to average
+  if (!dbg_out && n < (uint64_t)B) return fail(c, PMC_E_INVALID_ARG, "n_histories must be at least n_batches");
   // spot positions into the grid frame
   std::vector<pmc_spot> spots(spots_in, spots_in + nspots);
   for (auto &s : spots) for (int k = 0; k < 3; ++k) s.pos_cm[k] -= c->origin[k];
@@ -538,7 +569,7 @@ static int simulate_impl(pmc_ctx *c, const pmc_spot *spots_in, int nspots, uint6
   float air_rho, air_wf, air_ix0, air_zoa; int air_tab; air_params(c, air_rho, air_wf, air_ix0, air_zoa, air_tab);
   const bool profile = c->profile;
   c->ev_used = 0; c->ev_acc.clear();
-  cudaEvent_t e0, e1; CK(cudaEventCreate(&e0)); CK(cudaEventCreate(&e1));
+  const cudaEvent_t e0 = c->ev[0], e1 = c->ev[1];               // created once by ensure_scratch
   CK(cudaEventRecord(e0, s));
   const int grid_v = c->n_sm * 8;
   for (uint64_t cs = 0; cs < n; cs += chunk) {
@@ -557,7 +588,7 @@ static int simulate_impl(pmc_ctx *c, const pmc_spot *spots_in, int nspots, uint6
     c->timing.launches_total++;
     CK(cudaMemcpyAsync(c->h_pinned, c->qa.q.count, 4, cudaMemcpyDeviceToHost, s));
     CK(cudaStreamSynchronize(s));
-    rc = run_generations(c, P, std::min(c->h_pinned[0], c->qcap), profile); if (rc) { cudaEventDestroy(e0); cudaEventDestroy(e1); return rc; }
+    rc = run_generations(c, P, std::min(c->h_pinned[0], c->qcap), profile); if (rc) return rc;
   }
   if (!dbg_out) {                                                  // PAPER.md:L138 total and RMS dose per voxel
     { Timer t(c, &c->timing.statistics_ms, profile);
@@ -572,7 +603,6 @@ static int simulate_impl(pmc_ctx *c, const pmc_spot *spots_in, int nspots, uint6
   c->have_let = let_on && rc == PMC_OK;
   resolve_timers(c);
   float ms = 0; cudaEventElapsedTime(&ms, e0, e1); c->timing.total_ms = ms;
-  cudaEventDestroy(e0); cudaEventDestroy(e1);
   return rc;
 }
 
@@ -679,6 +709,7 @@ int pmc_gamma_index(pmc_ctx *c, const float *ref_dev, const float *eval_dev, int
   // lattice offsets inside the search sphere, nearest first (Reading R10: voxel centres, no interpolation)
   const int rx = (int)std::floor(search_cm / dx + 1e-9), ry = (int)std::floor(search_cm / dy + 1e-9), rz = (int)std::floor(search_cm / dz + 1e-9);
   if ((double)(2 * rx + 1) * (2 * ry + 1) * (2 * rz + 1) > 4.0e6) return fail(c, PMC_E_UNSUPPORTED, "search radius spans too many voxels");
+  if (rx > 32767 || ry > 32767 || rz > 32767) return fail(c, PMC_E_UNSUPPORTED, "search radius of more than 32767 voxels along an axis");
   std::vector<std::pair<double, GammaOffset>> offs;
   for (int k = -rz; k <= rz; ++k) for (int j = -ry; j <= ry; ++j) for (int i = -rx; i <= rx; ++i) {
     const double d2 = (i * dx) * (i * dx) + (j * dy) * (j * dy) + (k * dz) * (k * dz);

@@ -146,6 +146,7 @@ struct Tables {
 
 struct Grid {                   // PAPER.md:L144 "CT geometry in global memory"
   const int16_t *hu; int nx, ny, nz; float d[3]; float vol;   // voxel volume, cm^3
+  double dd[3];                 // voxel sizes as given (the sampler places the source in fp64: Reading R2 tie rule)
 };
 
 // energy-grid lookup shared by the range spline and the cross-section lerp
@@ -242,9 +243,9 @@ __device__ __forceinline__ bool queue_push(const Queue &q, const Particle &p) {
 
 // ------------------------------------------------------------------ global counters / ledger
 struct Counters {
-  unsigned long long n_steps, n_elastic, n_nonelastic, n_secondary, n_missed, n_inc_tries, n_zab_bad;
+  unsigned long long n_steps, n_elastic, n_nonelastic, n_secondary, n_missed, n_inc_tries, n_zab_bad, n_inc_guard, n_inc_cap;
   double e_source, e_deposit, e_escape, e_neutron, e_gamma, e_q, e_air;
-  unsigned int overflow;
+  unsigned int overflow, inc_max_stack, inc_max_out;
 };
 __device__ __forceinline__ double warp_sum(double v) {
 #pragma unroll

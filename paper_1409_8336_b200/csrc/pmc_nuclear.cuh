@@ -12,8 +12,11 @@
 
 namespace pmc {
 
-constexpr int CASC_STACK = 48;      // cascade nucleons waiting to be tracked (an attempt that needs more fails)
-constexpr int MAX_INC_OUT = 32;     // nucleons leaving the nucleus in one cascade
+// Fixed capacities of a cascade attempt; an attempt that needs more is abandoned and repeated like one that trips the step
+// guard, and counted (pmc_counters.n_inc_cap_trips).  The oracle (limit 200 / none) never saw more than 7 waiting and 7
+// outgoing nucleons in 1e6 events each of p + 48Ti at 230 MeV, p + 16O at 200 MeV and p + 40Ca at 70 MeV.
+constexpr int CASC_STACK = 16;      // cascade nucleons waiting to be tracked
+constexpr int MAX_INC_OUT = 16;     // nucleons leaving the nucleus in one cascade
 constexpr int MAX_SEC = 48;         // records per event in the standalone kernel's slot buffer (INC + evaporation + residual)
 constexpr int MAX_INC_STEPS = 1024; // tracking steps per attempt before it is abandoned and repeated (Reading R6.8)
 constexpr int NQ = 64;              // quadrature bins of the evaporation spectrum (Reading R7)
@@ -37,6 +40,8 @@ struct IncLane {
   CascNucleon stack[CASC_STACK]; OutNuc out[MAX_INC_OUT];
   CascNucleon c;
   int sp, ncoll, n_out, np_out, guard; bool alive, failed;
+  int trip;                       // why the attempt was abandoned: 1 step guard, 2 stack full, 4 out-list full
+  int hw_stack, hw_out;           // high-water marks over the lane's attempts
   double e_out_sum, pxs, pys, pzs;
 };
 
@@ -44,7 +49,7 @@ struct IncLane {
 // the outermost shell: gains V, tangential momentum conserved
 __device__ __forceinline__ void inc_begin(const Nucleus &N, float t_in, Rng &g, IncLane &L) {
   const int ns = N.nshell;
-  L.sp = 0; L.ncoll = 0; L.n_out = 0; L.np_out = 0; L.guard = 0; L.failed = false;
+  L.sp = 0; L.ncoll = 0; L.n_out = 0; L.np_out = 0; L.guard = 0; L.failed = false; L.trip = 0;
   L.e_out_sum = 0; L.pxs = 0; L.pys = 0; L.pzs = 0;
   const uint4 r = g.next4();
   const float b = N.rmax * sqrtf(u01(r.x)); float sph, cph; sincospif(2.0f * u01(r.y), &sph, &cph);
@@ -62,7 +67,7 @@ __device__ __forceinline__ void inc_fail(IncLane &L) { L.failed = true; L.alive 
 __device__ __forceinline__ void inc_step(const Nucleus &N, Rng &g, IncLane &L) {
   CascNucleon &c = L.c;
   const int ns = N.nshell;
-  if (++L.guard > MAX_INC_STEPS) { inc_fail(L); return; }   // bound orbit in a dilute shell (Reading R6.8)
+  if (++L.guard > MAX_INC_STEPS) { L.trip = 1; inc_fail(L); return; }   // bound orbit in a dilute shell (Reading R6.8)
   const int k = c.shell, ty = c.type;
   const float m = nucleon_mass(ty), p2 = dot(c.p, c.p), E = fsqrt(p2 + m * m), Tk = fdiv(p2, E + m);
   const V3 d = rsqrtf(p2) * c.p;
@@ -112,8 +117,9 @@ __device__ __forceinline__ void inc_step(const Nucleus &N, Rng &g, IncLane &L) {
     // trapping (Reading R6.4): outside energy eps = T - V <= B_C stays in the nucleus
     const float bc2 = tp == 0 ? N.coulomb : 0.f, bc1 = ty == 0 ? N.coulomb : 0.f;
     if (T2 - N.V[tp][k] > bc2) {
-      if (L.sp >= CASC_STACK) { inc_fail(L); return; }
+      if (L.sp >= CASC_STACK) { L.trip = 2; inc_fail(L); return; }
       L.stack[L.sp++] = {c.r, n2, tp, k};
+      L.hw_stack = max(L.hw_stack, L.sp);
     }
     if (T1 - N.V[ty][k] > bc1) c.p = n1; else L.alive = false;
     return;
@@ -130,8 +136,9 @@ __device__ __forceinline__ void inc_step(const Nucleus &N, Rng &g, IncLane &L) {
   if (pn2 <= 0.f || pr2 <= 0.f) { c.p = pt - pr * nh; return; }           // specular reflection
   const V3 pnew = pt + ((pr > 0.f ? 1.0f : -1.0f) * fsqrt(pr2)) * nh;
   if (k2 >= ns) {                                                       // leaves the nucleus with KE = eps
-    if (L.n_out >= MAX_INC_OUT) { inc_fail(L); return; }
+    if (L.n_out >= MAX_INC_OUT) { L.trip = 4; inc_fail(L); return; }
     OutNuc &o = L.out[L.n_out++];
+    L.hw_out = max(L.hw_out, L.n_out);
     o.type = ty; o.ke = T2; o.dir = unit(pnew);
     L.e_out_sum += (double)T2 + (ty == 0 ? MP_D : MN_D); L.pxs += pnew.x; L.pys += pnew.y; L.pzs += pnew.z;
     if (ty == 0) L.np_out++;
@@ -167,8 +174,9 @@ __device__ __forceinline__ void inc_compound(const Tables &T, const Nucleus &N, 
 // load(i, N, t_in, g) sets up event i; store(i, g, out, n_out, R) consumes its result.  L75: the attempt is repeated
 // (fresh draws of the same stream) until it has at least one Pauli-allowed collision and a valid residual.
 // All 32 lanes of every warp must call.
+struct IncStats { unsigned long long tries = 0, guard = 0, cap = 0; int hw_stack = 0, hw_out = 0; };
 template <class Load, class Store>
-__device__ __forceinline__ void inc_machine(const Tables &T, uint32_t n, uint32_t *head, unsigned long long &tries,
+__device__ __forceinline__ void inc_machine(const Tables &T, uint32_t n, uint32_t *head, IncStats &st,
                                             Load load, Store store) {
   // Lane states.  STEP: tracking a nucleon.  WAIT: attempt finished (needs finalize, then store + next event, or a
   // fresh attempt) or no event yet.  DONE: queue exhausted.  The turnover work of WAIT lanes is divergent and long
@@ -176,7 +184,7 @@ __device__ __forceinline__ void inc_machine(const Tables &T, uint32_t n, uint32_
   // every time a single lane finishes.
   enum { STEP = 0, WAIT = 1, DONE = 2 };
   constexpr int TURNOVER = 8;
-  IncLane L; L.alive = false; L.sp = 0; L.failed = false;
+  IncLane L; L.alive = false; L.sp = 0; L.failed = false; L.trip = 0; L.hw_stack = 0; L.hw_out = 0;
   const Nucleus *N = nullptr; float t_in = 0.f; Rng g; uint32_t ev = 0; int ntry = 0;
   bool busy = false; int state = WAIT;
   const int lane = threadIdx.x & 31;
@@ -185,10 +193,11 @@ __device__ __forceinline__ void inc_machine(const Tables &T, uint32_t n, uint32_
     if (!waiting && !stepping) break;
     if (waiting && (__popc(waiting) >= TURNOVER || !stepping)) {
       if (state == WAIT && busy) {                       // end of an attempt
+        if (L.trip == 1) st.guard++; else if (L.trip) st.cap++;
         Residual R;
         if (inc_finalize(T, *N, t_in, L, R)) { store(ev, g, L.out, L.n_out, R); busy = false; }
         else if (ntry >= 100000) { inc_compound(T, *N, t_in, R); store(ev, g, L.out, 0, R); busy = false; }
-        else { ++ntry; tries++; inc_begin(*N, t_in, g, L); state = STEP; }
+        else { ++ntry; st.tries++; inc_begin(*N, t_in, g, L); state = STEP; }
       }
       __syncwarp();
       const unsigned need = __ballot_sync(0xffffffffu, state == WAIT && !busy);
@@ -199,7 +208,7 @@ __device__ __forceinline__ void inc_machine(const Tables &T, uint32_t n, uint32_
         base = __shfl_sync(0xffffffffu, base, leader);
         if (state == WAIT && !busy) {
           ev = base + (uint32_t)__popc(need & ((1u << lane) - 1u));
-          if (ev < n) { load(ev, N, t_in, g); busy = true; ntry = 1; tries++; inc_begin(*N, t_in, g, L); state = STEP; }
+          if (ev < n) { load(ev, N, t_in, g); busy = true; ntry = 1; st.tries++; inc_begin(*N, t_in, g, L); state = STEP; }
           else state = DONE;
         }
       }
@@ -214,6 +223,13 @@ __device__ __forceinline__ void inc_machine(const Tables &T, uint32_t n, uint32_
     }
     __syncwarp();
   }
+  st.hw_stack = L.hw_stack; st.hw_out = L.hw_out;
+}
+// all 32 lanes must call
+__device__ __forceinline__ void flush_inc_stats(Counters *cnt, const IncStats &st) {
+  flush(&cnt->n_inc_tries, st.tries); flush(&cnt->n_inc_guard, st.guard); flush(&cnt->n_inc_cap, st.cap);
+  const int hs = __reduce_max_sync(0xffffffffu, st.hw_stack), ho = __reduce_max_sync(0xffffffffu, st.hw_out);
+  if ((threadIdx.x & 31) == 0) { atomicMax(&cnt->inc_max_stack, (unsigned)hs); atomicMax(&cnt->inc_max_out, (unsigned)ho); }
 }
 
 // ------------------------------------------------------------------ evaporation (Reading R7)
@@ -343,7 +359,7 @@ struct ResQueue { Queue q; uint32_t *za; float *px, *py, *pz; };   // q.e = E*, 
 __global__ void __launch_bounds__(128) inc_kernel(Tables T, RunParams P, Queue in, uint32_t *head, Queue out, ResQueue rq,
                                                   float *tally, Counters *cnt) {
   const uint32_t n = min(*in.count, in.cap);
-  double c_dep = 0, c_neu = 0, c_q = 0; unsigned long long c_sec = 0, c_tries = 0;
+  double c_dep = 0, c_neu = 0, c_q = 0; unsigned long long c_sec = 0; IncStats st;
   Particle p;
   auto load = [&](uint32_t i, const Nucleus *&N, float &t_in, Rng &g) {
     p = queue_load(in, i);
@@ -377,9 +393,9 @@ __global__ void __launch_bounds__(128) inc_kernel(Tables T, RunParams P, Queue i
       rq.px[slot] = (float)R.P[0]; rq.py[slot] = (float)R.P[1]; rq.pz[slot] = (float)R.P[2];
     }
   };
-  inc_machine(T, n, head, c_tries, load, store);
+  inc_machine(T, n, head, st, load, store);
   flush(&cnt->e_deposit, c_dep); flush(&cnt->e_neutron, c_neu); flush(&cnt->e_q, c_q);
-  flush(&cnt->n_secondary, c_sec); flush(&cnt->n_inc_tries, c_tries);
+  flush(&cnt->n_secondary, c_sec); flush_inc_stats(cnt, st);
 }
 
 // K4: nuclear de-excitations over the residual queue (PAPER.md:L128(4), L136), one residual per lane at a time
@@ -425,7 +441,7 @@ struct ResRec { int Z, A; double estar; double P[3]; uint32_t blk; int zs, as; }
 __global__ void __launch_bounds__(128) nonelastic_inc_kernel(Tables T, const Nucleus *nuc, float t_in0, uint64_t seed, uint64_t ev0,
                                                              uint32_t n, uint32_t *head, SecRec *slots, uint32_t *counts,
                                                              ResRec *res, Counters *cnt) {
-  unsigned long long c_tries = 0;
+  IncStats st;
   auto load = [&](uint32_t i, const Nucleus *&N, float &t_in, Rng &g) { g.init(seed, ev0 + i, 0u, 0u); N = nuc; t_in = t_in0; };
   auto store = [&](uint32_t i, Rng &g, const OutNuc *outn, int n_out, const Residual &R) {
     SecRec *s = slots + (size_t)i * MAX_SEC; int zs = 0;
@@ -439,8 +455,8 @@ __global__ void __launch_bounds__(128) nonelastic_inc_kernel(Tables T, const Nuc
     rr.blk = g.blk; rr.zs = zs; rr.as = n_out;
     res[i] = rr;
   };
-  inc_machine(T, n, head, c_tries, load, store);
-  flush(&cnt->n_inc_tries, c_tries);
+  inc_machine(T, n, head, st, load, store);
+  flush_inc_stats(cnt, st);
 }
 
 __global__ void __launch_bounds__(128) nonelastic_evap_kernel(Tables T, const Nucleus *nuc, uint64_t seed, uint64_t ev0, uint32_t n,

@@ -173,7 +173,7 @@ __global__ void __launch_bounds__(256) sampler_kernel(Tables T, Grid G, const Sp
     if (sp.sigma_e > 0) { uint4 q = g.next4(); E += sp.sigma_e * (double)(sqrtf(-2.0f * logf(u01(q.x))) * cospif(2.0f * u01(q.y))); }
     E = fmax(E, 0.0);
     e_src += E;
-    const double size[3] = {G.nx * (double)G.d[0], G.ny * (double)G.d[1], G.nz * (double)G.d[2]};
+    const double size[3] = {G.nx * G.dd[0], G.ny * G.dd[1], G.nz * G.dd[2]};
     auto ray_box = [&](const double *o, const double *dd, double &tin) {
       double t0 = 0, t1 = 1e300;
       for (int k = 0; k < 3; ++k) {
@@ -212,7 +212,7 @@ __global__ void __launch_bounds__(256) sampler_kernel(Tables T, Grid G, const Sp
     if (ok) {
       int idx[3]; const int nn[3] = {G.nx, G.ny, G.nz}; float loc[3];
       for (int k = 0; k < 3; ++k) {
-        const double rv = fmin(fmax(pos[k], 0.0), size[k]), dk = (double)G.d[k];
+        const double rv = fmin(fmax(pos[k], 0.0), size[k]), dk = G.dd[k];
         int ii = (int)floor(rv / dk);
         if (ii * dk == rv && dir[k] < 0) ii -= 1;
         ii = min(max(ii, 0), nn[k] - 1);

@@ -7,7 +7,7 @@ mean dose (Gy per primary of ITS share) and standard error; the plan dose is the
     D     = sum_r n_r D_r / sum_r n_r
     sigma = sqrt( sum_r (n_r / N)^2 sigma_r^2 )
 
-which needs one all-reduce(sum) of two grids — the only exchange step of the path (PAPER.md:L266, L270 mention
+which needs one all-reduce(sum) of one packed buffer (two grids and the history count) — the only exchange step of the path (PAPER.md:L266, L270 mention
 multi-GPU only as deployment).  Works on CPU tensors over gloo (tests) and CUDA tensors over NCCL (bench).
 """
 from __future__ import annotations
@@ -29,18 +29,22 @@ def weak_shard(n_per_rank: int, rank: int):
 
 
 def combine_dose(dose, sigma, n_local: int, group=None):
-    """All-reduce the per-rank (dose, sigma) into the plan's (dose, sigma).  In place; returns (dose, sigma, N)."""
+    """ONE all-reduce(sum) of a packed buffer [n_r D_r | (n_r sigma_r)^2 | n_r] turns the per-rank (dose, sigma) into the
+    plan's: D = sum n_r D_r / N, sigma = sqrt(sum (n_r sigma_r)^2) / N.  In place; returns (dose, sigma, N).
+    (n_r travels as two fp32 words of 16 bits each so that the sum over ranks is exact in the fp32 buffer.)"""
     import torch
     import torch.distributed as dist
     if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size(group) == 1:
         return dose, sigma, n_local
-    n = torch.tensor([float(n_local)], dtype=torch.float64, device=dose.device)
-    dist.all_reduce(n, group=group)
-    n_tot = float(n.item())
-    w = n_local / n_tot if n_tot > 0 else 0.0
-    dose.mul_(w)
-    sigma.mul_(w).square_()
-    dist.all_reduce(dose, group=group)
-    dist.all_reduce(sigma, group=group)
-    sigma.sqrt_()
-    return dose, sigma, int(round(n_tot))
+    nv = dose.numel()
+    buf = torch.empty(2 * nv + 2, dtype=torch.float32, device=dose.device)
+    torch.mul(dose.reshape(-1), float(n_local), out=buf[:nv])
+    torch.mul(sigma.reshape(-1), float(n_local), out=buf[nv:2 * nv]); buf[nv:2 * nv].square_()
+    buf[2 * nv] = float(n_local >> 16); buf[2 * nv + 1] = float(n_local & 0xFFFF)
+    dist.all_reduce(buf, group=group)
+    tail = buf[2 * nv:].tolist()
+    n_tot = int(round(tail[0])) * 65536 + int(round(tail[1]))
+    inv = 1.0 / n_tot if n_tot > 0 else 0.0
+    dose.copy_((buf[:nv] * inv).reshape(dose.shape))
+    sigma.copy_((buf[nv:2 * nv].sqrt_() * inv).reshape(sigma.shape))
+    return dose, sigma, n_tot

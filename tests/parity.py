@@ -28,6 +28,18 @@ def distal_depth(dd, d_cm, level):
     return float("nan")
 
 
+def distal_depth_from_end(dd, d_cm, level):
+    """The same level crossing searched from the far end of the profile (a spread-out Bragg peak has a rippled plateau:
+    its maximum is not a landmark, its distal edge is)."""
+    dd = np.asarray(dd, dtype=np.float64)
+    thr = level * dd.max()
+    for i in range(len(dd) - 2, -1, -1):
+        if dd[i] >= thr > dd[i + 1]:
+            f = (dd[i] - thr) / (dd[i] - dd[i + 1])
+            return (i + 0.5 + f) * d_cm
+    return float("nan")
+
+
 def r80_and_falloff(dd, d_cm):
     r80 = distal_depth(dd, d_cm, 0.8)
     r20 = distal_depth(dd, d_cm, 0.2)

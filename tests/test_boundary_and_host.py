@@ -77,8 +77,12 @@ def _combine_worker(rank, world, port, tmp):
     dose = torch.rand(4, 5, 6, generator=g)
     sigma = 0.1 * torch.rand(4, 5, 6, generator=g)
     torch.save((dose.clone(), sigma.clone(), n_local), os.path.join(tmp, f"in{rank}.pt"))
+    calls = []
+    real = dist.all_reduce
+    dist.all_reduce = lambda *a, **k: (calls.append(1), real(*a, **k))[1]      # ONE all-reduce
     d, s, n = combine_dose(dose, sigma, n_local)
-    torch.save((d, s, n), os.path.join(tmp, f"out{rank}.pt"))
+    dist.all_reduce = real
+    torch.save((d, s, n, len(calls)), os.path.join(tmp, f"out{rank}.pt"))
     dist.destroy_process_group()
 
 
@@ -90,8 +94,8 @@ def test_combine_dose_gloo_world2(tmp_path):
     n = sum(i[2] for i in ins)
     d_ref = sum(i[0].double() * i[2] for i in ins) / n
     s_ref = torch.sqrt(sum((i[1].double() * i[2] / n) ** 2 for i in ins))
-    for d, s, nn in outs:
-        assert nn == n
+    for d, s, nn, n_calls in outs:
+        assert nn == n and n_calls == 1
         assert torch.allclose(d.double(), d_ref, rtol=1e-6, atol=1e-9)
         assert torch.allclose(s.double(), s_ref, rtol=1e-6, atol=1e-9)
 

@@ -167,6 +167,10 @@ def test_nonelastic_c2_yields_spectra_angles(pm, oracle_c1, tables, Z, A, ie, e_
     so, oo = oracle_c1.nonelastic(Z, A, e_mev, n, seed + 5)
     # exact integers: charge and baryon number of every event (bit-exact bar)
     assert cg["n_zab_violations"] == 0
+    # Reading R6.8: the step guard and the fixed capacities of the CUDA cascade (16 waiting / 16 outgoing nucleons) end
+    # fewer than 1e-5 of the attempts, and the depth actually reached is the oracle's (7 in 1e6 events), far below them
+    assert cg["n_inc_guard_trips"] + cg["n_inc_cap_trips"] <= max(1, 2e-5 * cg["n_inc_tries"]), cg
+    assert 2 <= cg["inc_max_stack"] <= 10 and 2 <= cg["inc_max_out"] <= 10, cg
     zs = np.add.reduceat(sg["Z"].astype(np.int64), og[:-1]); as_ = np.add.reduceat(sg["A"].astype(np.int64), og[:-1])
     assert np.all(zs == Z + 1) and np.all(as_ == A + 1)
     assert og[0] == 0 and og[-1] == len(sg) and np.all(np.diff(og.astype(np.int64)) >= 2)
@@ -227,13 +231,26 @@ def _ledger_closes(c, rel=2e-4):
     return abs(sinks / c["e_source"] - 1) < rel
 
 
-def _dose_parity(pm, o, w_hu, vox, mats, spots, n, seed, axis=0, check_range=True, min_pass=0.99):
-    """north_star's dose tolerances between pmc_simulate and the oracle on the same inputs."""
-    dg, sg = pm.simulate(spots, n, seed)
-    cg = pm.counters()
-    dg, sg = dg.cpu().numpy().astype(np.float64), sg.cpu().numpy().astype(np.float64)
-    do, so = o.simulate(spots, n, seed)
-    co = o.counters()
+# The z statistic (D_gpu - D_oracle)/sqrt(sigma_g^2 + sigma_o^2) with both sigmas estimated from B batches is t-like: with
+# B = 10 only 99.25 % of the voxels fall within 3 under PERFECT parity (99.66 % with 50 batches), and the
+# pass fraction over nv voxels scatters binomially around that.  north_star's ">= 99 %" is therefore asserted literally
+# with B = 40 batches on both sides (SURVEY's own remedy: "keep B a run-time option"), and where a configuration fixes
+# B = 10 the bound is the expectation minus three binomial sigmas (voxels that share histories count as one in eight).
+def low_stat_bound(nv, expect=0.9925):
+    return expect - 3.0 * np.sqrt(expect * (1 - expect) / max(nv / 8.0, 1.0))
+
+
+def _dose_parity(pm, o, w_hu, vox, mats, spots, n, seed, axis=0, check_range=True, min_pass=0.99, batches=40, seed_o=None):
+    """north_star's dose tolerances between pmc_simulate and the oracle on the same inputs (B batches on both sides)."""
+    pm.set_option("n_batches", float(batches)); o.set_option("n_batches", float(batches))
+    try:
+        dg, sg = pm.simulate(spots, n, seed)
+        cg = pm.counters()
+        dg, sg = dg.cpu().numpy().astype(np.float64), sg.cpu().numpy().astype(np.float64)
+        do, so = o.simulate(spots, n, seed if seed_o is None else seed_o)
+        co = o.counters()
+    finally:
+        pm.set_option("n_batches", 10.0); o.set_option("n_batches", 10.0)
     assert np.all(np.isfinite(dg)) and np.all(dg >= 0) and np.all(sg >= 0)
     # integrated dose (= deposited energy per history) within 0.5 %
     rho = _density(w_hu, mats)
@@ -244,6 +261,9 @@ def _dose_parity(pm, o, w_hu, vox, mats, spots, n, seed, axis=0, check_range=Tru
     assert _ledger_closes(cg), cg
     # >= 99 % of voxels above 10 % of the maximum within 3 combined sigma
     frac, zmean, zrms, nv = parity.zscore_pass(dg, sg, do, so)
+    if min_pass is None:
+        min_pass = low_stat_bound(nv)
+    print(f"z-pass {frac:.4f} (bound {min_pass:.4f}) mean z {zmean:+.3f} rms z {zrms:.3f} voxels {nv} B {batches} n {n}")
     assert nv > 20 and frac >= min_pass, (frac, zmean, zrms, nv)
     assert abs(zmean) < 0.25 and zrms < 1.5, (zmean, zrms)
     # R80 and distal fall-off within 0.2 mm
@@ -273,28 +293,30 @@ def _density(hu, mats):
 
 
 def test_c1_water_phantom_as_configured(pm, tables):
+    """C1 exactly as BASELINE.json configures it (1e4 histories, seed 1, 10 batches): bound of SURVEY 8(c).8 at B = 10; the
+    same 1e4 histories with 40 batches: north_star's literal 99 %."""
     w = inputs.workload("c1")                                             # 1e4 histories, seed 1, full physics
     o = _setup(pm, tables, w["materials"], w["hu"], w["vox"])
-    _dose_parity(pm, o, w["hu"], w["vox"], w["materials"], w["spots"], w["n_histories"], w["seed"], min_pass=0.985)
+    _dose_parity(pm, o, w["hu"], w["vox"], w["materials"], w["spots"], w["n_histories"], w["seed"], min_pass=None, batches=10)
+    _dose_parity(pm, o, w["hu"], w["vox"], w["materials"], w["spots"], w["n_histories"], w["seed"])
+
+
+def _lateral_width(d, k):
+    p = d[k - 5:k + 1].sum(axis=(0, 1)); x = np.arange(len(p))
+    return np.sqrt((p * (x - (p * x).sum() / p.sum()) ** 2).sum() / p.sum())
 
 
 def test_c1_water_phantom_high_statistics(pm, tables):
+    """C1 at 3e6 histories (the paper's own pencil-beam statistics are 2.6e6), 30 batches, different seeds
+    on the two sides: every north_star tolerance at once, plus the lateral width at the Bragg peak (MCS + nuclear halo)
+    and the ledgers."""
     w = inputs.workload("c1")
     o = _setup(pm, tables, w["materials"], w["hu"], w["vox"])
-    # 40 batches: with 10-batch sigmas on both sides the z statistic is t-like and only 99.25 % of voxels fall within
-    # 3 under perfect parity; B is a run-time option on both sides
-    pm.set_option("n_batches", 40.0); o.set_option("n_batches", 40.0)
-    try:
-        dg, sg, do, so, cg, co = _dose_parity(pm, o, w["hu"], w["vox"], w["materials"], w["spots"], 400_000, 11)
-    finally:
-        pm.set_option("n_batches", 10.0)
-    # lateral profile at the Bragg peak: MCS + nuclear halo
+    dg, sg, do, so, cg, co = _dose_parity(pm, o, w["hu"], w["vox"], w["materials"], w["spots"], 3_000_000, 11, batches=30, seed_o=12)
     k = int(np.argmax(do.sum(axis=(1, 2))))
-    pg, po = dg[k - 5:k + 1].sum(axis=(0, 1)), do[k - 5:k + 1].sum(axis=(0, 1))
-    x = np.arange(len(po))
-    wg = np.sqrt((pg * (x - (pg * x).sum() / pg.sum()) ** 2).sum() / pg.sum())
-    wo = np.sqrt((po * (x - (po * x).sum() / po.sum()) ** 2).sum() / po.sum())
-    assert abs(wg / wo - 1) < 0.01
+    assert abs(_lateral_width(dg, k) / _lateral_width(do, k) - 1) < 3e-3
+    for key in ("e_neutron", "e_gamma", "e_q", "e_escape"):
+        assert abs(cg[key] / co[key] - 1) < 0.01, (key, cg[key], co[key])
 
 
 @pytest.mark.parametrize("switches", [dict(straggling=0, mcs=0, elastic=0, nonelastic=0),
@@ -302,16 +324,47 @@ def test_c1_water_phantom_high_statistics(pm, tables):
 def test_c1_physics_switches(pm, tables, switches):
     w = inputs.workload("c1")
     o = _setup(pm, tables, w["materials"], w["hu"], w["vox"], **switches)
-    _dose_parity(pm, o, w["hu"], w["vox"], w["materials"], w["spots"], 100_000, 21, min_pass=0.985)
+    _dose_parity(pm, o, w["hu"], w["vox"], w["materials"], w["spots"], 100_000, 21)
 
 
-@pytest.mark.parametrize("name,n", [("c3_70", 100_000), ("c3_150", 100_000), ("c3_230", 60_000)])
-def test_c3_slab_phantom(pm, tables, name, n):
+def test_pencil_on_a_voxel_edge(pm, tables):
+    """A zero-width pencil aimed exactly at the common edge of four voxel columns (x = y = 5.0 cm on the 2 mm grid).  Which of
+    the four voxels a start point on a face belongs to is decided by each side's own arithmetic (the oracle divides by
+    0.2 in fp64, the sampler by float(0.2)); Reading R3.8 makes that immaterial: a proton that is deflected away from its
+    voxel crosses the face in a zero-length boundary step.  So the dose must agree like anywhere else, and be symmetric
+    about the edge on both sides."""
+    w = inputs.workload("c1")
+    o = _setup(pm, tables, w["materials"], w["hu"], w["vox"])
+    spot = inputs.plan_single_spot((5.0, 5.0, 0.0), 150.0, 0.0)
+    dg, sg, do, so, cg, co = _dose_parity(pm, o, w["hu"], w["vox"], w["materials"], spot, 400_000, 61, seed_o=62)
+    # Every step scores in the voxel it starts in, so the voxel that owns the start point collects the first legs of all
+    # the protons and its column gets more than its three neighbours: an artefact of any class II scheme for a pencil of
+    # zero width, identical on both sides because both use the same tie rule (the start point belongs to the upper voxel,
+    # fp64 on both sides).  What must hold: the excess is the same, and the x <-> y mirror pair is equal.
+    ratio = []
+    for d, s_ in ((dg, sg), (do, so)):
+        col = d[:70].sum(axis=0); err = np.sqrt((s_[:70] ** 2).sum(axis=0))
+        assert abs(col[24, 25] - col[25, 24]) < 4.5 * np.hypot(err[24, 25], err[25, 24]), (col[24, 25], col[25, 24])
+        ratio.append((col[25, 25] / col[24, 24], col[25, 25] / col[24, 24] * np.hypot(err[25, 25] / col[25, 25], err[24, 24] / col[24, 24])))
+    assert ratio[0][0] > 1.01 and ratio[1][0] > 1.01                       # the owner of the edge is voxel (25, 25) on both sides
+    assert abs(ratio[0][0] - ratio[1][0]) < 4.5 * np.hypot(ratio[0][1], ratio[1][1]), ratio
+    # first steps from the edge: after 30 steps the transverse distribution is symmetric and equal on both sides
+    for k_ in ("elastic", "nonelastic"):
+        pm.set_option(k_, 0.0); o.set_option(k_, 0.0)
+    g = pm.first_steps(spot, 100_000, 5, 30).astype(np.float64); r = o.first_steps(spot, 100_000, 6, 30)
+    for col in (0, 1):
+        assert abs(g[:, col].mean() - 5.0) < 5 * g[:, col].std() / np.sqrt(1e5) and abs(r[:, col].mean() - 5.0) < 5 * r[:, col].std() / np.sqrt(1e5)
+        assert abs(g[:, col].std() / r[:, col].std() - 1) < 0.02
+
+
+@pytest.mark.parametrize("name", ["c3_70", "c3_150", "c3_230"])
+def test_c3_slab_phantom(pm, tables, name):
     w = inputs.workload(name)                                             # full 200x200x300 grid, 24-bin table
     o = _setup(pm, tables, w["materials"], w["hu"], w["vox"])
+    # as configured: 1e6 histories per energy (BASELINE.json C3), other seed on the oracle side
     # 230 MeV leaves the 30 cm slab (SURVEY 8(a)): no Bragg peak inside, so no R80
-    dg, sg, do, so, cg, co = _dose_parity(pm, o, w["hu"], w["vox"], w["materials"], w["spots"], n, w["seed"],
-                                          check_range=(name != "c3_230"), min_pass=0.985)
+    dg, sg, do, so, cg, co = _dose_parity(pm, o, w["hu"], w["vox"], w["materials"], w["spots"], w["n_histories"], w["seed"],
+                                          check_range=(name != "c3_230"), seed_o=w["seed"] + 100)
     if name == "c3_230":
         assert abs(cg["e_escape"] / co["e_escape"] - 1) < 5e-3
     # energy deposited per material class (water / bone / lung / Ti)
@@ -323,43 +376,79 @@ def test_c3_slab_phantom(pm, tables, name, n):
             assert abs(a / b - 1) < 1e-2, (lo, a, b)
 
 
-def test_c4_head_and_neck_full_size_against_oracle_subsample(pm, tables):
-    """C4 at BASELINE's full size (1e7 histories, the configuration bench.py times) on the GPU; the oracle runs a
-    4e5-history subsample of the same plan.  Doses are per primary, so projections and integrals compare directly."""
+def test_c4_head_and_neck_at_full_size_on_both_sides(pm, tables):
+    """north_star's target: C4 with 1e7 histories on the CUDA path AND on the oracle (different seeds), with the stated
+    tolerances: integrated dose 0.5 %, >= 99 % of the voxels above 10 % of the maximum within 3 combined sigma (asserted
+    with 40 batches on both sides; the CUDA path is also run with the configured 10 batches and that pass rate reported
+    and bounded).  Dose to air is left out of the voxel comparison (Reading R8.1 in DESIGN.md: with rho = 0.0012 g/cm3 a
+    voxel of air turns a single stopping proton into a dose a thousand times that of tissue, so the 'maximum dose' of the
+    grid would be set by one such voxel); the pass rate over ALL voxels is computed and bounded as well."""
     w = inputs.workload("c4")
     o = _setup(pm, tables, w["materials"], w["hu"], w["vox"])
-    n_g, n_o = w["n_histories"], 400_000
-    dg, sg = pm.simulate(w["spots"], n_g, w["seed"])
-    cg = pm.counters()
-    dg, sg = dg.cpu().numpy().astype(np.float64), sg.cpu().numpy().astype(np.float64)
-    do, so = o.simulate(w["spots"], n_o, w["seed"] + 1)
-    co = o.counters()
-    assert _ledger_closes(cg) and cg["n_zab_violations"] == 0
-    rho = _density(w["hu"], w["materials"])
-    vol = np.prod(w["vox"])
+    n = w["n_histories"]
+    rho = _density(w["hu"], w["materials"]); vol = np.prod(w["vox"]); tissue = w["hu"] >= -950
+    pm.set_option("n_batches", 40.0); o.set_option("n_batches", 40.0)
+    try:
+        dg, sg = pm.simulate(w["spots"], n, w["seed"]); cg = pm.counters()
+        dg, sg = dg.cpu().numpy().astype(np.float64), sg.cpu().numpy().astype(np.float64)
+        do, so = o.simulate(w["spots"], n, w["seed"] + 1); co = o.counters()
+    finally:
+        pm.set_option("n_batches", 10.0); o.set_option("n_batches", 10.0)
+    d10, s10 = pm.simulate(w["spots"], n, w["seed"])                    # the configured 10 batches, same histories
+    d10, s10 = d10.cpu().numpy().astype(np.float64), s10.cpu().numpy().astype(np.float64)
+    assert _ledger_closes(cg) and cg["n_zab_violations"] == 0 and co["n_zab_violations"] == 0
+    assert np.allclose(d10[tissue], dg[tissue], rtol=3e-4, atol=1e-16)  # the batch split does not change the dose
     eg, eo = (dg * rho).sum() * vol / parity.GY_PER_MEV_G, (do * rho).sum() * vol / parity.GY_PER_MEV_G
-    assert abs(eg / eo - 1) < 5e-3
-    assert abs(eg - cg["e_deposit"] / n_g) < 3e-4 * eg
+    assert abs(eg / eo - 1) < 5e-3 and abs(eg / eo - 1) < 1e-3, (eg, eo)             # integrated dose (0.5 % asked; 0.1 % seen)
+    assert abs(eg - cg["e_deposit"] / n) < 3e-4 * eg
     for k in ("n_steps", "n_elastic", "n_nonelastic", "n_secondary_protons", "n_missed"):
-        a, b = cg[k] / n_g, co[k] / n_o
-        assert abs(a - b) <= 5 * np.sqrt(b / n_o + a / n_g) + 5e-3 * b, (k, a, b)
-    # voxel z-scores: the GPU dose is nearly noise-free at 1e7, the oracle's sigma dominates
-    # (tissue voxels only: in the air bin, rho = 0.0012, one stopping proton is a 1000x dose spike that would set the
-    # "maximum" of a 4e5-history map)
-    frac, zmean, zrms, nv = parity.zscore_pass(dg, sg, do, so, region=w["hu"] >= -950)
-    assert nv > 1000 and frac >= 0.985 and abs(zmean) < 0.15 and zrms < 1.4, (frac, zmean, zrms, nv)
-    # the three 1-D projections of deposited energy
+        a, b = cg[k], co[k]
+        assert abs(a - b) <= 5 * np.sqrt(a + b + 1) + 2e-3 * b, (k, a, b)
+    for k in ("e_neutron", "e_gamma", "e_q", "e_escape", "e_air"):
+        assert abs(cg[k] / co[k] - 1) < 0.01, (k, cg[k], co[k])
+    frac, zmean, zrms, nv = parity.zscore_pass(dg, sg, do, so, region=tissue)
+    f_all, zm_all, zr_all, nv_all = parity.zscore_pass(dg, sg, do, so)
+    f10, zm10, zr10, nv10 = parity.zscore_pass(d10, s10, do, so, region=tissue)
+    print(f"C4 1e7 vs 1e7: tissue z-pass {frac:.4f} (mean {zmean:+.3f} rms {zrms:.3f}, {nv} voxels); all voxels {f_all:.4f} "
+          f"({nv_all}); CUDA path at B = 10: {f10:.4f}; integrated dose ratio - 1 = {eg / eo - 1:+.2e}")
+    assert nv > 30_000 and frac >= 0.99 and abs(zmean) < 0.1 and zrms < 1.15, (frac, zmean, zrms, nv)
+    assert f10 >= 0.99 - 0.003 and f_all >= 0.985, (f10, f_all)
+    # the three 1-D projections of deposited energy, slab by slab
     for ax in range(3):
         pg, po = parity.depth_dose(dg * rho, ax), parity.depth_dose(do * rho, ax)
+        eg_, eo_ = np.sqrt(parity.depth_dose((sg * rho) ** 2, ax)), np.sqrt(parity.depth_dose((so * rho) ** 2, ax))
         m = po > 0.05 * po.max()
-        # noise of the 4e5-history oracle projection scales as 1/sqrt(dose in the slab): ~1 % at the peak slab
-        tol = 0.01 + 0.012 * np.sqrt(po.max() / po[m])
-        assert np.all(np.abs(pg[m] / po[m] - 1) < tol), (ax, np.max(np.abs(pg[m] / po[m] - 1) / tol))
-    # sigma scales as 1/sqrt(N): median relative error in the high-dose region
-    tissue = w["hu"] >= -950
+        assert np.all(np.abs(pg[m] - po[m]) < 5 * np.hypot(eg_[m], eo_[m]) + 2e-3 * po[m]), ax
+    # sigma: same number of histories, same sigma (median relative error in the high-dose region)
     hi = tissue & (do > 0.5 * do[tissue].max())
-    ratio = np.median(sg[hi] / np.maximum(dg[hi], 1e-30)) / np.median(so[hi] / np.maximum(do[hi], 1e-30))
-    assert abs(ratio * np.sqrt(n_g / n_o) - 1) < 0.25
+    assert abs(np.median(sg[hi] / dg[hi]) / np.median(so[hi] / do[hi]) - 1) < 0.05
+
+
+@pytest.mark.parametrize("field", [0, 1, 2])
+def test_c4_range_of_each_field_along_its_own_axis(pm, tables, field):
+    """R80 and distal fall-off (R20 - R80) within 0.2 mm on the integrated depth dose of each of the three C4 fields along
+    its own axis (+x, -x, -y), each field's spots simulated separately with 2e6 histories on both sides.  The distal edge of
+    a multi-layer field is searched from the far end of the profile (its plateau has no usable maximum)."""
+    w = inputs.workload("c4")
+    o = _setup(pm, tables, w["materials"], w["hu"], w["vox"])
+    dirs = np.array([(1.0, 0.0, 0.0), (-1.0, 0.0, 0.0), (0.0, -1.0, 0.0)])
+    sel = np.all(np.abs(w["spots"][:, 3:6] - dirs[field]) < 1e-9, axis=1)
+    spots = np.ascontiguousarray(w["spots"][sel])
+    assert 300 < len(spots) < 1500
+    n = 2_000_000
+    dg, _ = pm.simulate(spots, n, 400 + field); dg = dg.cpu().numpy().astype(np.float64)
+    do, _ = o.simulate(spots, n, 500 + field)
+    rho = _density(w["hu"], w["materials"])
+    axis = 2 if field < 2 else 1; d_cm = w["vox"][0] if field < 2 else w["vox"][1]
+    pg, po = parity.depth_dose(dg * rho, axis), parity.depth_dose(do * rho, axis)
+    if dirs[field][0 if field < 2 else 1] < 0:
+        pg, po = pg[::-1], po[::-1]
+    assert abs(pg.sum() / po.sum() - 1) < 5e-3
+    r80g, r80o = parity.distal_depth_from_end(pg, d_cm, 0.8), parity.distal_depth_from_end(po, d_cm, 0.8)
+    r20g, r20o = parity.distal_depth_from_end(pg, d_cm, 0.2), parity.distal_depth_from_end(po, d_cm, 0.2)
+    print(f"C4 field {field}: R80 {r80g:.4f} vs {r80o:.4f} cm, fall-off {10 * (r20g - r80g):.3f} vs {10 * (r20o - r80o):.3f} mm")
+    assert np.isfinite([r80g, r80o, r20g, r20o]).all()
+    assert abs(r80g - r80o) < 0.02 and abs((r20g - r80g) - (r20o - r80o)) < 0.02
 
 
 def test_c4_two_seeds_eq5_and_gamma(pm, tables):
@@ -384,15 +473,20 @@ def test_c4_two_seeds_eq5_and_gamma(pm, tables):
 
 def test_c5_pelvis_full_size_against_oracle_subsample(pm, tables):
     """C5 (512x512x200 pelvis with Ti implants, 11033 spots, 100-230 MeV) at BASELINE's full 1e8 histories on the GPU
-    (6 sub-groups of 2^24 histories, 2.1 GB of per-batch tallies); the oracle runs a 5e5-history subsample."""
+    (6 sub-groups of 2^24 histories); the oracle runs the 1e6-history subsample SURVEY 8(d) assigns to this throughput
+    configuration.  40 batches on both sides for the voxel comparison (see low_stat_bound above)."""
     w = inputs.workload("c5")
     o = _setup(pm, tables, w["materials"], w["hu"], w["vox"])
-    n_g, n_o = w["n_histories"], 500_000
-    dg, sg = pm.simulate(w["spots"], n_g, w["seed"])
-    cg = pm.counters()
-    dg, sg = dg.cpu().numpy().astype(np.float64), sg.cpu().numpy().astype(np.float64)
-    do, so = o.simulate(w["spots"], n_o, w["seed"] + 1)
-    co = o.counters()
+    n_g, n_o = w["n_histories"], 1_000_000
+    pm.set_option("n_batches", 40.0); o.set_option("n_batches", 40.0)
+    try:
+        dg, sg = pm.simulate(w["spots"], n_g, w["seed"])
+        cg = pm.counters()
+        dg, sg = dg.cpu().numpy().astype(np.float64), sg.cpu().numpy().astype(np.float64)
+        do, so = o.simulate(w["spots"], n_o, w["seed"] + 1)
+        co = o.counters()
+    finally:
+        pm.set_option("n_batches", 10.0); o.set_option("n_batches", 10.0)
     assert _ledger_closes(cg) and cg["n_zab_violations"] == 0 and np.all(np.isfinite(dg)) and np.all(sg >= 0)
     rho = _density(w["hu"], w["materials"])
     vol = np.prod(w["vox"])
@@ -406,11 +500,10 @@ def test_c5_pelvis_full_size_against_oracle_subsample(pm, tables):
     ti = w["hu"] >= 3060
     a, b = (dg * rho)[ti].sum(), (do * rho)[ti].sum()
     assert b > 0 and abs(a / b - 1) < 0.03, (a, b)
-    # voxel z-scores in tissue and bone (not air, see C4); few oracle histories per voxel: the 10-batch sigma of a
-    # skewed voxel dose correlates with the dose itself, which pushes the mean z up and fattens the tails (measured: the
-    # 1e8-history map against a 5e5-history run of the CUDA path ITSELF gives 98.2 %, mean z 0.13, rms z 1.16)
+    # voxel z-scores in tissue and bone (not air, Reading R8.1)
     frac, zmean, zrms, nv = parity.zscore_pass(dg, sg, do, so, region=w["hu"] >= -950)
-    assert nv > 100_000 and frac >= 0.975 and abs(zmean) < 0.2 and zrms < 1.3, (frac, zmean, zrms, nv)
+    print(f"C5 1e8 vs oracle 1e6: z-pass {frac:.4f} mean z {zmean:+.3f} rms z {zrms:.3f} voxels {nv}")
+    assert nv > 100_000 and frac >= 0.99 and abs(zmean) < 0.2 and zrms < 1.3, (frac, zmean, zrms, nv)
     for ax in range(3):
         pg, po = parity.depth_dose(dg * rho, ax), parity.depth_dose(do * rho, ax)
         m = po > 0.05 * po.max()
@@ -543,7 +636,7 @@ def test_moliere_option_matches_oracle(pm, tables):
         # full physics on C1 with the Moliere option on both sides
         for k in ("elastic", "nonelastic", "straggling"):
             pm.set_option(k, 1.0); o.set_option(k, 1.0)
-        _dose_parity(pm, o, w["hu"], w["vox"], w["materials"], w["spots"], 100_000, 23, min_pass=0.985)
+        _dose_parity(pm, o, w["hu"], w["vox"], w["materials"], w["spots"], 100_000, 23)
         # without the tables the option is refused
         from paper_1409_8336_b200 import PmcError
     finally:
@@ -565,11 +658,19 @@ def test_simulate_edge_cases(pm, tables):
     assert c["n_missed"] == 1000 and c["n_steps"] == 0 and abs(c["e_escape"] - 150.0 * 1000) < 1e-6
     do, _ = o.simulate(away, 1000, 1)
     assert do.sum() == 0.0 and o.counters()["n_missed"] == 1000
-    # fewer histories than batches; a single history
+    # fewer histories than batches (every group needs its N/10 histories): refused on both sides
     for n in (1, 7):
-        d, s = pm.simulate(w["spots"], n, 3)
-        c = pm.counters()
-        assert _ledger_closes(c) and abs(c["e_source"] - 150.0 * n) < 1e-6 and float(d.sum()) > 0
+        with pytest.raises(PmcError) as e:
+            pm.simulate(w["spots"], n, 3)
+        assert e.value.code == -1
+        with pytest.raises(RuntimeError):
+            o.simulate(w["spots"], n, 3)
+    # one history per batch: the dose grid integrates to the deposited energy per history
+    d, s = pm.simulate(w["spots"], 10, 3)
+    c = pm.counters()
+    assert _ledger_closes(c) and abs(c["e_source"] - 150.0 * 10) < 1e-6
+    e_grid = float(d.double().sum()) * 1.0 * 0.2 ** 3 / parity.GY_PER_MEV_G          # water, rho = 1
+    assert abs(e_grid - c["e_deposit"] / 10) < 2e-4 * e_grid
     # air gap: source 20 cm upstream of the grid
     up = inputs.plan_single_spot((5.0, 5.0, -20.0), 150.0, 0.3)
     d, s = pm.simulate(up, 50_000, 5)
@@ -579,7 +680,7 @@ def test_simulate_edge_cases(pm, tables):
     assert cg["e_air"] > 0 and abs(cg["e_air"] / co["e_air"] - 1) < 0.02 and _ledger_closes(cg)
     # oblique beam entering through a side face
     ob_ = inputs.plan_single_spot((-3.0, 5.0, 6.0), 100.0, 0.3, direction=(0.8, 0.0, 0.6))
-    _dose_parity(pm, o, w["hu"], w["vox"], w["materials"], ob_, 60_000, 8, check_range=False, min_pass=0.98)
+    _dose_parity(pm, o, w["hu"], w["vox"], w["materials"], ob_, 60_000, 8, check_range=False)
     # zero-weight and bad inputs
     bad = w["spots"].copy(); bad[0, 12] = 0.0
     with pytest.raises(PmcError):
@@ -600,7 +701,7 @@ def test_ragged_grid_and_clamped_hu(pm, tables):
     vox = (0.13, 0.21, 0.17)
     o = _setup(pm, tables, mats, hu, vox)
     spot = inputs.plan_single_spot((2.4, 2.3, -1.0), 90.0, 0.25, direction=(0.05, 0.02, 1.0), sigma_e=0.8, div=0.004)
-    dg, sg, do, so, cg, co = _dose_parity(pm, o, hu, vox, mats, spot, 120_000, 17, check_range=False, min_pass=0.98)
+    dg, sg, do, so, cg, co = _dose_parity(pm, o, hu, vox, mats, spot, 120_000, 17, check_range=False)
     rho = _density(hu, mats)
     for sel in (hu == 5000, hu == 1200, hu == -700):
         a, b = (dg * rho)[sel].sum(), (do * rho)[sel].sum()
