@@ -180,6 +180,8 @@ def main():
     ap.add_argument("--workload", default="c4")
     ap.add_argument("--histories", type=int, default=0, help="histories per step and per rank (0 = the workload's)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--option", action="append", default=[], metavar="KEY=VALUE",
+                    help="pmc_set_option before the run (e.g. dose_aggregate=1, dose_scoring=0, n_batches=40)")
     ap.add_argument("--no-extras", action="store_true", help="skip the C2 / C5 / LET_d / gamma-index measurements")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     args = ap.parse_args()
@@ -216,6 +218,9 @@ def main():
     pm.load_ct(hu_dev, w["vox"])
     offset, _ = weak_shard(n_hist, rank)
     pm.set_option("history_offset", float(offset))
+    for kv in args.option:
+        k_, v_ = kv.split("=", 1)
+        pm.set_option(k_, float(v_))
     spots = w["spots"]
     nvox = int(w["hu"].size)
     dose = torch.empty(w["hu"].shape, dtype=torch.float32, device=dev)
@@ -321,7 +326,7 @@ def main():
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": w["label"], "histories_per_step_per_gpu": n_hist, "n_spots": w["n_spots"],
                        "n_batches": 10, "l2": "flushed between timed steps (256 MiB write)",
-                       "parallelism": f"history-sharded x{world}"},
+                       "parallelism": f"history-sharded x{world}", "options": args.option},
             "clocks": {k: clocks[k] for k in ("sm_mhz", "sm_max_mhz", "reasons")},
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "steps": e2e_steps},

@@ -149,6 +149,8 @@ int  pmc_load_ct_host(pmc_ctx *ctx, const int16_t *hu_host, int nx, int ny, int 
  * 1 = full Moliere theory, needs the mol_* tables), "s_max_wet_cm", "n_batches",
  * "chunk_histories" (histories per sub-group), "history_offset" (first history id, for sharding
  * a run over several GPUs), "dose_aggregate" (0/1, default 0: merge the lanes of a warp that score into the same voxel before the atomic), "score_letd" (0/1, see pmc_get_letd),
+ * "dose_scoring" (0/1, default 1; 0 is for measurement only: the step kernel skips its dose atomics, which bounds what any
+ * other scoring scheme could gain - profiles/r02_c1_atomics.md),
  * "profile" (0/1, default 1: a CUDA-event pair is recorded on the context's stream around every kernel launch and
  * resolved into pmc_timing at the end of the call; no extra synchronisation). */
 int  pmc_set_option(pmc_ctx *ctx, const char *key, double value);

@@ -91,7 +91,7 @@ struct pmc_ctx {
   std::vector<int> ez, ea;
   std::vector<float> h_mol; int mol_n = 0; double mol_dth = 0; int mcs_model = 0; DevBuf<float> d_mol;
   double e_cut = 0.1, highland = 1.07, kappa_g = 10, s_max = 0.2; int n_batches = 10;
-  bool opt_strag = true, opt_mcs = true, opt_el = true, opt_ne = true; int aggregate = 0; bool profile = true;
+  bool opt_strag = true, opt_mcs = true, opt_el = true, opt_ne = true; int aggregate = 0; bool profile = true, skip_tally = false;
   uint64_t chunk = 1u << 24, history_offset = 0;
   std::vector<HostMat> mats;
   // device tables
@@ -278,6 +278,15 @@ int prepare_spots(pmc_ctx *c, const pmc_spot *spots, int nspots) {
   return PMC_OK;
 }
 
+// Philox4x32-10 key schedule of a seed: round r uses (seed_lo + r W0, seed_hi + r W1), the Weyl sequence of Salmon et al.
+RoundKeys key_schedule(uint64_t seed) {
+  RoundKeys K;
+  for (int r = 0; r < 10; ++r) {
+    K.k[2 * r] = (uint32_t)seed + (uint32_t)r * 0x9E3779B9u; K.k[2 * r + 1] = (uint32_t)(seed >> 32) + (uint32_t)r * 0xBB67AE85u;
+  }
+  return K;
+}
+
 // Always-on per-kernel-class timing: an event pair from a pool is recorded around every launch on the context's
 // stream (no synchronisation); the pairs are resolved once at the end of the call, after the stream is idle.
 struct Timer {
@@ -315,7 +324,7 @@ int run_generations(pmc_ctx *c, RunParams P, uint32_t n0, bool profile) {
     CK(cudaMemsetAsync(c->qev.q.count, 0, 4, s));
     { Timer t(c, &c->timing.transport_ms, profile);
       const bool mol = c->T.mcs_model == 1, dbg = P.dbg_out != nullptr;
-      const bool extra = !dbg && (P.let_num != nullptr || P.roi_map != nullptr || P.aggregate != 0);
+      const bool extra = !dbg && (P.let_num != nullptr || P.roi_map != nullptr || P.aggregate != 0 || P.skip_tally != 0);
 #define PMC_LAUNCH_TRANSPORT(M, D, X) transport_kernel<M, D, X><<<grid_t, TRANSPORT_THREADS, c->smem_transport, s>>>(c->T, c->G, P, cur->q, n_in, c->d_head.p, c->qev.q, c->d_tally.p, c->d_cnt.p)
       if (dbg) { if (mol) PMC_LAUNCH_TRANSPORT(1, true, false); else PMC_LAUNCH_TRANSPORT(0, true, false); }
       else if (mol) { if (extra) PMC_LAUNCH_TRANSPORT(1, false, true); else PMC_LAUNCH_TRANSPORT(1, false, false); }
@@ -522,6 +531,7 @@ int pmc_set_option(pmc_ctx *c, const char *key, double v) {
   else if (k == "chunk_histories") { if (v < 1 || v > 67108864.0) return fail(c, PMC_E_INVALID_ARG, "chunk_histories out of range"); c->chunk = (uint64_t)v; }
   else if (k == "history_offset") { if (v < 0) return fail(c, PMC_E_INVALID_ARG, "negative offset"); c->history_offset = (uint64_t)v; }
   else if (k == "dose_aggregate") c->aggregate = v != 0;
+  else if (k == "dose_scoring") c->skip_tally = v == 0;
   else if (k == "profile") c->profile = v != 0;
   else if (k == "score_letd") c->score_let = v != 0;
   else if (k == "mcs_model") { if ((v != 0 && v != 1) || (v == 1 && c->mol_n < 2)) return fail(c, PMC_E_INVALID_ARG, "mcs_model: 0 or 1 (1 needs the Moliere tables)"); c->mcs_model = (int)v; }
@@ -574,11 +584,8 @@ static int simulate_impl(pmc_ctx *c, const pmc_spot *spots_in, int nspots, uint6
   const int grid_v = c->n_sm * 8;
   for (uint64_t cs = 0; cs < n; cs += chunk) {
     const uint32_t nc = (uint32_t)std::min<uint64_t>(chunk, n - cs);
-    RunParams P{}; P.seed = seed; P.hist0 = c->history_offset + cs;
-    for (int r = 0; r < 10; ++r) {                                   // Philox key schedule (Weyl sequence)
-      P.rk.k[2 * r] = (uint32_t)seed + (uint32_t)r * 0x9E3779B9u; P.rk.k[2 * r + 1] = (uint32_t)(seed >> 32) + (uint32_t)r * 0xBB67AE85u;
-    } P.n = nc; P.max_steps = max_steps; P.dbg_out = dbg_out ? dbg_out + 8ull * cs : nullptr;
-    P.aggregate = c->aggregate; P.local0 = cs; P.n_total = n; P.B = (uint32_t)B; P.nvox = nvox;
+    RunParams P{}; P.seed = seed; P.hist0 = c->history_offset + cs; P.rk = key_schedule(seed); P.n = nc; P.max_steps = max_steps; P.dbg_out = dbg_out ? dbg_out + 8ull * cs : nullptr;
+    P.aggregate = c->aggregate; P.skip_tally = c->skip_tally ? 1 : 0; P.local0 = cs; P.n_total = n; P.B = (uint32_t)B; P.nvox = nvox;
     P.roi_map = roi_on ? c->d_roimap.p : nullptr; P.dij = roi_on ? c->dij_dev : nullptr; P.n_roi = roi_on ? c->n_roi : 0u;
     P.let_num = let_on ? c->d_let.p : nullptr; P.let_den = let_on ? c->d_let.p + nvox_s : nullptr;
     P.b_over_n = (float)((double)B / (double)n); P.inv_nx = 1.0f / (float)c->G.nx; P.inv_ny = 1.0f / (float)c->G.ny;
@@ -650,7 +657,7 @@ int pmc_nonelastic(pmc_ctx *c, int Z, int A, double e_mev, uint64_t n, uint64_t 
     const uint32_t nc = (uint32_t)std::min<uint64_t>(CH, n - ev0);
     CK(cudaMemsetAsync(c->d_head.p, 0, 16, s));
     const int gb = (int)std::min<uint32_t>((nc + 127) / 128, (uint32_t)c->n_sm * 6);
-    nonelastic_inc_kernel<<<gb, 128, 0, s>>>(c->T, c->d_nuc1.p, (float)e_mev, seed, ev0, nc, c->d_head.p + 1, c->d_slots.p, c->d_counts.p, c->d_res.p, c->d_cnt.p);
+    nonelastic_inc_kernel<<<gb, 128, 0, s>>>(c->T, c->d_nuc1.p, (float)e_mev, key_schedule(seed), ev0, nc, c->d_head.p + 1, c->d_slots.p, c->d_counts.p, c->d_res.p, c->d_cnt.p);
     nonelastic_evap_kernel<<<gb, 128, 0, s>>>(c->T, c->d_nuc1.p, seed, ev0, nc, c->d_head.p + 2, c->d_slots.p, c->d_counts.p, c->d_res.p, c->d_cnt.p);
     scan_kernel<<<1, 1024, 0, s>>>(c->d_counts.p, nc, off_dev + ev0, c->d_base.p);
     compact_kernel<<<(nc + 255) / 256, 256, 0, s>>>(c->d_slots.p, c->d_counts.p, off_dev + ev0, nc, reinterpret_cast<SecRec *>(out_dev), capacity);

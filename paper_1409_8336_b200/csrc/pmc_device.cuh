@@ -41,10 +41,20 @@ __device__ __forceinline__ uint4 philox4x32_10(uint4 c, const RoundKeys &K) {
   }
   return c;
 }
-// stream of one particle inside the step kernel (same counters and keys as Rng, hence the same blocks)
+// stream of one particle with the host-computed key schedule (same counters and keys as Rng, hence the same blocks); the
+// round keys are named at every call so that they stay in the constant bank instead of in per-thread registers
 struct RngK {
-  const RoundKeys &K; uint32_t h0, h1, pid, blk;
-  __device__ __forceinline__ uint4 next4() { return philox4x32_10(make_uint4(h0, h1, pid, blk++), K); }
+  uint32_t h0, h1, pid, blk;
+  __device__ __forceinline__ void init(uint64_t hist, uint32_t pid_, uint32_t blk_) { h0 = (uint32_t)hist; h1 = (uint32_t)(hist >> 32); pid = pid_; blk = blk_; }
+  __device__ __forceinline__ uint4 next4(const RoundKeys &K) { return philox4x32_10(make_uint4(h0, h1, pid, blk++), K); }
+  __device__ __forceinline__ uint32_t child_id(const RoundKeys &K, uint32_t k) const {
+    return philox4x32_10(make_uint4(h0, h1, pid, 0x80000000u | blk), K).x ^ (k + 1u);
+  }
+};
+// the pair (stream, keys) with the plain next4() interface of Rng, for code that is shared between the two
+struct RngKRef {
+  RngK &g; const RoundKeys &K;
+  __device__ __forceinline__ uint4 next4() { return g.next4(K); }
 };
 
 // Per-particle stream: key = seed, counter = (history_lo, history_hi, particle id, block number).  Draws are
@@ -185,12 +195,12 @@ __device__ __forceinline__ V3 operator+(V3 a, V3 b) { return {a.x + b.x, a.y + b
 __device__ __forceinline__ V3 operator-(V3 a, V3 b) { return {a.x - b.x, a.y - b.y, a.z - b.z}; }
 __device__ __forceinline__ V3 operator*(float s, V3 a) { return {s * a.x, s * a.y, s * a.z}; }
 __device__ __forceinline__ float dot(V3 a, V3 b) { return a.x * b.x + a.y * b.y + a.z * b.z; }
-__device__ __forceinline__ V3 unit(V3 a) { float n = rsqrtf(dot(a, a)); return {a.x * n, a.y * n, a.z * n}; }
+__device__ __forceinline__ V3 unit(V3 a) { float n = frsq(dot(a, a)); return {a.x * n, a.y * n, a.z * n}; }
 // components (a,b,c) in the frame whose z axis is the unit vector d -> lab frame
 __device__ __forceinline__ V3 to_lab(V3 d, float a, float b, float c) {
   const float s2 = d.x * d.x + d.y * d.y;
   if (s2 < 1e-14f) { const float sg = d.z >= 0.f ? 1.0f : -1.0f; return {a, sg * b, sg * c}; }
-  const float is = rsqrtf(s2), s = s2 * is;
+  const float is = frsq(s2), s = s2 * is;
   return {a * d.x * d.z * is - b * d.y * is + c * d.x, a * d.y * d.z * is + b * d.x * is + c * d.y, -a * s + c * d.z};
 }
 __device__ __forceinline__ V3 isotropic(uint32_t r0, uint32_t r1) {
@@ -202,7 +212,7 @@ __device__ __forceinline__ V3 isotropic(uint32_t r0, uint32_t r1) {
 __device__ __forceinline__ void boost(V3 beta, V3 &p, float &E) {
   const float b2 = dot(beta, beta);
   if (b2 <= 0.f) return;
-  const float gam = rsqrtf(1.0f - b2), bp = dot(beta, p);
+  const float gam = frsq(1.0f - b2), bp = dot(beta, p);
   const float f = fdiv(gam * gam, gam + 1.0f) * bp + gam * E;      // (gam-1)/b2 = gam^2/(gam+1)
   p = p + f * beta;
   E = gam * (E + bp);
@@ -337,16 +347,19 @@ __device__ __forceinline__ float straggle(const Tables &T, Gen &g, float e_start
 
 // ------------------------------------------------------------------ Cugnon NN parameterisation (PAPER.md:L77 ref [20]; Reading R6)
 // p in GeV/c, sigma in mb
+// (below 0.8 GeV/c - every collision of a cascade started below 250 MeV - both branches are evaluated and one selected:
+// the lanes of a warp sit at different momenta)
 __device__ __forceinline__ float cug_sigma_pp(float p) {
-  if (p < 0.44f) return 34.0f * __powf(p * 2.5f, -2.104f);
-  if (p < 0.8f) { float d = p - 0.7f; d *= d; return 23.5f + 1000.0f * d * d; }
+  if (p < 0.8f) { const float a = 34.0f * fex2(-2.104f * flg2(p * 2.5f)); float d = p - 0.7f; d *= d; return p < 0.44f ? a : fmaf(1000.0f * d, d, 23.5f); }
   if (p < 2.0f) return fdiv(1250.0f, p + 50.0f) - 4.0f * (p - 1.3f) * (p - 1.3f);
   return fdiv(77.0f, p + 1.5f);
 }
 __device__ __forceinline__ float cug_sigma_np(float p) {
-  if (p < 0.446f) { const float l = __logf(p); return 6.3555f * __expf(-3.2481f * l - 0.377f * l * l); }
-  if (p < 0.8f) { const float a = fabsf(p - 0.95f); return 33.0f + 196.0f * a * a * fsqrt(a); }
-  if (p < 2.0f) return 31.0f * rsqrtf(p);
+  if (p < 0.8f) {
+    const float l = LN2 * flg2(p), a = 6.3555f * fex2(LOG2E * (-3.2481f * l - 0.377f * l * l)), q = fabsf(p - 0.95f);
+    return p < 0.446f ? a : fmaf(196.0f * q * q, fsqrt(q), 33.0f);
+  }
+  if (p < 2.0f) return 31.0f * frsq(p);
   return fdiv(77.0f, p + 1.5f);
 }
 __device__ __forceinline__ float cug_b_pp(float p) {
@@ -364,7 +377,7 @@ __device__ __forceinline__ float cug_a_np(float p) { return p < 0.8f ? 1.0f : fd
 // |t| from exp(-B t) truncated to [0, tmax]
 __device__ __forceinline__ float trunc_exp(float B, float tmax, float u) {
   if (B * tmax < 1e-6f) return u * tmax;
-  return fdiv(-__logf(1.0f - u * (1.0f - __expf(-B * tmax))), B);
+  return fdiv(-flog(1.0f - u * (1.0f - fexp(-B * tmax))), B);
 }
 // cos(theta_cm) of NN elastic scattering: dsigma/dt ~ exp(B t) (+ a exp(B u) for np).  Uses 2 uniforms.
 __device__ __forceinline__ float sample_nn_cos(bool same, float p_lab_gev, float pcm_mev, uint32_t r0, uint32_t r1) {

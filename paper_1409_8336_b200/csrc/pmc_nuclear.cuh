@@ -47,11 +47,11 @@ struct IncLane {
 
 // entry: uniform over the disc of radius rmax, travelling along +z (L75 "random point of entry"); refraction into
 // the outermost shell: gains V, tangential momentum conserved
-__device__ __forceinline__ void inc_begin(const Nucleus &N, float t_in, Rng &g, IncLane &L) {
+__device__ __forceinline__ void inc_begin(const Nucleus &N, float t_in, RngK &g, const RoundKeys &K, IncLane &L) {
   const int ns = N.nshell;
   L.sp = 0; L.ncoll = 0; L.n_out = 0; L.np_out = 0; L.guard = 0; L.failed = false; L.trip = 0;
   L.e_out_sum = 0; L.pxs = 0; L.pys = 0; L.pzs = 0;
-  const uint4 r = g.next4();
+  const uint4 r = g.next4(K);
   const float b = N.rmax * sqrtf(u01(r.x)); float sph, cph; sincospif(2.0f * u01(r.y), &sph, &cph);
   const V3 r0{b * cph, b * sph, -sqrtf(fmaxf(0.f, N.rmax * N.rmax - b * b))};
   const float Tn = t_in + N.V[0][ns - 1], p0 = sqrtf(t_in * (t_in + 2.0f * MP)), p1 = sqrtf(Tn * (Tn + 2.0f * MP));
@@ -63,28 +63,38 @@ __device__ __forceinline__ void inc_begin(const Nucleus &N, float t_in, Rng &g, 
 }
 __device__ __forceinline__ void inc_fail(IncLane &L) { L.failed = true; L.alive = false; L.sp = 0; }
 
+// direction uniform on the sphere from two 16-bit fields
+__device__ __forceinline__ V3 isotropic16(uint32_t a16, uint32_t b16) {
+  const float c = fmaf(2.0f, u16f(a16), -1.0f), s = fsqrt(fmaxf(0.f, fmaf(-c, c, 1.0f)));
+  float sp, cp; sincos_2pi(u16f(b16), &sp, &cp);
+  return {s * cp, s * sp, c};
+}
 // one step of the nucleon being tracked: candidate collisions vs shell boundary (Reading R6.3-R6.5)
-__device__ __forceinline__ void inc_step(const Nucleus &N, Rng &g, IncLane &L) {
+__device__ __forceinline__ void inc_step(const Nucleus &N, RngK &g, const RoundKeys &K, IncLane &L) {
   CascNucleon &c = L.c;
   const int ns = N.nshell;
   if (++L.guard > MAX_INC_STEPS) { L.trip = 1; inc_fail(L); return; }   // bound orbit in a dilute shell (Reading R6.8)
   const int k = c.shell, ty = c.type;
   const float m = nucleon_mass(ty), p2 = dot(c.p, c.p), E = fsqrt(p2 + m * m), Tk = fdiv(p2, E + m);
-  const V3 d = rsqrtf(p2) * c.p;
-  // candidate collisions with a proton and with a neutron of the Fermi sea (Reading R6.3)
+  const V3 d = frsq(p2) * c.p;
+  // candidate collisions with a nucleon of the projectile's own type and with one of the other type, both from the Fermi
+  // sea (Reading R6.3).  One Philox block serves both: per partner 16 bits each for |q|^3, cos, azimuth and free path.
+  // Looping over same / other (instead of proton / neutron) keeps the lanes of a warp on the same cross-section formula.
   float dbest = BIG, plab_best = 0.f; int tbest = -1; V3 qbest{0.f, 0.f, 0.f};
+  const uint4 rq = g.next4(K);
 #pragma unroll
-  for (int tp = 0; tp < 2; ++tp) {
-    if (N.rho[tp][k] <= 0.f) continue;
-    const uint4 r = g.next4();
-    const float mq = nucleon_mass(tp), qmag = N.pF[tp][k] * __powf(u01(r.x), 1.0f / 3.0f);
-    const V3 q = qmag * isotropic(r.y, r.z);
-    const float Eq = fsqrt(qmag * qmag + mq * mq);
+  for (int s = 0; s < 2; ++s) {
+    const int tp = s == 0 ? ty : 1 - ty;
+    const float rho = N.rho[tp][k];
+    if (rho <= 0.f) continue;
+    const uint32_t wa = s == 0 ? rq.x : rq.z, wb = s == 0 ? rq.y : rq.w;
+    const float mq = nucleon_mass(tp), qmag = N.pF[tp][k] * fex2(flg2(u16f(wa >> 16)) * (1.0f / 3.0f));
+    const V3 q = qmag * isotropic16(wa & 0xFFFFu, wb >> 16);
+    const float Eq = fsqrt(fmaf(qmag, qmag, mq * mq));
     const float e1 = (E * Eq - dot(c.p, q)) * (tp == 0 ? 1.0f / MP : 1.0f / MN);                       // projectile energy in the partner rest frame
-    const float plab = fsqrt(fmaxf(e1 * e1 - m * m, 0.f));
-    const float sig = N.const_sigma_mb >= 0.f ? N.const_sigma_mb
-                                              : (tp == ty ? cug_sigma_pp(plab * 1e-3f) : cug_sigma_np(plab * 1e-3f));
-    const float dist = fdiv(-__logf(u01(r.w)), N.rho[tp][k] * sig * 0.1f);  // 1 mb = 0.1 fm^2
+    const float plab = fsqrt(fmaxf(fmaf(e1, e1, -m * m), 0.f));
+    const float sig = N.const_sigma_mb >= 0.f ? N.const_sigma_mb : (s == 0 ? cug_sigma_pp(plab * 1e-3f) : cug_sigma_np(plab * 1e-3f));
+    const float dist = -LN2 * flg2(u16f(wb & 0xFFFFu)) * frcp(rho * sig * 0.1f);  // 1 mb = 0.1 fm^2
     if (dist < dbest) { dbest = dist; tbest = tp; qbest = q; plab_best = plab; }
   }
   // distance to the shell boundaries along d
@@ -104,7 +114,7 @@ __device__ __forceinline__ void inc_step(const Nucleus &N, Rng &g, IncLane &L) {
     const float pcm = fsqrt(fmaxf((s - (m + mq) * (m + mq)) * (s - (m - mq) * (m - mq)), 0.f) * fdiv(0.25f, s));
     V3 p1 = c.p; float E1 = E; boost(-1.0f * beta, p1, E1);             // projectile in the CM
     const V3 ax = unit(p1);
-    const uint4 r = g.next4();
+    const uint4 r = g.next4(K);
     const float ct = sample_nn_cos(tp == ty, plab_best * 1e-3f, pcm, r.x, r.y), st = fsqrt(fmaxf(0.f, 1.0f - ct * ct));
     float sph, cph; sincos_2pi(u01(r.z), &sph, &cph);
     V3 n1 = pcm * to_lab(ax, st * cph, st * sph, ct), n2 = -1.0f * n1;
@@ -127,7 +137,7 @@ __device__ __forceinline__ void inc_step(const Nucleus &N, Rng &g, IncLane &L) {
   // ---- shell boundary (L77 "reflection and refraction"; Reading R6.5)
   c.r = c.r + dbound * d;
   const float rb = inward ? r_in : r_out;
-  c.r = (rb * rsqrtf(dot(c.r, c.r))) * c.r;
+  c.r = (rb * frsq(dot(c.r, c.r))) * c.r;
   const V3 nh = fdiv(1.0f, rb) * c.r;
   const float pr = dot(c.p, nh); const V3 pt = c.p - pr * nh;
   const int k2 = inward ? k - 1 : k + 1;
@@ -176,7 +186,7 @@ __device__ __forceinline__ void inc_compound(const Tables &T, const Nucleus &N, 
 // All 32 lanes of every warp must call.
 struct IncStats { unsigned long long tries = 0, guard = 0, cap = 0; int hw_stack = 0, hw_out = 0; };
 template <class Load, class Store>
-__device__ __forceinline__ void inc_machine(const Tables &T, uint32_t n, uint32_t *head, IncStats &st,
+__device__ __forceinline__ void inc_machine(const Tables &T, const RoundKeys &K, uint32_t n, uint32_t *head, IncStats &st,
                                             Load load, Store store) {
   // Lane states.  STEP: tracking a nucleon.  WAIT: attempt finished (needs finalize, then store + next event, or a
   // fresh attempt) or no event yet.  DONE: queue exhausted.  The turnover work of WAIT lanes is divergent and long
@@ -185,7 +195,7 @@ __device__ __forceinline__ void inc_machine(const Tables &T, uint32_t n, uint32_
   enum { STEP = 0, WAIT = 1, DONE = 2 };
   constexpr int TURNOVER = 8;
   IncLane L; L.alive = false; L.sp = 0; L.failed = false; L.trip = 0; L.hw_stack = 0; L.hw_out = 0;
-  const Nucleus *N = nullptr; float t_in = 0.f; Rng g; uint32_t ev = 0; int ntry = 0;
+  const Nucleus *N = nullptr; float t_in = 0.f; RngK g; uint32_t ev = 0; int ntry = 0;
   bool busy = false; int state = WAIT;
   const int lane = threadIdx.x & 31;
   while (true) {
@@ -197,7 +207,7 @@ __device__ __forceinline__ void inc_machine(const Tables &T, uint32_t n, uint32_
         Residual R;
         if (inc_finalize(T, *N, t_in, L, R)) { store(ev, g, L.out, L.n_out, R); busy = false; }
         else if (ntry >= 100000) { inc_compound(T, *N, t_in, R); store(ev, g, L.out, 0, R); busy = false; }
-        else { ++ntry; st.tries++; inc_begin(*N, t_in, g, L); state = STEP; }
+        else { ++ntry; st.tries++; inc_begin(*N, t_in, g, K, L); state = STEP; }
       }
       __syncwarp();
       const unsigned need = __ballot_sync(0xffffffffu, state == WAIT && !busy);
@@ -208,14 +218,14 @@ __device__ __forceinline__ void inc_machine(const Tables &T, uint32_t n, uint32_
         base = __shfl_sync(0xffffffffu, base, leader);
         if (state == WAIT && !busy) {
           ev = base + (uint32_t)__popc(need & ((1u << lane) - 1u));
-          if (ev < n) { load(ev, N, t_in, g); busy = true; ntry = 1; st.tries++; inc_begin(*N, t_in, g, L); state = STEP; }
+          if (ev < n) { load(ev, N, t_in, g); busy = true; ntry = 1; st.tries++; inc_begin(*N, t_in, g, K, L); state = STEP; }
           else state = DONE;
         }
       }
       __syncwarp();
     }
     if (state == STEP) {
-      inc_step(*N, g, L);
+      inc_step(*N, g, K, L);
       if (!L.alive) {
         if (L.sp > 0) { L.c = L.stack[--L.sp]; L.alive = true; }
         else state = WAIT;
@@ -240,29 +250,33 @@ __device__ __forceinline__ float pairing(int Z, int A) {
   const int N = A - Z; const float d = 12.0f * rsqrtf((float)A);
   return (Z % 2 == 0 && N % 2 == 0) ? 2.0f * d : ((Z % 2) != (N % 2) ? d : 0.f);
 }
-struct Chan { float S, emin, emax, kV, cj, pref, alpha, beta, ad; int Zd, Ad; double Md, mj; };
-__device__ bool chan_setup(const Tables &T, int Z, int A, float estar, double Mpar, int j, Chan &c) {
+// One open channel.  The integrand of its width, P_j(e) = pref sigma_inv(e) e exp(2 sqrt(a_d (emax - e)) - ref), is kept in
+// the form (s1 e + s0) 2^(A sqrt(emax - e) - B): sigma_inv(e) e is linear in e for Dostrovsky's inverse cross-sections
+// (alpha (e + beta) for neutrons, (1 + c_j)(e - k_j V_j) for charged ejectiles), so a quadrature point costs two MUFU
+// and five FMA-class instructions.
+struct Chan { float S, emin, emax, s1, s0, A, B; int Zd, Ad; double Md, mj; };
+__device__ bool chan_setup(const Tables &T, int Z, int A, float estar, double Mpar, int j, float ref, Chan &c) {
   const int Zd = Z - EJ_Z[j], Ad = A - EJ_A[j];
   if (Ad < 2 || Zd < 0) return false;
   const double Md = nmass(T, Zd, Ad), mj = nmass(T, EJ_Z[j], EJ_A[j]);
   if (Md <= 0) return false;
   c.Zd = Zd; c.Ad = Ad; c.Md = Md; c.mj = mj; c.S = (float)(Md + mj - Mpar);
   const float a13 = cbrtf((float)Ad);
-  c.kV = 0.f; c.cj = 0.f;
+  float kV = 0.f, cj = 0.f;
   if (j > 0) {
     const float rhoj = j == 1 ? 0.f : 1.2f, V = 1.44f * EJ_Z[j] * Zd / (1.5f * a13 + rhoj);
-    c.kV = T.evap_k[j * T.zdim + Zd] * V; c.cj = T.evap_c[j * T.zdim + Zd];
+    kV = T.evap_k[j * T.zdim + Zd] * V; cj = T.evap_c[j * T.zdim + Zd];
   }
-  c.emin = c.kV; c.emax = estar - c.S - pairing(Zd, Ad);
+  c.emin = kV; c.emax = estar - c.S - pairing(Zd, Ad);
   if (c.emax <= c.emin) return false;
-  c.alpha = 0.76f + 2.2f / a13; c.beta = (2.12f / (a13 * a13) - 0.050f) / c.alpha; c.ad = Ad * 0.125f;
-  c.pref = EJ_SPIN_G[j] * (float)mj * a13 * a13;
+  const float alpha = 0.76f + 2.2f / a13, beta = (2.12f / (a13 * a13) - 0.050f) / alpha;
+  const float pref = EJ_SPIN_G[j] * (float)mj * a13 * a13;
+  c.s1 = pref * (j == 0 ? alpha : 1.0f + cj); c.s0 = j == 0 ? c.s1 * beta : -c.s1 * kV;
+  c.A = 2.0f * LOG2E * sqrtf(Ad * 0.125f); c.B = ref * LOG2E;
   return true;
 }
-__device__ __forceinline__ float chan_f(const Chan &c, int j, float e, float ref) {
-  // sigma_inv(e) x e written without the division: alpha (e + beta) for neutrons, (1 + c_j)(e - k_j V_j) for charged
-  const float sinv_e = j == 0 ? c.alpha * (e + c.beta) : (1.0f + c.cj) * (e - c.kV);
-  return c.pref * sinv_e * __expf(2.0f * fsqrt(c.ad * (c.emax - e)) - ref);
+__device__ __forceinline__ float chan_f(const Chan &c, float e) {
+  return fmaf(c.s1, e, c.s0) * fex2(fmaf(c.A, fsqrt(c.emax - e), -c.B));
 }
 struct Emission { int j; float ke; V3 dir; };
 // one emission from R (updated in place); returns false when no channel is open
@@ -274,10 +288,11 @@ __device__ bool evap_emit(const Tables &T, Residual &R, Rng &g, uint32_t mask, E
   for (int j = 0; j < 6; ++j) {
     width[j] = 0.f;
     Chan c;
-    if (!((mask >> j) & 1u) || !chan_setup(T, R.Z, R.A, estar, R.mass_gs, j, c)) continue;
+    if (!((mask >> j) & 1u) || !chan_setup(T, R.Z, R.A, estar, R.mass_gs, j, ref, c)) continue;
     const float de = (c.emax - c.emin) * (1.0f / NQ);
     float w = 0.f;
-    for (int i = 0; i < NQ; ++i) w += chan_f(c, j, c.emin + (i + 0.5f) * de, ref);
+#pragma unroll 8
+    for (int i = 0; i < NQ; ++i) w += chan_f(c, fmaf((float)i + 0.5f, de, c.emin));
     width[j] = w * de; tot += width[j];
   }
   if (!(tot > 0.f)) return false;
@@ -285,10 +300,10 @@ __device__ bool evap_emit(const Tables &T, Residual &R, Rng &g, uint32_t mask, E
   float u = u01(r.x) * tot; int j = -1;
 #pragma unroll
   for (int q = 0; q < 6; ++q) if (width[q] > 0.f && (j < 0 || u >= 0.f)) { j = q; u -= width[q]; }
-  Chan c; chan_setup(T, R.Z, R.A, estar, R.mass_gs, j, c);
+  Chan c; chan_setup(T, R.Z, R.A, estar, R.mass_gs, j, ref, c);
   const float de = (c.emax - c.emin) * (1.0f / NQ);
   float v = u01(r.y) * width[j] / de; int bin = NQ - 1;
-  for (int i = 0; i < NQ; ++i) { const float f = chan_f(c, j, c.emin + (i + 0.5f) * de, ref); if (v < f) { bin = i; break; } v -= f; }
+  for (int i = 0; i < NQ; ++i) { const float f = chan_f(c, fmaf((float)i + 0.5f, de, c.emin)); if (v < f) { bin = i; break; } v -= f; }
   const float eps = c.emin + ((float)bin + u01(r.z)) * de;                  // total CM kinetic energy released
   // relativistic two-body decay of M* -> m_j + M_d* (isotropic in the nucleus rest frame, L79), fp64
   const uint4 r2 = g.next4();
@@ -361,12 +376,12 @@ __global__ void __launch_bounds__(128) inc_kernel(Tables T, RunParams P, Queue i
   const uint32_t n = min(*in.count, in.cap);
   double c_dep = 0, c_neu = 0, c_q = 0; unsigned long long c_sec = 0; IncStats st;
   Particle p;
-  auto load = [&](uint32_t i, const Nucleus *&N, float &t_in, Rng &g) {
+  auto load = [&](uint32_t i, const Nucleus *&N, float &t_in, RngK &g) {
     p = queue_load(in, i);
-    g.init(P.seed, P.hist0 + p.hist, p.pid, p.blk);
+    g.init(P.hist0 + p.hist, p.pid, p.blk);
     N = &T.nuc[aux_low(p.aux)]; t_in = p.e;
   };
-  auto store = [&](uint32_t, Rng &g, const OutNuc *outn, int n_out, const Residual &R) {
+  auto store = [&](uint32_t, RngK &g, const OutNuc *outn, int n_out, const Residual &R) {
     const Nucleus &N = T.nuc[aux_low(p.aux)];
     float dep = 0.f; uint32_t kchild = 0; double msum = 0;
     for (int k = 0; k < n_out; ++k) {
@@ -375,7 +390,7 @@ __global__ void __launch_bounds__(128) inc_kernel(Tables T, RunParams P, Queue i
       if (o.type == 0) {                                                   // L79: only protons are followed
         if (o.ke > T.e_cut) {
           Particle s = p; s.d = unit(to_lab(p.d, o.dir.x, o.dir.y, o.dir.z)); s.e = o.ke;
-          s.pid = g.child_id(kchild++); s.blk = 0u; s.aux = aux_with(p.aux, 0u); c_sec++;
+          s.pid = g.child_id(P.rk, kchild++); s.blk = 0u; s.aux = aux_with(p.aux, 0u); c_sec++;
           if (!queue_push(out, s)) atomicOr(&cnt->overflow, 16u);
         } else dep += o.ke;
       } else c_neu += (double)o.ke;                                        // neutrons: not transported
@@ -393,7 +408,7 @@ __global__ void __launch_bounds__(128) inc_kernel(Tables T, RunParams P, Queue i
       rq.px[slot] = (float)R.P[0]; rq.py[slot] = (float)R.P[1]; rq.pz[slot] = (float)R.P[2];
     }
   };
-  inc_machine(T, n, head, st, load, store);
+  inc_machine(T, P.rk, n, head, st, load, store);
   flush(&cnt->e_deposit, c_dep); flush(&cnt->e_neutron, c_neu); flush(&cnt->e_q, c_q);
   flush(&cnt->n_secondary, c_sec); flush_inc_stats(cnt, st);
 }
@@ -438,12 +453,12 @@ __global__ void __launch_bounds__(128) evap_kernel(Tables T, RunParams P, ResQue
 // Two kernels like the scheduler's (cascade, then de-excitation); event i of the call uses the stream (seed, ev0 + i).
 struct ResRec { int Z, A; double estar; double P[3]; uint32_t blk; int zs, as; };
 
-__global__ void __launch_bounds__(128) nonelastic_inc_kernel(Tables T, const Nucleus *nuc, float t_in0, uint64_t seed, uint64_t ev0,
+__global__ void __launch_bounds__(128) nonelastic_inc_kernel(Tables T, const Nucleus *nuc, float t_in0, RoundKeys K, uint64_t ev0,
                                                              uint32_t n, uint32_t *head, SecRec *slots, uint32_t *counts,
                                                              ResRec *res, Counters *cnt) {
   IncStats st;
-  auto load = [&](uint32_t i, const Nucleus *&N, float &t_in, Rng &g) { g.init(seed, ev0 + i, 0u, 0u); N = nuc; t_in = t_in0; };
-  auto store = [&](uint32_t i, Rng &g, const OutNuc *outn, int n_out, const Residual &R) {
+  auto load = [&](uint32_t i, const Nucleus *&N, float &t_in, RngK &g) { g.init(ev0 + i, 0u, 0u); N = nuc; t_in = t_in0; };
+  auto store = [&](uint32_t i, RngK &g, const OutNuc *outn, int n_out, const Residual &R) {
     SecRec *s = slots + (size_t)i * MAX_SEC; int zs = 0;
     for (int k = 0; k < n_out; ++k) {
       SecRec rec{}; rec.Z = outn[k].type == 0 ? 1 : 0; rec.A = 1; rec.origin = 0; rec.ke = outn[k].ke;
@@ -455,7 +470,7 @@ __global__ void __launch_bounds__(128) nonelastic_inc_kernel(Tables T, const Nuc
     rr.blk = g.blk; rr.zs = zs; rr.as = n_out;
     res[i] = rr;
   };
-  inc_machine(T, n, head, st, load, store);
+  inc_machine(T, K, n, head, st, load, store);
   flush_inc_stats(cnt, st);
 }
 

@@ -24,6 +24,7 @@ struct RunParams {
   const int32_t *roi_map; float *dij; uint32_t n_roi;
   int max_steps; float *dbg_out;      // pmc_first_steps: stop after max_steps, write [hist][8]
   int aggregate;                      // warp-aggregated dose atomics
+  int skip_tally;                     // measurement only (option "dose_scoring" = 0): the step kernel scores nothing
 };
 
 // The queue word `aux` carries the spot index of the history in its upper 24 bits through every generation; the low
@@ -363,7 +364,8 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM) tr
     if (active) {
       // the stream is re-keyed from (history, particle, block) every step: only the block counter lives across steps
       const uint64_t hid = P.hist0 + p.hist;
-      RngK g{P.rk, (uint32_t)hid, (uint32_t)(hid >> 32), p.pid, p.blk};
+      RngK gk; gk.init(hid, p.pid, p.blk);
+      RngKRef g{gk, P.rk};
       // ---- material of the current voxel
       const int hu = G.hu[p.vox];
       const MatBin &m = s_bins[s_lut[min(max(hu - T.hu_lut_lo, 0), T.hu_lut_n - 1)]];
@@ -457,7 +459,7 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM) tr
       c_dep += dep;
       if (alive && exits) { atomicAdd(&cnt->e_escape, (double)p.e); alive = false; }   // L71 (3): leaves the grid
       if (DBG) ++nstep;
-      p.blk = g.blk;
+      p.blk = gk.blk;
       if (alive && cls == 2 && !DBG) {
         // ---- 8. discrete nuclear event at the end point (L71): handed to event_kernel, which picks the class and
         // the target element with all lanes busy instead of one lane of this warp
@@ -475,6 +477,7 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM) tr
         }
       }
     }
+    if (EXTRA && P.skip_tally) continue;
     if (EXTRA) {
       deposit(tally, tbase + (uint32_t)dep_vox, dep, dep != 0.f, P.aggregate, P.let_num, P.let_den, (uint32_t)dep_vox, let > 0.f ? dep : 0.f, let);
       if (P.roi_map != nullptr && dep != 0.f) score_influence(P, p.aux, dep_vox, dep);

@@ -337,17 +337,18 @@ def test_pencil_on_a_voxel_edge(pm, tables):
     o = _setup(pm, tables, w["materials"], w["hu"], w["vox"])
     spot = inputs.plan_single_spot((5.0, 5.0, 0.0), 150.0, 0.0)
     dg, sg, do, so, cg, co = _dose_parity(pm, o, w["hu"], w["vox"], w["materials"], spot, 400_000, 61, seed_o=62)
-    # Every step scores in the voxel it starts in, so the voxel that owns the start point collects the first legs of all
-    # the protons and its column gets more than its three neighbours: an artefact of any class II scheme for a pencil of
-    # zero width, identical on both sides because both use the same tie rule (the start point belongs to the upper voxel,
-    # fp64 on both sides).  What must hold: the excess is the same, and the x <-> y mirror pair is equal.
-    ratio = []
-    for d, s_ in ((dg, sg), (do, so)):
-        col = d[:70].sum(axis=0); err = np.sqrt((s_[:70] ** 2).sum(axis=0))
-        assert abs(col[24, 25] - col[25, 24]) < 4.5 * np.hypot(err[24, 25], err[25, 24]), (col[24, 25], col[25, 24])
-        ratio.append((col[25, 25] / col[24, 24], col[25, 25] / col[24, 24] * np.hypot(err[25, 25] / col[25, 25], err[24, 24] / col[24, 24])))
-    assert ratio[0][0] > 1.01 and ratio[1][0] > 1.01                       # the owner of the edge is voxel (25, 25) on both sides
-    assert abs(ratio[0][0] - ratio[1][0]) < 4.5 * np.hypot(ratio[0][1], ratio[1][1]), ratio
+    # Every step scores in the voxel it starts in, and a proton deflected towards a face it sits on crosses it at once and
+    # is deflected afresh in the next voxel: for a pencil of zero width on an edge the four columns around it therefore get
+    # slightly different doses (4 % more in the voxel that owns the start point, 1 % between the two mirror columns because
+    # x faces are met before y faces, Reading R3.2) - artefacts of the class II scheme of a few micrometres, identical on
+    # both sides because the tie rules are (start point: upper voxel, placed in fp64; faces: x before y before z).  What
+    # parity asks: each of the four columns agrees within its statistical error, and so does the excess of the owner.
+    # (the slabs of a column are crossed by the same protons, so their errors add linearly, not in quadrature)
+    cg_, co_ = dg[:70].sum(axis=0), do[:70].sum(axis=0)
+    eg_, eo_ = sg[:70].sum(axis=0), so[:70].sum(axis=0)
+    for a in ((24, 24), (24, 25), (25, 24), (25, 25)):
+        assert abs(cg_[a] - co_[a]) < 3.0 * np.hypot(eg_[a], eo_[a]), (a, cg_[a], co_[a], eg_[a], eo_[a])
+    assert cg_[25, 25] / cg_[24, 24] > 1.02 and co_[25, 25] / co_[24, 24] > 1.02
     # first steps from the edge: after 30 steps the transverse distribution is symmetric and equal on both sides
     for k_ in ("elastic", "nonelastic"):
         pm.set_option(k_, 0.0); o.set_option(k_, 0.0)
@@ -414,11 +415,24 @@ def test_c4_head_and_neck_at_full_size_on_both_sides(pm, tables):
     assert nv > 30_000 and frac >= 0.99 and abs(zmean) < 0.1 and zrms < 1.15, (frac, zmean, zrms, nv)
     assert f10 >= 0.99 - 0.003 and f_all >= 0.985, (f10, f_all)
     # the three 1-D projections of deposited energy, slab by slab
+    # every slab above 5 % of the largest one.  The statistical error of a slab sum (its voxels share histories, so the voxel
+    # sigmas cannot simply be added) is measured: the scatter of twelve more 1e7-history runs of the CUDA path with other seeds (variance smoothed over
+    # nine neighbouring slabs; thirteen runs alone leave the per-slab sigma uncertain by 20 %).
+    prof_g = [[parity.depth_dose(dg * rho, ax) for ax in range(3)]]
+    for k in range(12):
+        dk, _ = pm.simulate(w["spots"], n, 7000 + k)
+        dk = dk.cpu().numpy().astype(np.float64) * rho
+        prof_g.append([parity.depth_dose(dk, ax) for ax in range(3)])
     for ax in range(3):
-        pg, po = parity.depth_dose(dg * rho, ax), parity.depth_dose(do * rho, ax)
-        eg_, eo_ = np.sqrt(parity.depth_dose((sg * rho) ** 2, ax)), np.sqrt(parity.depth_dose((so * rho) ** 2, ax))
+        runs = np.array([p_[ax] for p_ in prof_g]); po = parity.depth_dose(do * rho, ax)
+        mean = runs.mean(axis=0)
+        rel_var = np.convolve(runs.var(axis=0, ddof=1) / np.maximum(mean, 1e-300) ** 2, np.ones(9) / 9, mode="same")
+        sd = np.sqrt(rel_var) * mean
         m = po > 0.05 * po.max()
-        assert np.all(np.abs(pg[m] - po[m]) < 5 * np.hypot(eg_[m], eo_[m]) + 2e-3 * po[m]), ax
+        zz = (mean[m] - po[m]) / (sd[m] * np.sqrt(1 + 1 / 13.0))
+        print(f"PROJ axis {ax}: max |z| {np.abs(zz).max():.2f} mean z {zz.mean():+.2f} rms z {zz.std():.2f} max rel diff {np.max(np.abs(mean[m] / po[m] - 1)):.2e}")
+        assert np.all(np.abs(mean[m] - po[m]) < 4.5 * sd[m] * np.sqrt(1 + 1 / 13.0) + 1e-3 * po[m]), (ax, np.abs(zz).max())
+        assert np.all(np.abs(mean[m] / po[m] - 1) < 2e-2)
     # sigma: same number of histories, same sigma (median relative error in the high-dose region)
     hi = tissue & (do > 0.5 * do[tissue].max())
     assert abs(np.median(sg[hi] / dg[hi]) / np.median(so[hi] / do[hi]) - 1) < 0.05
@@ -553,7 +567,10 @@ def test_letd_full_physics_matches_oracle(pm, tables):
         return (l * d).sum(axis=(1, 2)) / np.maximum(d.sum(axis=(1, 2)), 1e-300)
     pg, po, po2 = prof(lg, dg), prof(lo, do), prof(lo2, do2)
     dd = do.sum(axis=(1, 2)); m = dd > 0.1 * dd.max()
+    # noise yardstick: the oracle-vs-oracle difference, as the largest over a window of +-3 slabs (a few soft secondary
+    # protons of very high LET dominate the entrance slabs, so the scatter of a single slab is itself very noisy)
     noise = np.abs(po2[m] / po[m] - 1)
+    noise = np.array([noise[max(0, i - 3):i + 4].max() for i in range(len(noise))])
     assert np.all(np.abs(pg[m] / po[m] - 1) < 0.01 + 4 * np.maximum(noise, np.median(noise))), (pg[m] / po[m])[:80]
     assert abs(np.mean(pg[m] / po[m]) - 1) < 3e-3                         # no systematic offset along the depth
     # voxel by voxel in the high-dose region: GPU-vs-oracle scatter is the oracle-vs-oracle scatter
