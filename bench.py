@@ -334,7 +334,7 @@ def main():
             "roofline": roofline, "cpu_baseline": cpu, "extras": extras,
             "kernel_ms_per_step": {k: v / args.steps for k, v in klass.items()},
             "counters_last_step": {k: cnt_last[k] for k in ("n_steps", "n_elastic", "n_nonelastic",
-                                                            "n_secondary_protons", "n_generations", "n_missed")},
+                                                            "n_secondary_protons", "n_generations", "n_missed", "n_host_waits")},
             "context": "paper: ~20 s per 1e7 histories on a GTX680 incl. transfers (PAPER.md:L15), i.e. ~5e5 hist/s",
         }
         print(json.dumps(out))

@@ -103,6 +103,7 @@ typedef struct pmc_counters {    /* totals of the last pmc_simulate / pmc_nonela
   /* Reading R6.8 bookkeeping of the cascade: attempts abandoned by the 1024-step guard, attempts abandoned because the
    * fixed capacities were reached (16 waiting or 16 outgoing nucleons), and the deepest stack / most outgoing nucleons seen */
   uint64_t n_inc_guard_trips, n_inc_cap_trips, inc_max_stack, inc_max_out;
+  uint64_t n_host_waits;         /* times the scheduler waited for the device to learn a queue size (one per sub-group if <= 6 generations) */
 } pmc_counters;
 
 typedef struct pmc_timing {      /* CUDA-event time (ms) per kernel class over the last pmc_simulate call */

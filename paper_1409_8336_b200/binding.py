@@ -45,7 +45,7 @@ class Counters(C.Structure):
                                           "n_inc_tries", "n_generations")] + \
                [(k, C.c_double) for k in ("e_source", "e_deposit", "e_escape", "e_neutron", "e_gamma", "e_q", "e_air")] + \
                [(k, C.c_uint64) for k in ("n_zab_violations", "n_inc_guard_trips", "n_inc_cap_trips", "inc_max_stack",
-                                          "inc_max_out")]
+                                          "inc_max_out", "n_host_waits")]
 
 
 class Timing(C.Structure):

@@ -235,6 +235,9 @@ int sync_tables(pmc_ctx *c) {
   return PMC_OK;
 }
 
+// generations enqueued before the host first looks at a queue size, then per look; slots of the per-generation counts
+constexpr int GEN_BURST = 6, GEN_MORE = 2, GEN_SLOTS = 64;
+
 int ensure_scratch(pmc_ctx *c, uint64_t chunk) {
   const uint32_t cap = (uint32_t)std::max<uint64_t>(chunk + chunk / 4 + 4096, 8192);
   if (cap > c->qcap) {
@@ -242,8 +245,8 @@ int ensure_scratch(pmc_ctx *c, uint64_t chunk) {
     CK(c->d_resza.alloc(cap)); CK(c->d_resp.alloc((size_t)cap * 3));
     c->qcap = cap;
   }
-  CK(c->d_head.alloc(4)); CK(c->d_cnt.alloc(1));
-  if (!c->h_pinned) CK(cudaMallocHost(&c->h_pinned, 64));
+  CK(c->d_head.alloc(4 + GEN_SLOTS)); CK(c->d_cnt.alloc(1));
+  if (!c->h_pinned) CK(cudaMallocHost(&c->h_pinned, 4 * (GEN_SLOTS + 4)));
   if (!c->ev[0]) { CK(cudaEventCreate(&c->ev[0])); CK(cudaEventCreate(&c->ev[1])); }
   return PMC_OK;
 }
@@ -310,43 +313,53 @@ void resolve_timers(pmc_ctx *c) {       // stream must be idle
 }
 
 // The event-based scheduler (north_star; replaces the paper's transport kernel + Thrust collect/sort, L136):
-// generation loop over compacted queues until every queue is empty.
-int run_generations(pmc_ctx *c, RunParams P, uint32_t n0, bool profile) {
+// generation loop over compacted queues until every queue is empty.  Every kernel reads the size of its input queue on
+// the device, so the host does not wait between generations: it enqueues GEN_BURST generations, then reads the size of
+// the next queue once (C4 and C5 need 6 generations: one wait per sub-group) and goes on only if it is not empty.
+int run_generations(pmc_ctx *c, RunParams P, bool profile) {
   cudaStream_t s = c->stream;
   QueueMem *cur = &c->qa, *nxt = &c->qb;
-  uint32_t n_in = n0;
   const int grid_t = c->n_sm * TRANSPORT_BLOCKS_PER_SM, grid_e = c->n_sm * 4;
   ResQueue rq = res_queue(c);
-  while (n_in > 0) {
-    c->counters.n_generations++;
-    CK(cudaMemsetAsync(c->d_head.p, 0, 16, s)); CK(cudaMemsetAsync(nxt->q.count, 0, 4, s));
-    CK(cudaMemsetAsync(c->qel.q.count, 0, 4, s)); CK(cudaMemsetAsync(c->qne.q.count, 0, 4, s)); CK(cudaMemsetAsync(c->qres.q.count, 0, 4, s));
-    CK(cudaMemsetAsync(c->qev.q.count, 0, 4, s));
-    { Timer t(c, &c->timing.transport_ms, profile);
-      const bool mol = c->T.mcs_model == 1, dbg = P.dbg_out != nullptr;
-      const bool extra = !dbg && (P.let_num != nullptr || P.roi_map != nullptr || P.aggregate != 0 || P.skip_tally != 0);
-#define PMC_LAUNCH_TRANSPORT(M, D, X) transport_kernel<M, D, X><<<grid_t, TRANSPORT_THREADS, c->smem_transport, s>>>(c->T, c->G, P, cur->q, n_in, c->d_head.p, c->qev.q, c->d_tally.p, c->d_cnt.p)
-      if (dbg) { if (mol) PMC_LAUNCH_TRANSPORT(1, true, false); else PMC_LAUNCH_TRANSPORT(0, true, false); }
-      else if (mol) { if (extra) PMC_LAUNCH_TRANSPORT(1, false, true); else PMC_LAUNCH_TRANSPORT(1, false, false); }
-      else { if (extra) PMC_LAUNCH_TRANSPORT(0, false, true); else PMC_LAUNCH_TRANSPORT(0, false, false); }
+  uint32_t *gen_n = c->d_head.p + 4;                 // particles entering generation g (read back at the end)
+  CK(cudaMemsetAsync(gen_n, 0, GEN_SLOTS * 4, s));
+  int g = 0, burst = GEN_BURST;
+  while (true) {
+    for (int k = 0; k < burst && g < GEN_SLOTS; ++k, ++g) {
+      CK(cudaMemsetAsync(c->d_head.p, 0, 16, s)); CK(cudaMemsetAsync(nxt->q.count, 0, 4, s));
+      CK(cudaMemsetAsync(c->qel.q.count, 0, 4, s)); CK(cudaMemsetAsync(c->qne.q.count, 0, 4, s)); CK(cudaMemsetAsync(c->qres.q.count, 0, 4, s));
+      CK(cudaMemsetAsync(c->qev.q.count, 0, 4, s));
+      { Timer t(c, &c->timing.transport_ms, profile);
+        const bool mol = c->T.mcs_model == 1, dbg = P.dbg_out != nullptr;
+        const bool extra = !dbg && (P.let_num != nullptr || P.roi_map != nullptr || P.aggregate != 0 || P.skip_tally != 0);
+#define PMC_LAUNCH_TRANSPORT(M, D, X) transport_kernel<M, D, X><<<grid_t, TRANSPORT_THREADS, c->smem_transport, s>>>(c->T, c->G, P, cur->q, gen_n + g, c->d_head.p, c->qev.q, c->d_tally.p, c->d_cnt.p)
+        if (dbg) { if (mol) PMC_LAUNCH_TRANSPORT(1, true, false); else PMC_LAUNCH_TRANSPORT(0, true, false); }
+        else if (mol) { if (extra) PMC_LAUNCH_TRANSPORT(1, false, true); else PMC_LAUNCH_TRANSPORT(1, false, false); }
+        else { if (extra) PMC_LAUNCH_TRANSPORT(0, false, true); else PMC_LAUNCH_TRANSPORT(0, false, false); }
 #undef PMC_LAUNCH_TRANSPORT
+      }
+      c->timing.launches_total++; c->timing.launches_transport++;
+      if (P.dbg_out) return PMC_OK;
+      { Timer t(c, &c->timing.elastic_ms, profile);
+        event_kernel<<<grid_e, 256, 0, s>>>(c->T, c->G, P, c->qev.q, c->qel.q, c->qne.q, nxt->q, c->d_cnt.p);
+        elastic_kernel<<<grid_e, 256, 0, s>>>(c->T, P, c->qel.q, nxt->q, c->d_tally.p, c->d_cnt.p); }
+      { Timer t(c, &c->timing.inc_ms, profile);
+        inc_kernel<<<c->n_sm * 6, 128, 0, s>>>(c->T, P, c->qne.q, c->d_head.p + 1, nxt->q, rq, c->d_tally.p, c->d_cnt.p); }
+      { Timer t(c, &c->timing.evaporation_ms, profile);
+        evap_kernel<<<c->n_sm * 8, 128, 0, s>>>(c->T, P, rq, c->d_head.p + 2, nxt->q, c->d_tally.p, c->d_cnt.p); }
+      c->timing.launches_total += 4;
+      std::swap(cur, nxt);
     }
-    c->timing.launches_total++; c->timing.launches_transport++;
-    if (P.dbg_out) break;
-    { Timer t(c, &c->timing.elastic_ms, profile);
-      event_kernel<<<grid_e, 256, 0, s>>>(c->T, c->G, P, c->qev.q, c->qel.q, c->qne.q, nxt->q, c->d_cnt.p);
-      elastic_kernel<<<grid_e, 256, 0, s>>>(c->T, P, c->qel.q, nxt->q, c->d_tally.p, c->d_cnt.p); }
-    { Timer t(c, &c->timing.inc_ms, profile);
-      inc_kernel<<<c->n_sm * 6, 128, 0, s>>>(c->T, P, c->qne.q, c->d_head.p + 1, nxt->q, rq, c->d_tally.p, c->d_cnt.p); }
-    { Timer t(c, &c->timing.evaporation_ms, profile);
-      evap_kernel<<<c->n_sm * 8, 128, 0, s>>>(c->T, P, rq, c->d_head.p + 2, nxt->q, c->d_tally.p, c->d_cnt.p); }
-    c->timing.launches_total += 4;
-    CK(cudaMemcpyAsync(c->h_pinned, nxt->q.count, 4, cudaMemcpyDeviceToHost, s));
+    CK(cudaMemcpyAsync(c->h_pinned, cur->q.count, 4, cudaMemcpyDeviceToHost, s));
+    CK(cudaMemcpyAsync(c->h_pinned + 1, gen_n, GEN_SLOTS * 4, cudaMemcpyDeviceToHost, s));
     CK(cudaStreamSynchronize(s));
-    n_in = c->h_pinned[0];
-    if (n_in > c->qcap) return fail(c, PMC_E_CAPACITY, "particle queue overflow (raise chunk capacity / lower chunk_histories)");
-    std::swap(cur, nxt);
+    c->counters.n_host_waits++;
+    if (c->h_pinned[0] > c->qcap) return fail(c, PMC_E_CAPACITY, "particle queue overflow (raise chunk capacity / lower chunk_histories)");
+    if (c->h_pinned[0] == 0) break;
+    if (g >= GEN_SLOTS) return fail(c, PMC_E_UNSUPPORTED, "more than 64 generations of secondaries");
+    burst = GEN_MORE;
   }
+  for (int k = 0; k < g; ++k) if (c->h_pinned[1 + k] > 0) c->counters.n_generations++;
   return PMC_OK;
 }
 
@@ -593,9 +606,7 @@ static int simulate_impl(pmc_ctx *c, const pmc_spot *spots_in, int nspots, uint6
     { Timer t(c, &c->timing.sampler_ms, profile);
       sampler_kernel<<<(int)std::min<uint32_t>((nc + 255) / 256, (uint32_t)c->n_sm * 8), 256, 0, s>>>(c->T, c->G, c->d_spots.p, c->d_cdf.p, nspots, P, c->qa.q, c->d_cnt.p, air_rho, air_wf, air_ix0, air_zoa, air_tab); }
     c->timing.launches_total++;
-    CK(cudaMemcpyAsync(c->h_pinned, c->qa.q.count, 4, cudaMemcpyDeviceToHost, s));
-    CK(cudaStreamSynchronize(s));
-    rc = run_generations(c, P, std::min(c->h_pinned[0], c->qcap), profile); if (rc) return rc;
+    rc = run_generations(c, P, profile); if (rc) return rc;
   }
   if (!dbg_out) {                                                  // PAPER.md:L138 total and RMS dose per voxel
     { Timer t(c, &c->timing.statistics_ms, profile);

@@ -286,9 +286,12 @@ __device__ __forceinline__ void deposit(float *tally, uint32_t tvox, float e, bo
 // leaves the grid or reaches a discrete nuclear event, then refills from the queue (warp-aggregated fetch).
 // Particles that reach an event are appended to the elastic or non-elastic queue; nothing else is written back.
 #ifndef PMC_TRANSPORT_BLOCKS
-#define PMC_TRANSPORT_BLOCKS 3
+#define PMC_TRANSPORT_BLOCKS 4
 #endif
-constexpr int TRANSPORT_THREADS = 256, TRANSPORT_BLOCKS_PER_SM = PMC_TRANSPORT_BLOCKS;
+#ifndef PMC_TRANSPORT_THREADS
+#define PMC_TRANSPORT_THREADS 224
+#endif
+constexpr int TRANSPORT_THREADS = PMC_TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM = PMC_TRANSPORT_BLOCKS;
 
 // distance along one axis to the face the particle is heading for (voxel-local r in [0, size], inv = 1/d); BIG if d = 0
 __device__ __forceinline__ float axis_dist(float r, float d, float size) {
@@ -314,8 +317,12 @@ __device__ __forceinline__ V3 rotate(V3 d, float st, float ct, float sp, float c
 // carries neither its registers nor its branches.
 // EXTRA: LET_d scoring, per-spot dose influence or warp-merged dose atomics are on (the plain kernel carries none of it)
 template <int MCS_MODEL, bool DBG, bool EXTRA>
-__global__ void __launch_bounds__(TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM) transport_kernel(Tables T, Grid G, RunParams P, Queue in, uint32_t n_in,
+__global__ void __launch_bounds__(TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM) transport_kernel(Tables T, Grid G, RunParams P, Queue in, uint32_t *gen_n,
                                                            uint32_t *head, Queue q_ev, float *tally, Counters *cnt) {
+  // the generation's particle count stays on the device (the host does not wait for it): an empty generation ends here
+  const uint32_t n_in = min(*in.count, in.cap);
+  if (blockIdx.x == 0 && threadIdx.x == 0) *gen_n = n_in;
+  if (n_in == 0u) return;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   // shared-memory staging of the stopping-power/range and cross-section tables (PAPER.md:L144 used textures): spline
   // knots interleaved with their second derivatives (one 8-byte load per knot), ln R(ln E) first, then ln E(ln R), then
