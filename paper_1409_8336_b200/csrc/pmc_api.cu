@@ -105,7 +105,7 @@ struct pmc_ctx {
   DevBuf<uint32_t> d_head; DevBuf<Counters> d_cnt; DevBuf<float> d_tally, d_out, d_let;
   bool score_let = false, have_let = false;
   DevBuf<int32_t> d_roimap, d_roivox; uint32_t n_roi = 0; float *dij_dev = nullptr; uint64_t dij_cap = 0;
-  DevBuf<SpotDev> d_spots; DevBuf<double> d_cdf;
+  DevBuf<SpotDev> d_spots; DevBuf<double> d_cdf; DevBuf<uint32_t> d_guide;
   DevBuf<SecRec> d_slots; DevBuf<uint32_t> d_counts; DevBuf<unsigned long long> d_base; DevBuf<ResRec> d_res;
   DevBuf<GammaOffset> d_goff; DevBuf<unsigned long long> d_gscr;
   uint32_t *h_pinned = nullptr;     // pinned readback word(s)
@@ -277,7 +277,12 @@ int prepare_spots(pmc_ctx *c, const pmc_spot *spots, int nspots) {
     acc += s.weight; cdf[i] = acc / tot;
   }
   cdf[nspots - 1] = 1.0;
-  CK(c->d_spots.upload(sd, c->stream)); CK(c->d_cdf.upload(cdf, c->stream));
+  std::vector<uint32_t> guide(SPOT_GUIDE + 1);
+  for (int j = 0, i = 0; j <= SPOT_GUIDE; ++j) {       // first spot whose cumulative weight reaches j / SPOT_GUIDE
+    while (i < nspots - 1 && cdf[i] < (double)j / SPOT_GUIDE) ++i;
+    guide[j] = (uint32_t)i;
+  }
+  CK(c->d_spots.upload(sd, c->stream)); CK(c->d_cdf.upload(cdf, c->stream)); CK(c->d_guide.upload(guide, c->stream));
   return PMC_OK;
 }
 
@@ -604,7 +609,7 @@ static int simulate_impl(pmc_ctx *c, const pmc_spot *spots_in, int nspots, uint6
     P.b_over_n = (float)((double)B / (double)n); P.inv_nx = 1.0f / (float)c->G.nx; P.inv_ny = 1.0f / (float)c->G.ny;
     CK(cudaMemsetAsync(c->qa.q.count, 0, 4, s));
     { Timer t(c, &c->timing.sampler_ms, profile);
-      sampler_kernel<<<(int)std::min<uint32_t>((nc + 255) / 256, (uint32_t)c->n_sm * 8), 256, 0, s>>>(c->T, c->G, c->d_spots.p, c->d_cdf.p, nspots, P, c->qa.q, c->d_cnt.p, air_rho, air_wf, air_ix0, air_zoa, air_tab); }
+      sampler_kernel<<<(int)std::min<uint32_t>((nc + 255) / 256, (uint32_t)c->n_sm * 8), 256, 0, s>>>(c->T, c->G, c->d_spots.p, c->d_cdf.p, c->d_guide.p, nspots, P, c->qa.q, c->d_cnt.p, air_rho, air_wf, air_ix0, air_zoa, air_tab); }
     c->timing.launches_total++;
     rc = run_generations(c, P, profile); if (rc) return rc;
   }

@@ -5,6 +5,7 @@
 
 namespace pmc {
 
+constexpr int SPOT_GUIDE = 4096;  // entries of the guide table of the spot CDF
 struct SpotDev {                 // pmc_spot, prepared on the host (axis normalised, transverse basis built)
   double pos[3]; double ax[3], ex[3], ey[3];
   double e, sigma_e, sx, sy, divx, divy;
@@ -137,7 +138,7 @@ __device__ __forceinline__ float mean_loss(const Tables &T, const float *lnE, co
 // ------------------------------------------------------------------ K1: beam-spot sampler (Reading R2)
 __device__ __forceinline__ double u01d(uint32_t x) { return ((double)x + 0.5) * (1.0 / 4294967296.0); }
 
-__global__ void __launch_bounds__(256) sampler_kernel(Tables T, Grid G, const SpotDev *spots, const double *cdf, int nspots,
+__global__ void __launch_bounds__(256) sampler_kernel(Tables T, Grid G, const SpotDev *spots, const double *cdf, const uint32_t *guide, int nspots,
                                                      RunParams P, Queue out, Counters *cnt, float air_rho, float air_wf,
                                                      float air_inv_x0, float air_zoa, int air_table) {
   // Block-stride loop (same trip count for every thread of a block) so that a block makes ONE allocation in the
@@ -151,11 +152,13 @@ __global__ void __launch_bounds__(256) sampler_kernel(Tables T, Grid G, const Sp
   bool push = false; Particle p{};
   if (i < P.n) {
     const uint64_t hist = P.hist0 + i;
-    Rng g; g.init(P.seed, hist, 0u, 0u);
+    RngK gk; gk.init(hist, 0u, 0u);
+    RngKRef g{gk, P.rk};
     uint4 r = g.next4();
-    // spot ~ weight: first cdf entry >= u
+    // spot ~ weight: first cdf entry >= u; guide[j] = first entry >= j / SPOT_GUIDE brackets the search to a spot or two
     const double us = u01d(r.x);
-    int lo = 0, hi = nspots - 1;
+    const int gj = min((int)(us * SPOT_GUIDE), SPOT_GUIDE - 1);
+    int lo = (int)guide[gj], hi = min((int)guide[gj + 1], nspots - 1);
     while (lo < hi) { int mid = (lo + hi) >> 1; if (cdf[mid] < us) lo = mid + 1; else hi = mid; }
     const SpotDev sp = spots[lo];
     // Gaussian deviates in fp32 (relative error 1e-7 of sigma), accumulated onto the fp64 spot position
@@ -179,7 +182,8 @@ __global__ void __launch_bounds__(256) sampler_kernel(Tables T, Grid G, const Sp
       double t0 = 0, t1 = 1e300;
       for (int k = 0; k < 3; ++k) {
         if (dd[k] == 0) { if (o[k] < 0 || o[k] > size[k]) return false; continue; }
-        double ta = (0 - o[k]) / dd[k], tb = (size[k] - o[k]) / dd[k];
+        const double inv = 1.0 / dd[k];
+        double ta = (0 - o[k]) * inv, tb = (size[k] - o[k]) * inv;
         if (ta > tb) { double s = ta; ta = tb; tb = s; }
         t0 = fmax(t0, ta); t1 = fmin(t1, tb);
       }
@@ -221,7 +225,7 @@ __global__ void __launch_bounds__(256) sampler_kernel(Tables T, Grid G, const Sp
       }
       p.r = {loc[0], loc[1], loc[2]}; p.d = unit(V3{(float)dir[0], (float)dir[1], (float)dir[2]}); p.e = (float)E;
       p.vox = (idx[2] * G.ny + idx[1]) * G.nx + idx[0];
-      p.hist = i; p.pid = 0u; p.blk = g.blk; p.aux = (uint32_t)lo << 8;
+      p.hist = i; p.pid = 0u; p.blk = gk.blk; p.aux = (uint32_t)lo << 8;
       push = true;
     }
   }
