@@ -750,6 +750,30 @@ def test_call_order_and_argument_errors(tables):
     p.close()
 
 
+def test_scratch_comes_from_the_callers_allocator(tables):
+    """pmc_create_with_allocator: with the binding's default the queues and tallies are PyTorch allocations
+    (torch sees them, and they return to its pool when the context is destroyed); with torch_allocator=False they are
+    plain cudaMalloc and torch sees nothing.  Same result either way."""
+    from paper_1409_8336_b200 import Pmc
+    w = inputs.workload("c1")
+    hu = torch.as_tensor(w["hu"], device="cuda")
+    doses = []
+    for use_torch in (True, False):
+        torch.cuda.synchronize(); torch.cuda.empty_cache()
+        before = torch.cuda.memory_allocated()
+        p = Pmc(0, torch_allocator=use_torch)
+        p.load_physics_tables(tables); p.set_hu_materials(w["materials"]); p.load_ct(hu, w["vox"])
+        d, _ = p.simulate(w["spots"], 20_000, 5)
+        doses.append(d.clone())
+        held = torch.cuda.memory_allocated() - before - 3 * d.numel() * 4          # minus dose, sigma and the clone
+        # six queues of 12 words x 1.25 x 20000 histories + 10 tallies of 250000 voxels = about 17 MB
+        assert (held > 12e6) if use_torch else (abs(held) < 1e6), (use_torch, held)
+        p.close(); del d
+        torch.cuda.synchronize()
+        assert torch.cuda.memory_allocated() - before < 4e6                      # only the result tensors are left
+    assert torch.equal(doses[0], doses[1]) or torch.allclose(doses[0], doses[1], rtol=2e-4, atol=1e-16)
+
+
 def test_streams_are_schedule_independent(pm, tables):
     """Philox streams are keyed per history (north_star): sub-group size, history offset and the stream the context
     runs on change the schedule, not the physics.  Integer counters are identical; float tallies agree up to the
