@@ -435,15 +435,16 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM) tr
       // boundary step: the neighbour voxel (done before the energy loss, whose registers it would otherwise compete with;
       // if the proton stops in this step the advanced index is simply not used)
       bool exits = false;
-      if (cls == 1) {
-        const bool up = (ax2 == 0 ? dnew.x : ax2 == 1 ? dnew.y : dnew.z) > 0.f;
+      if (cls == 1) {                    // selects, not branches: the lanes of a warp leave through different faces
+        const bool a0 = ax2 == 0, a1 = ax2 == 1;
+        const bool up = (a0 ? dnew.x : a1 ? dnew.y : dnew.z) > 0.f;
         const int sg2 = up ? 1 : -1;
-        int nidx, nmax;
-        if (ax2 == 0) { ix += sg2; nidx = ix; nmax = G.nx; p.r.x = up ? 0.f : szx; }
-        else if (ax2 == 1) { iy += sg2; nidx = iy; nmax = G.ny; p.r.y = up ? 0.f : szy; }
-        else { iz += sg2; nidx = iz; nmax = G.nz; p.r.z = up ? 0.f : szz; }
-        exits = nidx < 0 || nidx >= nmax;
-        if (!exits) p.vox = (iz * G.ny + iy) * G.nx + ix;
+        ix += a0 ? sg2 : 0; iy += a1 ? sg2 : 0; iz += (a0 || a1) ? 0 : sg2;
+        const float face = up ? 0.f : (a0 ? szx : a1 ? szy : szz);
+        p.r.x = a0 ? face : p.r.x; p.r.y = a1 ? face : p.r.y; p.r.z = (a0 || a1) ? p.r.z : face;
+        const int nidx = a0 ? ix : a1 ? iy : iz, nmax = a0 ? G.nx : a1 ? G.ny : G.nz;
+        exits = (unsigned)nidx >= (unsigned)nmax;
+        p.vox += sg2 * (a0 ? 1 : a1 ? G.nx : G.nx * G.ny);
       }
       // ---- 6. energy loss from the range table (Eq.2) + straggling (L61)
       float loss;
