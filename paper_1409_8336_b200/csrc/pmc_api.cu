@@ -74,7 +74,6 @@ struct QueueMem {
     q.count = count.p; q.cap = cap;
     return cudaSuccess;
   }
-  void release() { f.release(); vox.release(); u.release(); count.release(); q = Queue{}; }
 };
 
 }  // namespace
