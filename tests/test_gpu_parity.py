@@ -76,20 +76,46 @@ def test_range_tables_match_oracle(pm, oracle_c1, table):
 
 
 # ------------------------------------------------------------------ S5 straggling: cumulants and distribution
-@pytest.mark.parametrize("e_mev,rho_l", [(230.0, 0.1), (150.0, 0.2), (70.0, 0.2), (30.0, 0.25), (5.0, 0.02)])
+@pytest.mark.parametrize("e_mev,rho_l", [(230.0, 0.1), (150.0, 0.2), (70.0, 0.2), (30.0, 0.25), (5.0, 0.02), (200.0, 0.0003)])
 def test_straggling_distribution(pm, oracle_c1, e_mev, rho_l):
     zoa, n = 0.555087, 400_000
-    mean = 0.5 * rho_l * 5.0
+    mean = 0.5 * rho_l * 5.0 + (0.01 if rho_l < 0.001 else 0.0)          # (the 3 um step: keep the loss clear of the clamp at 0)
     g = pm.straggle(e_mev, mean, rho_l, zoa, n, 11).astype(np.float64)
     o = oracle_c1.straggle(e_mev, mean, rho_l, zoa, n, 12)
     sd = o.std()
     assert abs(g.mean() - o.mean()) < 5 * sd / np.sqrt(n) * np.sqrt(2) + 1e-6
-    assert abs(g.var() / o.var() - 1) < 0.03
+    # (sampling error of a variance: sqrt((kurtosis - 1)/n); the 3 um step is Landau-like, kurtosis ~ 1/(3 kappa) = 2000)
+    kurt = np.mean((o - o.mean()) ** 4) / o.var() ** 2
+    assert abs(g.var() / o.var() - 1) < max(0.03, 4 * np.sqrt(2 * (kurt - 1) / n))
     m3g, m3o = np.mean((g - g.mean()) ** 3), np.mean((o - o.mean()) ** 3)
-    assert abs(m3g - m3o) < 0.15 * abs(m3o) + 0.02 * sd ** 3
+    if kurt < 100:
+        assert abs(m3g - m3o) < 0.15 * abs(m3o) + 0.02 * sd ** 3
     # quantiles of the bulk agree to a small fraction of the width
     q = np.array([0.01, 0.05, 0.25, 0.5, 0.75, 0.95, 0.99])
     assert np.max(np.abs(np.quantile(g, q) - np.quantile(o, q))) < 0.03 * sd
+
+
+@pytest.mark.parametrize("e_mev,rho_l", [(230.0, 0.1), (150.0, 0.2), (70.0, 0.2), (30.0, 0.25), (200.0, 0.02)])
+def test_straggling_against_the_vavilov_distribution_itself(pm, e_mev, rho_l):
+    """The CUDA sampler (hard collisions + shifted-gamma soft part, Reading R4) against Vavilov's distribution computed from
+    its characteristic function (tests/vavilov_ref.py) - a reference that involves neither the oracle nor any sampling.
+    kappa from 0.011 to 5.3; Kolmogorov distance below 0.6 % (4e5 samples resolve 0.3 %; measured 0.1-0.3 %).  Thinner steps
+    (xi below a few keV) are outside this comparison: Reading R4 lumps the collisions below 1 keV into a Gaussian of
+    variance xi x 1 keV on BOTH sides, which is then wider than Vavilov's own sub-keV structure (0.3 keV - immaterial for the
+    dose); there the CUDA sampler is compared with the oracle (test_straggling_distribution, the 3 um case)."""
+    from scipy import stats
+    from vavilov_ref import vavilov_cdf
+    from inputs.physics_tables import M_P, M_E, K_BETHE
+    g_ = 1 + e_mev / M_P; b2 = 1 - 1 / g_ ** 2
+    tmax = 2 * M_E * b2 * g_ * g_ / (1 + 2 * g_ * M_E / M_P + (M_E / M_P) ** 2)
+    xi = 0.5 * K_BETHE * 0.555087 * rho_l / b2
+    kappa = xi / tmax
+    mean_loss = 8.0 * xi + 2.0 * np.sqrt(xi * tmax) + 0.5
+    x = pm.straggle(e_mev, mean_loss, rho_l, 0.555087, 400_000, 123).astype(np.float64)
+    y, cdf = vavilov_cdf(kappa, b2)
+    d = stats.kstest((x - mean_loss) / tmax, lambda t: np.interp(t, y, cdf)).statistic
+    print(f"kappa {kappa:.3g}: Kolmogorov distance to Vavilov {d:.4f}")
+    assert d < 0.006, (kappa, d)
 
 
 # ------------------------------------------------------------------ S10 nuclear elastic (Eq.3) and p-p

@@ -679,3 +679,27 @@ def test_moliere_single_step_core_and_rutherford_tail(tables):
     o.set_option("mcs_model", 1)
     b = o.first_steps(inputs.plan_single_spot((5.1, 5.1, 0.0), 150.0, 0.0), 2000, 7, 3)
     assert np.array_equal(a, b)
+
+
+# ------------------------------------------------------------------ straggling: the whole Vavilov distribution (reading R4)
+from vavilov_ref import vavilov_cdf as _vavilov_cdf
+
+
+@pytest.mark.parametrize("e_mev,rho_l", [(230.0, 0.1), (150.0, 0.2), (70.0, 0.2), (30.0, 0.25), (200.0, 0.02)])
+def test_straggling_is_vavilov_distributed(oracle_c1, e_mev, rho_l):
+    """The sampled losses against Vavilov's distribution itself (not only its first three cumulants), computed from the
+    characteristic function of the collision process.  kappa = 0.01 ... 5.3 here.  Fails if the hard-collision spectrum,
+    the thinning with (1 - beta^2 T/Tmax), the Poisson number or the re-centring on the mean are wrong (each shifts or
+    reshapes the curve by far more than the 0.4 % resolution of the Kolmogorov distance at 4e5 samples)."""
+    xi, tmax, b2 = _straggle_params(e_mev, rho_l)
+    kappa = xi / tmax
+    assert 0.004 < kappa < 8
+    mean_loss = 8.0 * xi + 2.0 * np.sqrt(xi * tmax) + 0.5     # far enough from the clamp at zero
+    n = 400_000
+    x = oracle_c1.straggle(e_mev, mean_loss, rho_l, 0.555087, n, 99)
+    y, cdf = _vavilov_cdf(kappa, b2)
+    d = stats.kstest((x - mean_loss) / tmax, lambda t: np.interp(t, y, cdf)).statistic
+    assert d < 0.004, (kappa, d)
+    # and the same curve reproduces the textbook moments (a check of the reference itself)
+    pdf = np.diff(cdf); yc = 0.5 * (y[1:] + y[:-1])
+    assert abs((pdf * yc).sum()) < 0.02 * np.sqrt(kappa) and (pdf * yc ** 2).sum() == pytest.approx(kappa * (1 - b2 / 2), rel=0.02)
