@@ -234,6 +234,13 @@ int sync_tables(pmc_ctx *c) {
   return PMC_OK;
 }
 
+// one launch instead of six memsets per generation: work-fetch heads and the counts of the queues the generation fills
+__global__ void reset_kernel(uint32_t *head4, uint32_t *a, uint32_t *b, uint32_t *c_, uint32_t *d, uint32_t *e) {
+  const int t = threadIdx.x;
+  if (t < 4) head4[t] = 0u;
+  else if (t == 4) *a = 0u; else if (t == 5) *b = 0u; else if (t == 6) *c_ = 0u; else if (t == 7) *d = 0u; else if (t == 8) *e = 0u;
+}
+
 // generations enqueued before the host first looks at a queue size, then per look; slots of the per-generation counts
 constexpr int GEN_BURST = 6, GEN_MORE = 2, GEN_SLOTS = 64;
 
@@ -330,9 +337,8 @@ int run_generations(pmc_ctx *c, RunParams P, bool profile) {
   int g = 0, burst = GEN_BURST;
   while (true) {
     for (int k = 0; k < burst && g < GEN_SLOTS; ++k, ++g) {
-      CK(cudaMemsetAsync(c->d_head.p, 0, 16, s)); CK(cudaMemsetAsync(nxt->q.count, 0, 4, s));
-      CK(cudaMemsetAsync(c->qel.q.count, 0, 4, s)); CK(cudaMemsetAsync(c->qne.q.count, 0, 4, s)); CK(cudaMemsetAsync(c->qres.q.count, 0, 4, s));
-      CK(cudaMemsetAsync(c->qev.q.count, 0, 4, s));
+      reset_kernel<<<1, 32, 0, s>>>(c->d_head.p, nxt->q.count, c->qel.q.count, c->qne.q.count, c->qres.q.count, c->qev.q.count);
+      c->timing.launches_total++;
       { Timer t(c, &c->timing.transport_ms, profile);
         const bool mol = c->T.mcs_model == 1, dbg = P.dbg_out != nullptr;
         const bool extra = !dbg && (P.let_num != nullptr || P.roi_map != nullptr || P.aggregate != 0 || P.skip_tally != 0);
