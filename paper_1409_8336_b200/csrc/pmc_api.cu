@@ -425,6 +425,9 @@ int pmc_create_with_allocator(pmc_ctx **out, int device, void *cuda_stream, pmc_
   c->allocator.alloc = alloc_fn; c->allocator.free = free_fn; c->allocator.user = user;
   for (DevBufBase *b : c->bufs) b->A = &c->allocator;
   c->device = device; c->stream = (cudaStream_t)cuda_stream;
+  float sq[NQ];                                   // square roots of the evaporation quadrature (pmc_nuclear.cuh: EVAP_SQ)
+  for (int i = 0; i < NQ; ++i) sq[i] = (float)std::sqrt((double)NQ - 0.5 - i);
+  if (cudaMemcpyToSymbol(EVAP_SQ, sq, sizeof(sq)) != cudaSuccess) { delete c; return PMC_E_CUDA; }
   cudaDeviceProp prop{};
   if (cudaGetDeviceProperties(&prop, device) == cudaSuccess) c->n_sm = prop.multiProcessorCount;
   *out = c;

@@ -275,8 +275,14 @@ __device__ bool chan_setup(const Tables &T, int Z, int A, float estar, double Mp
   c.A = 2.0f * LOG2E * sqrtf(Ad * 0.125f); c.B = ref * LOG2E;
   return true;
 }
-__device__ __forceinline__ float chan_f(const Chan &c, float e) {
-  return fmaf(c.s1, e, c.s0) * fex2(fmaf(c.A, fsqrt(c.emax - e), -c.B));
+// Midpoint i of the NQ bins of [emin, emax]: e_i = emin + (i + 1/2) de, emax - e_i = (NQ - 1/2 - i) de, so that
+// P(e_i) = (lin1 (i + 1/2) + lin0) 2^(Ade sqrt(NQ - 1/2 - i) - B) with the square roots a constant table (filled by
+// pmc_create): one MUFU and three FMAs per point.
+__constant__ float EVAP_SQ[NQ];
+struct ChanQ { float lin0, lin1, Ade, B; };
+__device__ __forceinline__ ChanQ chan_quad(const Chan &c, float de) { return {fmaf(c.s1, c.emin, c.s0), c.s1 * de, c.A * fsqrt(de), c.B}; }
+__device__ __forceinline__ float chan_f(const ChanQ &q, int i) {
+  return fmaf(q.lin1, (float)i + 0.5f, q.lin0) * fex2(fmaf(q.Ade, EVAP_SQ[i], -q.B));
 }
 struct Emission { int j; float ke; V3 dir; };
 // one emission from R (updated in place); returns false when no channel is open
@@ -290,9 +296,10 @@ __device__ bool evap_emit(const Tables &T, Residual &R, Rng &g, uint32_t mask, E
     Chan c;
     if (!((mask >> j) & 1u) || !chan_setup(T, R.Z, R.A, estar, R.mass_gs, j, ref, c)) continue;
     const float de = (c.emax - c.emin) * (1.0f / NQ);
+    const ChanQ q = chan_quad(c, de);
     float w = 0.f;
-#pragma unroll 8
-    for (int i = 0; i < NQ; ++i) w += chan_f(c, fmaf((float)i + 0.5f, de, c.emin));
+#pragma unroll
+    for (int i = 0; i < NQ; ++i) w += chan_f(q, i);
     width[j] = w * de; tot += width[j];
   }
   if (!(tot > 0.f)) return false;
@@ -303,7 +310,8 @@ __device__ bool evap_emit(const Tables &T, Residual &R, Rng &g, uint32_t mask, E
   Chan c; chan_setup(T, R.Z, R.A, estar, R.mass_gs, j, ref, c);
   const float de = (c.emax - c.emin) * (1.0f / NQ);
   float v = u01(r.y) * width[j] / de; int bin = NQ - 1;
-  for (int i = 0; i < NQ; ++i) { const float f = chan_f(c, fmaf((float)i + 0.5f, de, c.emin)); if (v < f) { bin = i; break; } v -= f; }
+  const ChanQ cq = chan_quad(c, de);
+  for (int i = 0; i < NQ; ++i) { const float f = chan_f(cq, i); if (v < f) { bin = i; break; } v -= f; }
   const float eps = c.emin + ((float)bin + u01(r.z)) * de;                  // total CM kinetic energy released
   // relativistic two-body decay of M* -> m_j + M_d* (isotropic in the nucleus rest frame, L79), fp64
   const uint4 r2 = g.next4();
