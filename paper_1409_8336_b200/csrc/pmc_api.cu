@@ -110,6 +110,7 @@ struct pmc_ctx {
   uint32_t *h_pinned = nullptr;     // pinned readback word(s)
   uint32_t qcap = 0;
   int n_sm = 148; size_t smem_transport = 0;
+  int inc_bpsm = 0, evap_bpsm = 0;     // resident blocks per SM of the two warp-synchronous engines (occupancy API)
   pmc_counters counters{}; pmc_timing timing{};
   cudaEvent_t ev[2] = {nullptr, nullptr};
   std::vector<cudaEvent_t> ev_pool; size_t ev_used = 0; std::vector<float *> ev_acc;
@@ -254,6 +255,11 @@ int ensure_scratch(pmc_ctx *c, uint64_t chunk) {
   CK(c->d_head.alloc(4 + GEN_SLOTS)); CK(c->d_cnt.alloc(1));
   if (!c->h_pinned) CK(cudaMallocHost(&c->h_pinned, 4 * (GEN_SLOTS + 4)));
   if (!c->ev[0]) { CK(cudaEventCreate(&c->ev[0])); CK(cudaEventCreate(&c->ev[1])); }
+  if (!c->inc_bpsm) {                  // persistent engines: exactly one wave of blocks
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->inc_bpsm, inc_kernel, 128, 0));
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->evap_bpsm, evap_kernel, 128, 0));
+    c->inc_bpsm = std::max(c->inc_bpsm, 1); c->evap_bpsm = std::max(c->evap_bpsm, 1);
+  }
   return PMC_OK;
 }
 
@@ -354,9 +360,9 @@ int run_generations(pmc_ctx *c, RunParams P, bool profile) {
         event_kernel<<<grid_e, 256, 0, s>>>(c->T, c->G, P, c->qev.q, c->qel.q, c->qne.q, nxt->q, c->d_cnt.p);
         elastic_kernel<<<grid_e, 256, 0, s>>>(c->T, P, c->qel.q, nxt->q, c->d_tally.p, c->d_cnt.p); }
       { Timer t(c, &c->timing.inc_ms, profile);
-        inc_kernel<<<c->n_sm * 6, 128, 0, s>>>(c->T, P, c->qne.q, c->d_head.p + 1, nxt->q, rq, c->d_tally.p, c->d_cnt.p); }
+        inc_kernel<<<c->n_sm * c->inc_bpsm, 128, 0, s>>>(c->T, P, c->qne.q, c->d_head.p + 1, nxt->q, rq, c->d_tally.p, c->d_cnt.p); }
       { Timer t(c, &c->timing.evaporation_ms, profile);
-        evap_kernel<<<c->n_sm * 8, 128, 0, s>>>(c->T, P, rq, c->d_head.p + 2, nxt->q, c->d_tally.p, c->d_cnt.p); }
+        evap_kernel<<<c->n_sm * c->evap_bpsm, 128, 0, s>>>(c->T, P, rq, c->d_head.p + 2, nxt->q, c->d_tally.p, c->d_cnt.p); }
       c->timing.launches_total += 4;
       std::swap(cur, nxt);
     }
