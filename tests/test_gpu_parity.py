@@ -245,6 +245,8 @@ def test_nonelastic_edge_cases(pm):
     with pytest.raises(PmcError) as e:                                    # hydrogen has no cascade
         pm.nonelastic(1, 1, 200.0, 10, 3)
     assert e.value.code == -5
+    sec, off = pm.nonelastic(8, 16, 200.0, 0, 3)                          # no events at all
+    assert len(sec) == 0 and len(off) == 1 and off[0] == 0
     # reproducible: same seed -> identical records; event i depends only on (seed, i)
     a, oa = pm.nonelastic(20, 40, 100.0, 5000, 9)
     b, ob_ = pm.nonelastic(20, 40, 100.0, 2500, 9)
@@ -724,6 +726,16 @@ def test_simulate_edge_cases(pm, tables):
     # oblique beam entering through a side face
     ob_ = inputs.plan_single_spot((-3.0, 5.0, 6.0), 100.0, 0.3, direction=(0.8, 0.0, 0.6))
     _dose_parity(pm, o, w["hu"], w["vox"], w["materials"], ob_, 60_000, 8, check_range=False)
+    # the smallest grid there is: one voxel, everything the protons lose before they leave is in it
+    one = np.zeros((1, 1, 1), dtype=np.int16)
+    pm.load_ct(torch.as_tensor(one, device="cuda"), (0.5, 0.5, 0.5)); o.load_ct(one, (0.5, 0.5, 0.5))
+    mid = inputs.plan_single_spot((0.25, 0.25, 0.0), 150.0, 0.0)
+    d1, _ = pm.simulate(mid, 20_000, 9); c1 = pm.counters()
+    do1, _ = o.simulate(mid, 20_000, 10); co1 = o.counters()
+    assert d1.shape == (1, 1, 1) and _ledger_closes(c1)
+    assert abs(c1["e_deposit"] / co1["e_deposit"] - 1) < 0.02 and abs(c1["e_escape"] / co1["e_escape"] - 1) < 1e-3
+    assert abs(float(d1[0, 0, 0]) / do1[0, 0, 0] - 1) < 0.02
+    pm.load_ct(torch.as_tensor(w["hu"], device="cuda"), w["vox"]); o.load_ct(w["hu"], w["vox"])
     # zero-weight and bad inputs
     bad = w["spots"].copy(); bad[0, 12] = 0.0
     with pytest.raises(PmcError):
