@@ -290,10 +290,10 @@ __device__ __forceinline__ void deposit(float *tally, uint32_t tvox, float e, bo
 // leaves the grid or reaches a discrete nuclear event, then refills from the queue (warp-aggregated fetch).
 // Particles that reach an event are appended to the elastic or non-elastic queue; nothing else is written back.
 #ifndef PMC_TRANSPORT_BLOCKS
-#define PMC_TRANSPORT_BLOCKS 4
+#define PMC_TRANSPORT_BLOCKS 1
 #endif
 #ifndef PMC_TRANSPORT_THREADS
-#define PMC_TRANSPORT_THREADS 224
+#define PMC_TRANSPORT_THREADS 896
 #endif
 constexpr int TRANSPORT_THREADS = PMC_TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM = PMC_TRANSPORT_BLOCKS;
 
