@@ -349,6 +349,7 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM) tr
   const int lane = threadIdx.x & 31;
   bool active = false, exhausted = false;
   Particle p; int ix = 0, iy = 0, iz = 0, nstep = 0; float path = 0.f; uint32_t tbase = 0;
+  int hu = 0;                           // HU of the current voxel: fetched when the voxel changes, a step ahead of its use
   uint32_t c_steps = 0;                 // per-lane partial sums (a lane sees < 1e7 steps and < 1e4 MeV): 32-bit is enough
   float c_dep = 0.f;
   const bool nuclear = T.opt_el || T.opt_ne;
@@ -365,7 +366,7 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM) tr
         if (idx < n_in) {
           p = queue_load(in, idx);
           int t; divmod(p.vox, G.nx, P.inv_nx, t, ix); divmod(t, G.ny, P.inv_ny, iz, iy);
-          active = true; nstep = 0; path = 0.f; tbase = batch_base(P, p.hist);
+          active = true; nstep = 0; path = 0.f; tbase = batch_base(P, p.hist); hu = G.hu[p.vox];
         } else exhausted = true;
       }
     }
@@ -378,7 +379,6 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM) tr
       RngK gk; gk.init(hid, p.pid, p.blk);
       RngKRef g{gk, P.rk};
       // ---- material of the current voxel
-      const int hu = G.hu[p.vox];
       const MatBin &m = s_bins[s_lut[min(max(hu - T.hu_lut_lo, 0), T.hu_lut_n - 1)]];
       const float rho = fmaf(m.slope, fminf(fmaxf((float)hu - m.hu_lo, 0.f), m.dhu), m.rho_lo), wf = rho * m.wet;
       c_steps++;
@@ -445,6 +445,7 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM) tr
         const int nidx = a0 ? ix : a1 ? iy : iz, nmax = a0 ? G.nx : a1 ? G.ny : G.nz;
         exits = (unsigned)nidx >= (unsigned)nmax;
         p.vox += sg2 * (a0 ? 1 : a1 ? G.nx : G.nx * G.ny);
+        if (!exits) hu = G.hu[p.vox];
       }
       // ---- 6. energy loss from the range table (Eq.2) + straggling (L61)
       float loss;
