@@ -95,7 +95,7 @@ struct pmc_ctx {
   std::vector<HostMat> mats;
   // device tables
   DevBuf<float> d_lnR, d_lnR2, d_lnE, d_lnE2, d_sel, d_sne, d_sigbin, d_ek, d_ec;
-  DevBuf<double> d_mass; DevBuf<MatBin> d_bins; DevBuf<uint8_t> d_lut; DevBuf<Nucleus> d_nuc, d_nuc1;
+  DevBuf<double> d_mass; DevBuf<MatBin> d_bins; DevBuf<uint8_t> d_lut; DevBuf<int2> d_lut2; DevBuf<Nucleus> d_nuc, d_nuc1;
   std::vector<Nucleus> h_nuc;
   Tables T{}; Grid G{}; double origin[3] = {0, 0, 0};
   DevBuf<int16_t> d_hu_own;
@@ -220,10 +220,22 @@ int sync_tables(pmc_ctx *c) {
     std::vector<uint8_t> lut((size_t)(hi - lo + 1));
     for (int hu = lo, b = 0; hu <= hi; ++hu) { while (b < nb - 1 && hu >= c->mats[b].b.hu_hi) ++b; lut[hu - lo] = (uint8_t)b; }
     T.hu_lut_lo = lo; T.hu_lut_n = (int)lut.size();
+    // the same table with the density of every HU value beside its bin (step kernel: one 8-byte load instead of the bin's
+    // density line); the first and the last bin have one entry each, exact only if their density does not depend on HU
+    std::vector<int2> lut2(lut.size());
+    for (int hu = lo; hu <= hi; ++hu) {
+      const pmc_hu_bin &h = c->mats[lut[hu - lo]].b;
+      const int hh = std::min(std::max(hu, h.hu_lo), h.hu_hi);
+      const float rho = (float)(h.rho_lo + (h.rho_hi - h.rho_lo) * ((double)hh - h.hu_lo) / ((double)h.hu_hi - h.hu_lo));
+      int bits; std::memcpy(&bits, &rho, 4);
+      lut2[hu - lo] = make_int2(bits, (int)lut[hu - lo]);
+    }
+    T.lut_ends_vary = (c->mats.front().b.rho_lo != c->mats.front().b.rho_hi || c->mats.back().b.rho_lo != c->mats.back().b.rho_hi) ? 1 : 0;
+    CK(c->d_lut2.upload(lut2, s)); T.hu_lut2 = c->d_lut2.p;
     CK(c->d_bins.upload(bins, s)); CK(c->d_sigbin.upload(sig, s)); CK(c->d_lut.upload(lut, s));
     T.bins = c->d_bins.p; T.sig_bin = c->d_sigbin.p; T.hu_lut = c->d_lut.p;
     c->smem_transport = ((size_t)2 * c->n_sr * c->n_e + (size_t)2 * c->n_sr * c->n_r + (size_t)nb * c->n_e) * 4 + (size_t)nb * sizeof(MatBin) +
-                        lut.size() + 16;
+                        lut.size() * sizeof(int2) + 32;
     if (c->smem_transport > 200 * 1024) return fail(c, PMC_E_UNSUPPORTED, "tables too large for shared-memory staging");
 #define PMC_SMEM_ATTR(M, D, X) CK(cudaFuncSetAttribute(transport_kernel<M, D, X>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_transport))
     PMC_SMEM_ATTR(0, false, false); PMC_SMEM_ATTR(0, false, true); PMC_SMEM_ATTR(1, false, false); PMC_SMEM_ATTR(1, false, true);

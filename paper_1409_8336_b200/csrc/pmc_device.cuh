@@ -148,6 +148,8 @@ struct Tables {
   const float *sig_bin;         // [nbins][n_e] total macroscopic cross-section per unit density, cm^2/g
   const MatBin *bins;           // [nbins]
   const uint8_t *hu_lut;        // [hu_lut_n] HU -> bin
+  const int2 *hu_lut2;          // [hu_lut_n] HU -> {density as float bits, bin}: one 8-byte load in the step kernel
+  int lut_ends_vary;            // the first or last bin (one table entry each) has a density that depends on HU
   const Nucleus *nuc;           // [n_elem]
   const double *mass;           // [zdim][adim]
   const float *evap_k, *evap_c; // [6][zdim]

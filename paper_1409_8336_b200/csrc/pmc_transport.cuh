@@ -330,18 +330,18 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM) tr
   extern __shared__ __align__(16) unsigned char smem_raw[];
   // shared-memory staging of the stopping-power/range and cross-section tables (PAPER.md:L144 used textures): spline
   // knots interleaved with their second derivatives (one 8-byte load per knot), ln R(ln E) first, then ln E(ln R), then
-  // Sigma/rho per HU bin, the HU bins and the HU -> bin table; MatBin holds each bin's offsets into these arrays
+  // Sigma/rho per HU bin, the HU bins and the HU -> {density, bin} table; MatBin holds each bin's offsets into these arrays
   float2 *s_R = reinterpret_cast<float2 *>(smem_raw);
   float2 *s_E = s_R + T.n_sr * T.n_e;
   float *s_sig = reinterpret_cast<float *>(s_E + T.n_sr * T.n_r);
   MatBin *s_bins = reinterpret_cast<MatBin *>(s_sig + T.nbins * T.n_e);
-  uint8_t *s_lut = reinterpret_cast<uint8_t *>(s_bins + T.nbins);
+  int2 *s_lut = reinterpret_cast<int2 *>(reinterpret_cast<unsigned char *>(s_bins + T.nbins) + ((8 - (T.nbins * (int)sizeof(MatBin)) % 8) % 8));
   for (int i = threadIdx.x; i < T.n_sr * T.n_e; i += blockDim.x) s_R[i] = make_float2(T.lnR[i], T.lnR2[i]);
   for (int i = threadIdx.x; i < T.n_sr * T.n_r; i += blockDim.x) s_E[i] = make_float2(T.lnE[i], T.lnE2[i]);
   for (int i = threadIdx.x; i < T.nbins * T.n_e; i += blockDim.x) s_sig[i] = T.sig_bin[i];
   for (int i = threadIdx.x; i < T.nbins * (int)(sizeof(MatBin) / 4); i += blockDim.x)
     reinterpret_cast<uint32_t *>(s_bins)[i] = reinterpret_cast<const uint32_t *>(T.bins)[i];
-  for (int i = threadIdx.x; i < T.hu_lut_n; i += blockDim.x) s_lut[i] = T.hu_lut[i];
+  for (int i = threadIdx.x; i < T.hu_lut_n; i += blockDim.x) s_lut[i] = T.hu_lut2[i];
   __syncthreads();
   const float *s_f = reinterpret_cast<const float *>(smem_raw);   // every table offset in MatBin counts floats from here
 
@@ -379,8 +379,12 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM) tr
       RngK gk; gk.init(hid, p.pid, p.blk);
       RngKRef g{gk, P.rk};
       // ---- material of the current voxel
-      const MatBin &m = s_bins[s_lut[min(max(hu - T.hu_lut_lo, 0), T.hu_lut_n - 1)]];
-      const float rho = fmaf(m.slope, fminf(fmaxf((float)hu - m.hu_lo, 0.f), m.dhu), m.rho_lo), wf = rho * m.wet;
+      const int li = min(max(hu - T.hu_lut_lo, 0), T.hu_lut_n - 1);
+      const int2 le = s_lut[li];                                  // {density of this HU, bin}
+      const MatBin &m = s_bins[le.y];
+      float rho = __int_as_float(le.x);
+      if (T.lut_ends_vary && (li == 0 || li == T.hu_lut_n - 1)) rho = fmaf(m.slope, fminf(fmaxf((float)hu - m.hu_lo, 0.f), m.dhu), m.rho_lo);
+      const float wf = rho * m.wet;
       c_steps++;
       // draws of the step: r.x nuclear distance, r.y hinge (upper half), r.z and r.w (upper half) the MCS deflection; the
       // lower halves of r.y and r.w go to the straggling sampler
