@@ -764,6 +764,30 @@ def test_ragged_grid_and_clamped_hu(pm, tables):
     assert cg["e_air"] > 0 and abs(cg["e_air"] / co["e_air"] - 1) < 0.02
 
 
+def test_density_varies_inside_the_first_and_last_hu_bin(pm, tables):
+    """Two water-like HU bins whose density is linear in HU (rho(HU) inside a bin), with HU values spread over
+    both and beyond both ends of the table: the step kernel's per-HU density table holds one entry for each of the two end
+    bins and must fall back to the bin's own line there."""
+    water = inputs.make_materials_c1()[1]
+    lo = dict(water, hu_lo=-600, hu_hi=0, rho_lo=0.4, rho_hi=1.0)
+    hi = dict(water, hu_lo=0, hu_hi=1000, rho_lo=1.0, rho_hi=1.8)
+    mats = [lo, hi]
+    nz, ny, nx = 80, 21, 21
+    hu = np.zeros((nz, ny, nx), dtype=np.int16)
+    for k in range(nz):
+        hu[k] = [-900, -500, -250, -1, 0, 300, 700, 999, 1500, -100][k % 10]      # -900 and 1500 are clamped to the end bins
+    vox = (0.2, 0.2, 0.2)
+    o = _setup(pm, tables, mats, hu, vox)
+    spot = inputs.plan_single_spot((2.1, 2.1, 0.0), 140.0, 0.3)
+    dg, sg, do, so, cg, co = _dose_parity(pm, o, hu, vox, mats, spot, 400_000, 71, seed_o=72)
+    rho = _density(hu, mats)
+    assert rho.min() == pytest.approx(0.4) and rho.max() == pytest.approx(1.8)
+    for val in (-900, -250, 700, 1500):                                            # energy deposited per HU value
+        m = hu == val
+        a, b = (dg * rho)[m].sum(), (do * rho)[m].sum()
+        assert b > 0 and abs(a / b - 1) < 1e-2, (val, a, b)
+
+
 def test_call_order_and_argument_errors(tables):
     from paper_1409_8336_b200 import Pmc, PmcError
     p = Pmc(0)
