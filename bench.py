@@ -54,8 +54,8 @@ ALGO_INST_PER_STEP = float(sum(ALGO_ITEMS.values()))
 # (profiles/r02_transport_full.md; NOT measured in this run): DRAM bytes per history, executed thread-instructions per
 # condensed step, active lanes per warp instruction, issue-slot utilisation.
 NCU_CAPTURE = {"source": "profiles/r02_transport_full.md (one-off ncu capture, not measured in this run)",
-               "dram_bytes_per_history_c4": 78.0, "executed_thread_inst_per_step": 635.0, "lanes_per_warp_inst": 29.3,
-               "issue_slot_utilisation_pct": 79.8}
+               "dram_bytes_per_history_c4": 79.3, "executed_thread_inst_per_step": 634.0, "lanes_per_warp_inst": 29.2,
+               "issue_slot_utilisation_pct": 81.6}
 ISSUE_LANES_PER_SM_PER_CLK = 128.0     # 4 schedulers x 32 lanes
 N_SM = 148
 
