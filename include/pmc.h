@@ -209,6 +209,33 @@ int  pmc_gamma_index(pmc_ctx *ctx, const float *ref_dev, const float *eval_dev, 
                      double dx_cm, double dy_cm, double dz_cm, double dd_frac, double dta_cm, double low_dose_frac,
                      double search_cm, float *gamma_dev, double *pass_rate_host);
 
+/* The same gamma index for callers that must not allocate device memory.  pmc_gamma_index obtains its working memory
+ * (the offsets of the search sphere, two voxel counts, the maximum of the reference grid) from cudaMalloc or from the
+ * context's allocator, on first use and again whenever the search sphere grows.  That rules it out for a dose-comparison
+ * loop that shares the GPU with a framework whose pool already owns all of the device memory (the allocation fails), for
+ * one with a latency budget (cudaMalloc and cudaFree may wait for everything else running on the device), and for
+ * services that allow no allocation once they are up.  pmc_gamma_index_static takes the same arguments, gives the same
+ * gamma_dev and *pass_rate_host, and calls no cudaMalloc, no cudaFree, no context allocator and no other allocating
+ * routine: its working memory is one fixed array of PMC_GAMMA_STATIC_SCRATCH_BYTES inside the library image, which every
+ * GPU that loads libpmc holds until the process exits, used or not.  Inputs and outputs stay the caller's.
+ *   Limit: the search sphere may hold at most PMC_GAMMA_STATIC_MAX_OFFSETS voxel centres, i.e. about
+ * (4 pi / 3) search_cm^3 / (dx dy dz) <= 8192 (2 mm DTA with the default 4 mm search radius on 1 mm voxels needs 257,
+ * on 0.5 mm voxels 2109).  Beyond it the call returns PMC_E_CAPACITY with a message that names the limit and writes nothing.
+ *   First call on a device: it looks up the device address of the array (once per device, with that device current)
+ *   before it launches anything, so make that first call outside any stream capture.
+ *   Sharing: there is one array per GPU and every call uses it, so it still holds the previous call's offsets and
+ * counts when the next one starts; each call clears the counts and the maximum on the stream before its first kernel
+ * and overwrites as much of the offset list as it reads.  Two calls in flight on one GPU at the same time would
+ * corrupt each other's list and counts.  Within a process the entry point rules that out itself: it holds a lock from
+ * its first enqueue until its stream has drained, which serialises calls from all threads and contexts (so it is
+ * synchronous on return, like every call here).  Do not let anything else write the array.
+ * Errors: as pmc_gamma_index, plus PMC_E_CAPACITY (above) and PMC_E_UNSUPPORTED for a device ordinal above 63. */
+#define PMC_GAMMA_STATIC_MAX_OFFSETS 8192
+#define PMC_GAMMA_STATIC_SCRATCH_BYTES (256 + 12 * PMC_GAMMA_STATIC_MAX_OFFSETS)
+int  pmc_gamma_index_static(pmc_ctx *ctx, const float *ref_dev, const float *eval_dev, int nx, int ny, int nz,
+                            double dx_cm, double dy_cm, double dz_cm, double dd_frac, double dta_cm, double low_dose_frac,
+                            double search_cm, float *gamma_dev, double *pass_rate_host);
+
 int  pmc_get_counters(pmc_ctx *ctx, pmc_counters *out_host);
 int  pmc_get_timing(pmc_ctx *ctx, pmc_timing *out_host);
 const char *pmc_last_error(pmc_ctx *ctx);     /* owned by ctx, valid until the next call on ctx */

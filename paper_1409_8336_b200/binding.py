@@ -19,7 +19,7 @@ _I = C.POINTER(C.c_int32)
 
 EXPORTS = ["pmc_create", "pmc_create_with_allocator", "pmc_destroy", "pmc_load_physics_tables", "pmc_set_hu_materials", "pmc_load_ct",
            "pmc_load_ct_host", "pmc_set_option", "pmc_simulate", "pmc_simulate_host", "pmc_nonelastic",
-           "pmc_get_counters", "pmc_get_timing", "pmc_get_letd", "pmc_gamma_index", "pmc_set_dose_influence", "pmc_last_error", "pmc_philox4x32_10", "pmc_range_of_energy",
+           "pmc_get_counters", "pmc_get_timing", "pmc_get_letd", "pmc_gamma_index", "pmc_gamma_index_static", "pmc_set_dose_influence", "pmc_last_error", "pmc_philox4x32_10", "pmc_range_of_energy",
            "pmc_energy_of_range", "pmc_straggle", "pmc_elastic", "pmc_first_steps"]
 
 
@@ -237,6 +237,28 @@ class Pmc:
                                            C.c_double(vox[0]), C.c_double(vox[1]), C.c_double(vox[2]),
                                            C.c_double(dd_frac), C.c_double(dta_cm), C.c_double(low_dose_frac),
                                            C.c_double(search_cm), _ptr(out), C.byref(rate)))
+        return out, rate.value
+
+    def gamma_index_static(self, ref, ev, vox, dd_frac=0.02, dta_cm=0.2, low_dose_frac=0.1, search_cm=0.0, out=None):
+        """gamma_index() for callers that may not allocate on the device (their framework's pool owns all of the GPU's
+        memory, they have a latency budget that a cudaMalloc would break, or they allow no allocation once started):
+        pmc_gamma_index_static keeps its working memory in a fixed array inside libpmc, so the call fails with
+        PMC_E_CAPACITY when the search sphere holds more than 8192 voxel centres.  Same results as gamma_index().
+        Pass `out` (and contiguous float32 inputs) if this wrapper is not to ask torch for memory either.  Every call
+        shares that one array per GPU; the library serialises the calls.  Make the first call on a device outside any
+        stream capture (it looks up the array's device address then)."""
+        t = self.torch
+        ref = ref.contiguous(); ev = ev.contiguous()
+        if ref.dtype != t.float32 or ev.dtype != t.float32 or ref.shape != ev.shape or ref.dim() != 3:
+            raise ValueError("ref and ev must be float32 CUDA tensors of the same (nz, ny, nx) shape")
+        if out is None:
+            out = t.empty_like(ref)
+        nz, ny, nx = ref.shape
+        rate = C.c_double(0.0)
+        self._chk(self.lib.pmc_gamma_index_static(self.ctx, _ptr(ref), _ptr(ev), C.c_int(nx), C.c_int(ny), C.c_int(nz),
+                                                  C.c_double(vox[0]), C.c_double(vox[1]), C.c_double(vox[2]),
+                                                  C.c_double(dd_frac), C.c_double(dta_cm), C.c_double(low_dose_frac),
+                                                  C.c_double(search_cm), _ptr(out), C.byref(rate)))
         return out, rate.value
 
     def nonelastic(self, Z, A, e_mev, n, seed, capacity=None):

@@ -7,8 +7,8 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpmc.so")
-SOURCES = ["pmc_api.cu"]
-HEADERS = ["pmc_device.cuh", "pmc_transport.cuh", "pmc_nuclear.cuh", "pmc_gamma.cuh"]
+SOURCES = ["pmc_api.cu", "pmc_gamma_static.cu"]
+HEADERS = ["pmc_device.cuh", "pmc_transport.cuh", "pmc_nuclear.cuh", "pmc_gamma.cuh", "pmc_ctx_access.h"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "--compiler-options", "-fPIC", "-shared"]
 

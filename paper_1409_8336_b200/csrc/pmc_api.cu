@@ -841,3 +841,12 @@ extern "C" int pmc_elastic(pmc_ctx *c, int Z, int A, double t_mev, uint64_t n, u
   CK(cudaStreamSynchronize(c->stream)); CK(cudaGetLastError());
   return PMC_OK;
 }
+
+// ---- pmc_ctx_access.h: read-only facts about a context for the library's other translation units
+#include "pmc_ctx_access.h"
+namespace pmc {
+int ctx_device(const pmc_ctx *c) { return c->device; }
+cudaStream_t ctx_stream(const pmc_ctx *c) { return c->stream; }
+int ctx_sm_count(const pmc_ctx *c) { return c->n_sm; }
+int ctx_fail(pmc_ctx *c, int code, const char *msg) { return fail(c, code, msg); }
+}  // namespace pmc
