@@ -335,7 +335,12 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM) tr
   float2 *s_E = s_R + T.n_sr * T.n_e;
   float *s_sig = reinterpret_cast<float *>(s_E + T.n_sr * T.n_r);
   MatBin *s_bins = reinterpret_cast<MatBin *>(s_sig + T.nbins * T.n_e);
-  int2 *s_lut = reinterpret_cast<int2 *>(reinterpret_cast<unsigned char *>(s_bins + T.nbins) + ((8 - (T.nbins * (int)sizeof(MatBin)) % 8) % 8));
+  // 8-byte entries: the byte offset of the table is rounded up to 8 from the start of the (16-byte aligned) block - the bins
+  // sit after nbins * n_e floats, i.e. at 4 mod 8 when both counts are odd, and a MatBin is 25 words.  (Offset arithmetic,
+  // not pointer-to-integer casts, so that the compiler still sees a shared-memory address.)  The launch's shared-memory
+  // size carries 32 spare bytes for the padding.
+  const int lut_off = ((2 * T.n_sr * (T.n_e + T.n_r) + T.nbins * T.n_e) * 4 + T.nbins * (int)sizeof(MatBin) + 7) & ~7;
+  int2 *s_lut = reinterpret_cast<int2 *>(smem_raw + lut_off);
   for (int i = threadIdx.x; i < T.n_sr * T.n_e; i += blockDim.x) s_R[i] = make_float2(T.lnR[i], T.lnR2[i]);
   for (int i = threadIdx.x; i < T.n_sr * T.n_r; i += blockDim.x) s_E[i] = make_float2(T.lnE[i], T.lnE2[i]);
   for (int i = threadIdx.x; i < T.nbins * T.n_e; i += blockDim.x) s_sig[i] = T.sig_bin[i];
