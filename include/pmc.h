@@ -159,8 +159,14 @@ int  pmc_set_option(pmc_ctx *ctx, const char *key, double value);
 /* PAPER.md:L134-138 (Fig 2): simulate n_histories primaries drawn from the spot list (HOST, nspots entries),
  * in n_batches groups; history h uses the Philox4x32-10 stream keyed (seed, h).  dose_dev / sigma_dev: DEVICE
  * arrays of nx*ny*nz float, overwritten: mean dose in Gy per primary history and its standard error from the
- * batch-to-batch scatter (Reading R8).  n_batches <= n_histories < 2^32 per call (a batch needs a history, L134).
- * Errors: PMC_E_STATE (tables/materials/CT missing), PMC_E_CAPACITY (particle queue overflow), PMC_E_CUDA. */
+ * batch-to-batch scatter (Reading R8).  n_batches <= n_histories < 2^32 per call (a batch needs a history, L134): a
+ * run of fewer histories than the default 10 batches is refused with PMC_E_INVALID_ARG; lower option "n_batches" (>= 2)
+ * first.
+ * Errors: PMC_E_STATE (tables/materials/CT missing), PMC_E_CUDA, PMC_E_CAPACITY (particle queue overflow).  Overflow is
+ * not looked for generation by generation: a kernel that cannot append to a full queue sets a flag on the device and
+ * drops the particle, the scheduler keeps enqueuing, and the flag is read with the counters once the call's work has
+ * drained.  A call that returns PMC_E_CAPACITY has therefore done all its work, and its dose, sigma, LET_d and dose
+ * influence are NOT valid (particles are missing): lower "chunk_histories" and call again. */
 int  pmc_simulate(pmc_ctx *ctx, const pmc_spot *spots_host, int nspots, uint64_t n_histories, uint64_t seed,
                   float *dose_dev, float *sigma_dev);
 /* Same with HOST output arrays (device -> host copies included; end-to-end path). */
@@ -253,7 +259,9 @@ int  pmc_straggle(pmc_ctx *ctx, double e_mev, double mean_loss, double rhoL_gcm2
  * opening angle (rad). */
 int  pmc_elastic(pmc_ctx *ctx, int Z, int A, double t_mev, uint64_t n, uint64_t seed, float *out_dev);
 /* follow n primaries of spot[0] for at most max_steps condensed steps (no secondaries);
- * out_dev [n][8] = x,y,z (cm, grid frame), u,v,w, E, path length. */
+ * out_dev [n][8] = x,y,z (cm, grid frame), u,v,w, E, path length.  A debug path: the dose of these steps goes to an
+ * internal tally that is not returned, LET_d and dose influence are not scored even if switched on, the counters hold
+ * n_generations = 1 and the sums of that one generation, and a queue overflow cannot occur (nothing is appended). */
 int  pmc_first_steps(pmc_ctx *ctx, const pmc_spot *spot_host, uint64_t n, uint64_t seed, int max_steps,
                      float *out_dev);
 #ifdef __cplusplus

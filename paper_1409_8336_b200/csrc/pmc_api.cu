@@ -367,7 +367,7 @@ int run_generations(pmc_ctx *c, RunParams P, bool profile) {
 #undef PMC_LAUNCH_TRANSPORT
       }
       c->timing.launches_total++; c->timing.launches_transport++;
-      if (P.dbg_out) return PMC_OK;
+      if (P.dbg_out) { c->counters.n_generations = 1; return PMC_OK; }     // first-steps path: the primaries' generation only
       { Timer t(c, &c->timing.elastic_ms, profile);
         event_kernel<<<grid_e, 256, 0, s>>>(c->T, c->G, P, c->qev.q, c->qel.q, c->qne.q, nxt->q, c->d_cnt.p);
         elastic_kernel<<<grid_e, 256, 0, s>>>(c->T, P, c->qel.q, nxt->q, c->d_tally.p, c->d_cnt.p); }
