@@ -64,7 +64,7 @@ def _load():
         _lib = C.CDLL(build_oracle())
         _lib.opmc_last_error.restype = C.c_char_p
         for f in ("opmc_test_range_gcm2", "opmc_test_energy_of_range", "opmc_test_inc_uniform_sphere",
-                  "opmc_test_nucleus", "opmc_test_fermi_p2", "opmc_test_cugnon"):
+                  "opmc_test_nucleus", "opmc_test_nucleus_neutron", "opmc_test_fermi_p2", "opmc_test_cugnon"):
             getattr(_lib, f).restype = C.c_double
     return _lib
 
@@ -249,6 +249,12 @@ class Oracle:
         out = np.zeros((15, 6))
         rmax = self.lib.opmc_test_nucleus(self.ctx, Z, A, _dp(out))
         return rmax, out
+
+    def nucleus_neutron(self, Z, A):
+        """-> (Coulomb barrier B_C, [15][3] = pF_n, EF_n, V_n)."""
+        out = np.zeros((15, 3))
+        bc = self.lib.opmc_test_nucleus_neutron(self.ctx, Z, A, _dp(out))
+        return bc, out
 
     def fermi_p2(self, Z, A, n, seed):
         return self.lib.opmc_test_fermi_p2(self.ctx, Z, A, C.c_uint64(n), C.c_uint64(seed))

@@ -1110,6 +1110,12 @@ double opmc_test_nucleus(opmc_ctx *c, int Z, int A, double *out) {
   for (int k = 0; k < 15; ++k) { double *o = out + 6 * k; o[0] = N.rout[k]; o[1] = N.rho[0][k]; o[2] = N.rho[1][k]; o[3] = N.pF[0][k]; o[4] = N.EF[0][k]; o[5] = N.V[0][k]; }
   return N.rmax;
 }
+// the neutron side of the same model (test hook, no arithmetic of its own): out[15][3] = pF_n, EF_n, V_n
+double opmc_test_nucleus_neutron(opmc_ctx *c, int Z, int A, double *out) {
+  Nucleus N = build_nucleus(c->T, Z, A);
+  for (int k = 0; k < 15; ++k) { double *o = out + 3 * k; o[0] = N.pF[1][k]; o[1] = N.EF[1][k]; o[2] = N.V[1][k]; }
+  return N.coulomb;
+}
 double opmc_test_fermi_p2(opmc_ctx *c, int Z, int A, uint64_t n, uint64_t seed) {
   Nucleus N = build_nucleus(c->T, Z, A); double acc = 0;
   Rng g(seed, 0, 0);

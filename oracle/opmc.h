@@ -124,6 +124,7 @@ double opmc_test_inc_uniform_sphere(double radius_fm, double rho_fm3, double sig
                                     uint64_t n, uint64_t seed);
 /* shells of nucleus (Z,A): out[15][6] = r_out, rho_p, rho_n, pF_p, EF_p, V_p ; returns r_max */
 double opmc_test_nucleus(opmc_ctx *, int Z, int A, double *out);
+double opmc_test_nucleus_neutron(opmc_ctx *, int Z, int A, double *out);   /* out[15][3] = pF_n, EF_n, V_n; returns B_C */
 /* mean of p^2 over n sampled Fermi partners in the central shell divided by pF^2 (-> 3/5) */
 double opmc_test_fermi_p2(opmc_ctx *, int Z, int A, uint64_t n, uint64_t seed);
 /* evaporation of (Z,A,E*) at rest: widths[6] by quadrature; first emission of n samples restricted to
