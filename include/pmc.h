@@ -252,6 +252,12 @@ int  pmc_philox4x32_10(pmc_ctx *ctx, const uint32_t *in_dev, uint64_t n, uint32_
 /* CSDA range R(E) (g/cm2) of table `table` and its inverse; e_dev/r_dev DEVICE float[n]. */
 int  pmc_range_of_energy(pmc_ctx *ctx, int table, const float *e_dev, uint64_t n, float *r_dev);
 int  pmc_energy_of_range(pmc_ctx *ctx, int table, const float *r_dev, uint64_t n, float *e_dev);
+/* The same two functions through the step kernel's own look-up: tables staged in shared memory,
+ * knot index from log2(E), interleaved spline knots, for HU bin `hu_bin` (index into the array given to
+ * pmc_set_hu_materials; its table_id selects the table).  Needs the materials.  Ranges are g/cm2 of the table medium,
+ * i.e. before the f_m scaling of Eq.1/Eq.2.  Errors: PMC_E_STATE (no tables or materials), PMC_E_INVALID_ARG (bin). */
+int  pmc_step_range_of_energy(pmc_ctx *ctx, int hu_bin, const float *e_dev, uint64_t n, float *r_dev);
+int  pmc_step_energy_of_range(pmc_ctx *ctx, int hu_bin, const float *r_dev, uint64_t n, float *e_dev);
 /* n straggled losses for a step with mean loss mean_loss, mass thickness rhoL (g/cm2), <Z/A>. */
 int  pmc_straggle(pmc_ctx *ctx, double e_mev, double mean_loss, double rhoL_gcm2, double z_over_a,
                   uint64_t n, uint64_t seed, float *out_dev);

@@ -20,7 +20,7 @@ _I = C.POINTER(C.c_int32)
 EXPORTS = ["pmc_create", "pmc_create_with_allocator", "pmc_destroy", "pmc_load_physics_tables", "pmc_set_hu_materials", "pmc_load_ct",
            "pmc_load_ct_host", "pmc_set_option", "pmc_simulate", "pmc_simulate_host", "pmc_nonelastic",
            "pmc_get_counters", "pmc_get_timing", "pmc_get_letd", "pmc_gamma_index", "pmc_gamma_index_static", "pmc_set_dose_influence", "pmc_last_error", "pmc_philox4x32_10", "pmc_range_of_energy",
-           "pmc_energy_of_range", "pmc_straggle", "pmc_elastic", "pmc_first_steps"]
+           "pmc_energy_of_range", "pmc_step_range_of_energy", "pmc_step_energy_of_range", "pmc_straggle", "pmc_elastic", "pmc_first_steps"]
 
 
 class Tables(C.Structure):
@@ -303,6 +303,21 @@ class Pmc:
         a = t.as_tensor(np.ascontiguousarray(r, dtype=np.float32), device=self.device)
         out = t.empty_like(a)
         self._chk(self.lib.pmc_energy_of_range(self.ctx, C.c_int(table), _ptr(a), C.c_uint64(a.numel()), _ptr(out)))
+        return out.cpu().numpy()
+
+    def step_range_of_energy(self, hu_bin, e):
+        """R(E) of HU bin hu_bin through the step kernel's shared-memory look-up (g/cm2 of the table medium)."""
+        t = self.torch
+        a = t.as_tensor(np.ascontiguousarray(e, dtype=np.float32), device=self.device)
+        out = t.empty_like(a)
+        self._chk(self.lib.pmc_step_range_of_energy(self.ctx, C.c_int(hu_bin), _ptr(a), C.c_uint64(a.numel()), _ptr(out)))
+        return out.cpu().numpy()
+
+    def step_energy_of_range(self, hu_bin, r):
+        t = self.torch
+        a = t.as_tensor(np.ascontiguousarray(r, dtype=np.float32), device=self.device)
+        out = t.empty_like(a)
+        self._chk(self.lib.pmc_step_energy_of_range(self.ctx, C.c_int(hu_bin), _ptr(a), C.c_uint64(a.numel()), _ptr(out)))
         return out.cpu().numpy()
 
     def straggle(self, e, mean_loss, rho_l, zoa, n, seed):

@@ -809,6 +809,23 @@ static int range_impl(pmc_ctx *c, int table, const float *in, uint64_t n, float 
 int pmc_range_of_energy(pmc_ctx *c, int table, const float *e_dev, uint64_t n, float *r_dev) { return range_impl(c, table, e_dev, n, r_dev, 0); }
 int pmc_energy_of_range(pmc_ctx *c, int table, const float *r_dev, uint64_t n, float *e_dev) { return range_impl(c, table, r_dev, n, e_dev, 1); }
 
+static int step_range_impl(pmc_ctx *c, int bin, const float *in, uint64_t n, float *out, int inverse) {
+  if (!c || (n && (!in || !out))) return fail(c, PMC_E_INVALID_ARG, "null argument");
+  if (!c->have_tables || !c->have_mats) return fail(c, PMC_E_STATE, "load physics tables and HU materials first");
+  if (bin < 0 || bin >= (int)c->mats.size()) return fail(c, PMC_E_INVALID_ARG, "bad HU bin index");
+  cudaSetDevice(c->device);
+  int rc = sync_tables(c); if (rc) return rc;
+  if (n) {
+    CK(cudaFuncSetAttribute(step_range_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_transport));
+    const unsigned grid = (unsigned)std::min<uint64_t>((n + 255) / 256, (uint64_t)c->n_sm * 4);
+    step_range_kernel<<<grid, 256, c->smem_transport, c->stream>>>(c->T, bin, in, n, out, inverse);
+  }
+  CK(cudaStreamSynchronize(c->stream)); CK(cudaGetLastError());
+  return PMC_OK;
+}
+int pmc_step_range_of_energy(pmc_ctx *c, int hu_bin, const float *e_dev, uint64_t n, float *r_dev) { return step_range_impl(c, hu_bin, e_dev, n, r_dev, 0); }
+int pmc_step_energy_of_range(pmc_ctx *c, int hu_bin, const float *r_dev, uint64_t n, float *e_dev) { return step_range_impl(c, hu_bin, r_dev, n, e_dev, 1); }
+
 int pmc_straggle(pmc_ctx *c, double e, double mean, double rhoL, double zoa, uint64_t n, uint64_t seed, float *out_dev) {
   if (!c || !out_dev) return fail(c, PMC_E_INVALID_ARG, "null argument");
   if (!c->have_tables) return fail(c, PMC_E_STATE, "load physics tables first");

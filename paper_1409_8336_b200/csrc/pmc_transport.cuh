@@ -315,22 +315,13 @@ __device__ __forceinline__ V3 rotate(V3 d, float st, float ct, float sp, float c
   return {n.x * in, n.y * in, n.z * in};
 }
 
-// MCS_MODEL: 0 = Highland (the paper's choice), 1 = full Moliere; a template so that the default kernel carries none of
-// the Moliere code or its registers
-// DBG: the pmc_first_steps variant (stop after max_steps, write the state of every primary); the production kernel
-// carries neither its registers nor its branches.
-// EXTRA: LET_d scoring, per-spot dose influence or warp-merged dose atomics are on (the plain kernel carries none of it)
-template <int MCS_MODEL, bool DBG, bool EXTRA>
-__global__ void __launch_bounds__(TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM) transport_kernel(Tables T, Grid G, RunParams P, Queue in, uint32_t *gen_n,
-                                                           uint32_t *head, Queue q_ev, float *tally, Counters *cnt) {
-  // the generation's particle count stays on the device (the host does not wait for it): an empty generation ends here
-  const uint32_t n_in = min(*in.count, in.cap);
-  if (blockIdx.x == 0 && threadIdx.x == 0) *gen_n = n_in;
-  if (n_in == 0u) return;
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  // shared-memory staging of the stopping-power/range and cross-section tables (PAPER.md:L144 used textures): spline
-  // knots interleaved with their second derivatives (one 8-byte load per knot), ln R(ln E) first, then ln E(ln R), then
-  // Sigma/rho per HU bin, the HU bins and the HU -> {density, bin} table; MatBin holds each bin's offsets into these arrays
+// ---- the step kernel's tables in shared memory (PAPER.md:L144 used textures) and its look-ups, shared with step_range_kernel
+// Layout from the start of the dynamic shared memory: spline knots interleaved with their second derivatives (one 8-byte
+// load per knot), ln R(ln E) first, then ln E(ln R), then Sigma/rho per HU bin, the HU bins and the HU -> {density, bin}
+// table; MatBin holds each bin's offsets (in floats) into these arrays.
+struct StepTables { const float *f; const MatBin *bins; const int2 *lut; };
+// all threads of the block call; the caller synchronises before the first look-up
+__device__ __forceinline__ StepTables stage_step_tables(const Tables &T, unsigned char *smem_raw) {
   float2 *s_R = reinterpret_cast<float2 *>(smem_raw);
   float2 *s_E = s_R + T.n_sr * T.n_e;
   float *s_sig = reinterpret_cast<float *>(s_E + T.n_sr * T.n_r);
@@ -347,8 +338,44 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM) tr
   for (int i = threadIdx.x; i < T.nbins * (int)(sizeof(MatBin) / 4); i += blockDim.x)
     reinterpret_cast<uint32_t *>(s_bins)[i] = reinterpret_cast<const uint32_t *>(T.bins)[i];
   for (int i = threadIdx.x; i < T.hu_lut_n; i += blockDim.x) s_lut[i] = T.hu_lut2[i];
+  return {reinterpret_cast<const float *>(smem_raw), s_bins, s_lut};
+}
+// knot and fraction of the forward tables from l2 = log2(E), E already clamped to the table: t = (ln E - ln e_min) / dlnE
+// in one FMA with the two constants folded on the host
+__device__ __forceinline__ EIdx step_e_index(const Tables &T, float l2) {
+  const float te = fmaf(l2, T.c_l2, -T.c_e0);
+  const int ke = min(max((int)te, 0), T.n_e - 2);
+  return {ke, te - (float)ke};
+}
+// ln R (g/cm2 of the bin's table medium) at that knot position
+__device__ __forceinline__ float step_ln_range(const float *s_f, const MatBin &m, EIdx k) {
+  return spline_eval2(reinterpret_cast<const float2 *>(s_f + m.off_e), k.i, k.b);
+}
+// ln E at ln R = xr from the bin's inverse table, clamped to the table's ends
+__device__ __forceinline__ float step_ln_energy(const Tables &T, const float *s_f, const MatBin &m, float xr) {
+  const float tr = (xr - m.lnr_lo) * m.inv_hr;
+  const int kr = min(max((int)tr, 0), T.n_r - 2);
+  const float lnE1 = spline_eval2(reinterpret_cast<const float2 *>(s_f + m.off_r), kr, tr - (float)kr);
+  return xr <= m.lnr_lo ? T.ln_emin : (xr >= m.lnr_hi ? T.ln_emax : lnE1);
+}
+
+// MCS_MODEL: 0 = Highland (the paper's choice), 1 = full Moliere; a template so that the default kernel carries none of
+// the Moliere code or its registers
+// DBG: the pmc_first_steps variant (stop after max_steps, write the state of every primary); the production kernel
+// carries neither its registers nor its branches.
+// EXTRA: LET_d scoring, per-spot dose influence or warp-merged dose atomics are on (the plain kernel carries none of it)
+template <int MCS_MODEL, bool DBG, bool EXTRA>
+__global__ void __launch_bounds__(TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM) transport_kernel(Tables T, Grid G, RunParams P, Queue in, uint32_t *gen_n,
+                                                           uint32_t *head, Queue q_ev, float *tally, Counters *cnt) {
+  // the generation's particle count stays on the device (the host does not wait for it): an empty generation ends here
+  const uint32_t n_in = min(*in.count, in.cap);
+  if (blockIdx.x == 0 && threadIdx.x == 0) *gen_n = n_in;
+  if (n_in == 0u) return;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const StepTables S = stage_step_tables(T, smem_raw);
   __syncthreads();
-  const float *s_f = reinterpret_cast<const float *>(smem_raw);   // every table offset in MatBin counts floats from here
+  const float *s_f = S.f;                                         // every table offset in MatBin counts floats from here
+  const MatBin *s_bins = S.bins; const int2 *s_lut = S.lut;
 
   const float szx = G.d[0], szy = G.d[1], szz = G.d[2];
   const int lane = threadIdx.x & 31;
@@ -397,13 +424,11 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM) tr
       const uint32_t spare = __byte_perm(r.y, r.w, 0x5410);
       // ---- 1. nuclear distance, face distance, residual range
       const float e0 = p.e, l2 = flg2(fminf(fmaxf(e0, T.e_min), T.e_max)), lnEv = l2 * LN2;
-      const float te = fmaf(l2, T.c_l2, -T.c_e0);
-      const int ke = min(max((int)te, 0), T.n_e - 2);
-      const EIdx k{ke, te - (float)ke};
+      const EIdx k = step_e_index(T, l2);
       float lam = BIG;
       if (nuclear) { const float Sig = rho * lerp_tab(s_f + m.off_sig, k); lam = Sig > 0.f ? -LN2 * flg2(u23(r.x)) * frcp(Sig) : BIG; }
       const float dface = fminf(fminf(axis_dist(p.r.x, p.d.x, szx), axis_dist(p.r.y, p.d.y, szy)), axis_dist(p.r.z, p.d.z, szz));
-      const float lnRv = spline_eval2(reinterpret_cast<const float2 *>(s_f + m.off_e), k.i, k.b), Rg = fex2(lnRv * LOG2E), iwf = frcp(wf);
+      const float lnRv = step_ln_range(s_f, m, k), Rg = fex2(lnRv * LOG2E), iwf = frcp(wf);
       const float R = Rg * iwf, smax = T.s_max > 0.f ? T.s_max * iwf : BIG;
       // ---- 2. step = min (Reading R3.2)
       float dx = lam; int lim = 2;
@@ -465,11 +490,7 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM) tr
         const float dr = L * wf;
         float lnE1 = T.ln_emin;
         if (Rg - dr > 0.f) {
-          const float xr = lnRv + log1p_small(-dr * frcp(Rg));
-          const float tr = (xr - m.lnr_lo) * m.inv_hr;
-          const int kr = min(max((int)tr, 0), T.n_r - 2);
-          lnE1 = spline_eval2(reinterpret_cast<const float2 *>(s_f + m.off_r), kr, tr - (float)kr);
-          lnE1 = xr <= m.lnr_lo ? T.ln_emin : (xr >= m.lnr_hi ? T.ln_emax : lnE1);
+          lnE1 = step_ln_energy(T, s_f, m, lnRv + log1p_small(-dr * frcp(Rg)));
         }
         loss = fminf(fmaxf(-e0 * expm1_small(lnE1 - lnEv), 0.f), e0);
         if (EXTRA) let = fdiv(0.1f * loss, L);                   // keV/um of this step (Reading R9)
@@ -507,6 +528,24 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS, TRANSPORT_BLOCKS_PER_SM) tr
   }
   flush(&cnt->n_steps, (unsigned long long)c_steps);
   flush(&cnt->e_deposit, (double)c_dep);
+}
+
+// ------------------------------------------------------------------ sub-step: the step kernel's own table look-ups
+// R(E) and E(R) of HU bin `bin` through exactly what transport_kernel uses - the tables staged in shared memory by
+// stage_step_tables, the knot index from log2(E) (step_e_index), the interleaved splines (step_ln_range, step_ln_energy)
+// and the single-MUFU log2 / exp2 - so that the production look-up is compared with the oracle element by element
+// (pmc_range_of_energy evaluates the global-memory splines with logf / expf / floorf instead).
+__global__ void __launch_bounds__(256) step_range_kernel(Tables T, int bin, const float *in, uint64_t n, float *out, int inverse) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const StepTables S = stage_step_tables(T, smem_raw);
+  __syncthreads();
+  const MatBin &m = S.bins[bin];
+  for (uint64_t i = blockIdx.x * (uint64_t)blockDim.x + threadIdx.x; i < n; i += (uint64_t)gridDim.x * blockDim.x) {
+    if (!inverse) {
+      const float l2 = flg2(fminf(fmaxf(in[i], T.e_min), T.e_max));
+      out[i] = fex2(step_ln_range(S.f, m, step_e_index(T, l2)) * LOG2E);
+    } else out[i] = fex2(step_ln_energy(T, S.f, m, flg2(fmaxf(in[i], 1e-30f)) * LN2) * LOG2E);
+  }
 }
 
 // ------------------------------------------------------------------ event class and target element (Reading R5)

@@ -75,6 +75,31 @@ def test_range_tables_match_oracle(pm, oracle_c1, table):
     assert np.max(np.abs(e_back / e - 1)) < 1e-4
 
 
+@pytest.mark.parametrize("mats_name,hu_bin", [("c1", 0), ("c1", 1), ("c1", 2), ("24", 1), ("24", 23)])
+def test_step_kernel_table_lookup_matches_oracle(pm, tables, oracle_c1, mats_name, hu_bin):
+    # the production look-up of the step kernel (shared-memory tables, knot index from log2 E in one FMA, interleaved
+    # knots, MUFU log2 / exp2), element by element.  On top of the 1e-5 of the spline evaluation: the fp32 knot coordinate
+    # of up to 255 carries up to ~3e-5 knots (2^-24 of itself and of its two constants), i.e. ~2e-6 of R with
+    # d ln R / d knot = 0.06; lg2.approx / ex2.approx add ~2 ulp of ln R ~ 5 and of the result: 4e-5 in all
+    mats = inputs.make_materials_c1() if mats_name == "c1" else inputs.make_materials_24()
+    pm.load_physics_tables(tables); pm.set_hu_materials(mats)
+    table = mats[hu_bin]["table_id"]
+    e = np.exp(np.linspace(np.log(0.06), np.log(290.0), 70001)).astype(np.float32)          # several blocks, ragged tail
+    r_g = pm.step_range_of_energy(hu_bin, e).astype(np.float64)
+    r_o = np.array([oracle_c1.range_gcm2(table, float(x)) for x in e[::17]])
+    assert np.max(np.abs(r_g[::17] / r_o - 1)) < 4e-5
+    assert np.max(np.abs(r_g / pm.range_of_energy(table, e) - 1)) < 5e-5                    # every element, vs the plain path
+    e_back = pm.step_energy_of_range(hu_bin, r_g.astype(np.float32)).astype(np.float64)
+    e_o = np.array([oracle_c1.energy_of_range(table, float(x)) for x in r_g[::17]])
+    assert np.max(np.abs(e_back[::17] / e_o - 1)) < 4e-5
+    assert np.max(np.abs(e_back / e - 1)) < 1e-4
+    # clamps of the step kernel: below / above the table the end values come back
+    lo_hi = pm.step_range_of_energy(hu_bin, np.array([1e-3, 1e4], dtype=np.float32))
+    assert lo_hi[0] == pytest.approx(oracle_c1.range_gcm2(table, 0.05), rel=4e-5)
+    assert lo_hi[1] == pytest.approx(oracle_c1.range_gcm2(table, 300.0), rel=4e-5)
+    assert pm.step_range_of_energy(hu_bin, np.zeros(0, dtype=np.float32)).shape == (0,)
+
+
 # ------------------------------------------------------------------ S5 straggling: cumulants and distribution
 @pytest.mark.parametrize("e_mev,rho_l", [(230.0, 0.1), (150.0, 0.2), (70.0, 0.2), (30.0, 0.25), (5.0, 0.02), (200.0, 0.0003)])
 def test_straggling_distribution(pm, oracle_c1, e_mev, rho_l):
@@ -307,13 +332,18 @@ def _cascade_capacities_hold(cg, tag=""):
 
 
 def _dose_parity(pm, o, w_hu, vox, mats, spots, n, seed, axis=0, check_range=True, min_pass=0.99, batches=40, seed_o=None):
-    """north_star's dose tolerances between pmc_simulate and the oracle on the same inputs (B batches on both sides)."""
+    """north_star's dose tolerances between pmc_simulate and the oracle on the same inputs (B batches on both sides).
+    The oracle runs another seed (seed + 1000 unless given): with the same seed both sides draw the spot and the lateral
+    position of every primary from the same Philox words, which correlates the two dose maps (rms z 0.82-0.92 was seen)
+    and makes the comparison look better than it is.  rms z is held to a window around 1 for that reason."""
+    if seed_o is None:
+        seed_o = seed + 1000
     pm.set_option("n_batches", float(batches)); o.set_option("n_batches", float(batches))
     try:
         dg, sg = pm.simulate(spots, n, seed)
         cg = pm.counters()
         dg, sg = dg.cpu().numpy().astype(np.float64), sg.cpu().numpy().astype(np.float64)
-        do, so = o.simulate(spots, n, seed if seed_o is None else seed_o)
+        do, so = o.simulate(spots, n, seed_o)
         co = o.counters()
     finally:
         pm.set_option("n_batches", 10.0); o.set_option("n_batches", 10.0)
@@ -322,7 +352,10 @@ def _dose_parity(pm, o, w_hu, vox, mats, spots, n, seed, axis=0, check_range=Tru
     rho = _density(w_hu, mats)
     vol = vox[0] * vox[1] * vox[2]
     eg, eo = (dg * rho).sum() * vol / parity.GY_PER_MEV_G, (do * rho).sum() * vol / parity.GY_PER_MEV_G
-    assert abs(eg / eo - 1) < 5e-3, (eg, eo)
+    # north_star's 0.5 %, plus three standard errors of the difference of two independent runs: with nuclear events on the
+    # energy a history deposits has an rms of ~15 % of its mean (one in five loses tens of MeV to neutrons and photons),
+    # i.e. 0.2 % on the difference at the 1e4 histories of C1 as configured, 0.02 % at 1e6
+    assert abs(eg / eo - 1) < 5e-3 + 3 * 0.15 * np.sqrt(2.0 / n), (eg, eo)
     assert abs(eg - cg["e_deposit"] / n) < 2e-4 * eg                       # tally == ledger (fp32 atomics)
     assert _ledger_closes(cg), cg
     assert _cascade_capacities_hold(cg), cg
@@ -330,9 +363,16 @@ def _dose_parity(pm, o, w_hu, vox, mats, spots, n, seed, axis=0, check_range=Tru
     frac, zmean, zrms, nv = parity.zscore_pass(dg, sg, do, so)
     if min_pass is None:
         min_pass = low_stat_bound(nv)
+    else:            # the literal 99 % wherever the voxel count carries it (nv > ~5000); P(|t| < 3) = 99.6 % at B = 40
+        min_pass = min(min_pass, low_stat_bound(nv, expect=0.996))
     print(f"z-pass {frac:.4f} (bound {min_pass:.4f}) mean z {zmean:+.3f} rms z {zrms:.3f} voxels {nv} B {batches} n {n}")
     assert nv > 20 and frac >= min_pass, (frac, zmean, zrms, nv)
-    assert abs(zmean) < 0.25 and zrms < 1.5, (zmean, zrms)
+    # independent runs: z has unit variance (t-like with 2(B - 1) degrees of freedom: 1.03 at B = 40, 1.12 at B = 10); the
+    # voxels of a beam share histories (count one in eight), so rms z over nv voxels scatters by 2 / sqrt(nv)
+    z_lo, z_hi = 0.95 - 6.0 / np.sqrt(nv), (1.2 if batches >= 30 else 1.3) + 6.0 / np.sqrt(nv)
+    if seed_o == seed:
+        z_lo = 0.0           # the same positions on both sides on purpose (deterministic case): no lower bound
+    assert abs(zmean) < 0.25 and z_lo < zrms < z_hi, (zmean, zrms, z_lo, z_hi)
     # R80 and distal fall-off within 0.2 mm
     if check_range:
         d_cm = vox[2 - axis]
@@ -343,7 +383,8 @@ def _dose_parity(pm, o, w_hu, vox, mats, spots, n, seed, axis=0, check_range=Tru
     for k in ("n_elastic", "n_nonelastic", "n_secondary_protons"):
         a, b = cg[k], co[k]
         assert abs(a - b) < 5 * np.sqrt(a + b + 1) + 0.002 * b, (k, a, b)
-    assert abs(cg["n_steps"] / co["n_steps"] - 1) < 5e-3
+    # steps per history: rms ~ 30 % of the mean (a non-elastic event ends the primary anywhere along its track)
+    assert abs(cg["n_steps"] / co["n_steps"] - 1) < 5e-3 + 3 * 0.3 * np.sqrt(2.0 / n)
     return dg, sg, do, so, cg, co
 
 
@@ -391,7 +432,11 @@ def test_c1_water_phantom_high_statistics(pm, tables):
 def test_c1_physics_switches(pm, tables, switches):
     w = inputs.workload("c1")
     o = _setup(pm, tables, w["materials"], w["hu"], w["vox"], **switches)
-    _dose_parity(pm, o, w["hu"], w["vox"], w["materials"], w["spots"], 100_000, 21)
+    # With every fluctuation off all histories are the same CSDA track and only the spot position is random: the voxels
+    # of a column then fluctuate together (a handful of independent z values, not 475), so that case is compared with the
+    # SAME seed on both sides - the same positions, hence the same dose up to fp32 (rms z ~ 0.001) - a deterministic check.
+    same = "mcs" in switches and "straggling" in switches
+    _dose_parity(pm, o, w["hu"], w["vox"], w["materials"], w["spots"], 100_000, 21, seed_o=21 if same else None)
 
 
 def test_pencil_on_a_voxel_edge(pm, tables):
@@ -555,11 +600,11 @@ def test_c4_two_seeds_eq5_and_gamma(pm, tables):
 
 def test_c5_pelvis_full_size_against_oracle_subsample(pm, tables):
     """C5 (512x512x200 pelvis with Ti implants, 11033 spots, 100-230 MeV) at BASELINE's full 1e8 histories on the GPU
-    (6 sub-groups of 2^24 histories); the oracle runs the 1e6-history subsample SURVEY 8(d) assigns to this throughput
-    configuration.  40 batches on both sides for the voxel comparison (see low_stat_bound above)."""
+    (6 sub-groups of 2^24 histories); the oracle runs a 1e7-history subsample (ten times what SURVEY 8(d) assigns to this
+    throughput configuration, so that its own noise in low-count voxels no longer skews the z scores).  40 batches on both sides for the voxel comparison (see low_stat_bound above)."""
     w = inputs.workload("c5")
     o = _setup(pm, tables, w["materials"], w["hu"], w["vox"])
-    n_g, n_o = w["n_histories"], 1_000_000
+    n_g, n_o = w["n_histories"], 10_000_000
     pm.set_option("n_batches", 40.0); o.set_option("n_batches", 40.0)
     try:
         dg, sg = pm.simulate(w["spots"], n_g, w["seed"])
@@ -585,8 +630,11 @@ def test_c5_pelvis_full_size_against_oracle_subsample(pm, tables):
     assert b > 0 and abs(a / b - 1) < 0.03, (a, b)
     # voxel z-scores in tissue and bone (not air, Reading R8.1)
     frac, zmean, zrms, nv = parity.zscore_pass(dg, sg, do, so, region=w["hu"] >= -950)
-    print(f"C5 1e8 vs oracle 1e6: z-pass {frac:.4f} mean z {zmean:+.3f} rms z {zrms:.3f} voxels {nv}")
-    assert nv > 100_000 and frac >= 0.99 and abs(zmean) < 0.2 and zrms < 1.3, (frac, zmean, zrms, nv)
+    print(f"C5 1e8 vs oracle 1e7: z-pass {frac:.4f} mean z {zmean:+.3f} rms z {zrms:.3f} voxels {nv}")
+    # mean z: +0.120 against a 1e6-history oracle run, +0.067 against 1e7 - it falls as the ORACLE's statistics improve
+    # (skewed low-count voxels of the sparser run), where a bias of the CUDA path would grow in units of the shrinking sigma;
+    # C4 with 1e7 histories on both sides has +0.008
+    assert nv > 100_000 and frac >= 0.99 and abs(zmean) < 0.1 and 0.95 < zrms < 1.2, (frac, zmean, zrms, nv)
     for ax in range(3):
         pg, po = parity.depth_dose(dg * rho, ax), parity.depth_dose(do * rho, ax)
         m = po > 0.05 * po.max()
