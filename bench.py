@@ -53,9 +53,16 @@ ALGO_INST_PER_STEP = float(sum(ALGO_ITEMS.values()))
 # One-off `ncu --set full` capture of the first-generation step-kernel launch of a 1e7-history C4 step
 # (profiles/r02_transport_full.md; NOT measured in this run): DRAM bytes per history, executed thread-instructions per
 # condensed step, active lanes per warp instruction, issue-slot utilisation.
-NCU_CAPTURE = {"source": "profiles/r02_transport_full.md (one-off ncu capture, not measured in this run)",
+NCU_CAPTURE = {"source": "profiles/r02_transport_full.md, profiles/r03_transport_pipes.md, profiles/r03_c5_transport.md (one-off ncu "
+                         "captures at head c17c33c, step kernel unchanged since r02: 2.9848e10 warp instructions in both; not "
+                         "measured in this run)",
                "dram_bytes_per_history_c4": 79.3, "executed_thread_inst_per_step": 634.0, "lanes_per_warp_inst": 29.2,
-               "issue_slot_utilisation_pct": 81.6}
+               "issue_slot_utilisation_pct": 81.6,
+               # which pipe binds (r03): none - the busiest pipe is the ALU at 56 % of its issue rate, the MUFU (XU) pipe 42 %,
+               # FMA heavy / lite 40 / 37 %; the kernel is bound by the issue slots themselves (81.6 % busy)
+               "binding": "issue slots", "pipe_pct_of_peak": {"alu": 56.4, "xu": 42.4, "fmaheavy": 40.5, "fmalite": 37.4,
+                                                              "adu": 24.1, "lsu": 10.2, "cbu": 3.9, "uniform": 0.5},
+               "dram_bytes_per_history_c5": 68.6, "c5_l2_hit_rate_pct": 70.1, "c5_issue_slot_utilisation_pct": 82.2}
 ISSUE_LANES_PER_SM_PER_CLK = 128.0     # 4 schedulers x 32 lanes
 N_SM = 148
 
@@ -218,9 +225,12 @@ def main():
     pm.load_ct(hu_dev, w["vox"])
     offset, _ = weak_shard(n_hist, rank)
     pm.set_option("history_offset", float(offset))
+    n_batches = int(tables["n_batches"])            # what the context runs with: the tables' value unless an option sets it
     for kv in args.option:
         k_, v_ = kv.split("=", 1)
         pm.set_option(k_, float(v_))
+        if k_ == "n_batches":
+            n_batches = int(float(v_))
     spots = w["spots"]
     nvox = int(w["hu"].size)
     dose = torch.empty(w["hu"].shape, dtype=torch.float32, device=dev)
@@ -325,7 +335,7 @@ def main():
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": w["label"], "histories_per_step_per_gpu": n_hist, "n_spots": w["n_spots"],
-                       "n_batches": 10, "l2": "flushed between timed steps (256 MiB write)",
+                       "n_batches": n_batches, "l2": "flushed between timed steps (256 MiB write)",
                        "parallelism": f"history-sharded x{world}", "options": args.option},
             "clocks": {k: clocks[k] for k in ("sm_mhz", "sm_max_mhz", "reasons")},
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
@@ -392,6 +402,15 @@ def measure_extras(pm, w, n_hist, spots, hu_dev, stream, dev, tables):
                  "ms_device": tm["total_ms"], "seconds_wall": dt, "steps_per_history": cn["n_steps"] / w5["n_histories"],
                  "kernel_ms": {k: tm[k] for k in ("sampler_ms", "transport_ms", "elastic_ms", "inc_ms", "evaporation_ms",
                                                   "statistics_ms")}, "n_spots": w5["n_spots"]}
+    # C5's own roofline block (same plain-ALU issue bound as C4: profiles/r03_c5_transport.md shows 82 % issue-slot
+    # utilisation, 70 % L2 hit rate and 0.2 % of the HBM peak although its 2.1 GB of tallies do not fit the L2)
+    peak5 = N_SM * ISSUE_LANES_PER_SM_PER_CLK * 1965.0e6 / 1e9
+    ach5 = ALGO_INST_PER_STEP * cn["n_steps"] / (tm["transport_ms"] * 1e-3) / 1e9 if tm["transport_ms"] > 0 else 0.0
+    out["c5"]["roofline"] = {"bound": "alu", "kernel": "transport_kernel", "achieved": ach5, "peak": peak5,
+                             "unit": "Gthread-inst/s", "frac": ach5 / peak5, "peak_source": "148 SMs x 128 lanes x 1965 MHz (nominal; "
+                             "the main line uses the clock sampled under load)",
+                             "traffic": NCU_CAPTURE["dram_bytes_per_history_c5"] * w5["n_histories"],
+                             "traffic_note": "DRAM bytes of a first-generation launch from the one-off capture, per history x histories"}
     pm.set_hu_materials(w["materials"]); pm.load_ct(hu_dev, w["vox"])
     return out
 
