@@ -909,7 +909,11 @@ def test_scratch_comes_from_the_callers_allocator(tables):
     w = inputs.workload("c1")
     hu = torch.as_tensor(w["hu"], device="cuda")
     doses = []
+    import gc
     for use_torch in (True, False):
+        # garbage of earlier tests (contexts, result tensors in reference cycles) must be gone BEFORE the baseline is read:
+        # if the collector frees it in the middle of this test the torch-side byte count drops and the deltas below lie
+        gc.collect()
         torch.cuda.synchronize(); torch.cuda.empty_cache()
         before = torch.cuda.memory_allocated()
         p = Pmc(0, torch_allocator=use_torch)
